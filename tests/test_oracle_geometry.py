@@ -327,11 +327,11 @@ def test_batches_partition_every_spot():
 
 def test_gamma_tool():
     z, y, x = np.meshgrid(np.arange(20), np.arange(20), np.arange(20), indexing="ij")
-    ref = np.exp(-((x - 10) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 30.0)
+    ref = np.exp(-((x - 10) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 120.0)
     assert orc.gamma_pass_rate(ref, ref, (1, 1, 1)) == 1.0
     assert orc.gamma_pass_rate(ref, ref * 1.005, (1, 1, 1)) == 1.0            # inside 1% dose
     assert orc.gamma_pass_rate(ref, ref * 1.2, (1, 1, 1)) < 0.9               # 20% off fails somewhere
-    shifted = np.exp(-((x - 10.5) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 30.0)
+    shifted = np.exp(-((x - 10.5) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 120.0)
     assert orc.gamma_pass_rate(ref, shifted, (1, 1, 1), dd=0.01, dta=1.0) > 0.99   # 0.5 mm shift within 1 mm DTA
-    far = np.exp(-((x - 13) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 30.0)
+    far = np.exp(-((x - 13) ** 2 + (y - 10) ** 2 + (z - 10) ** 2) / 120.0)
     assert orc.gamma_pass_rate(ref, far, (1, 1, 1), dd=0.01, dta=1.0) < 0.5
