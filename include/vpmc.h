@@ -1,0 +1,207 @@
+/*
+ * vpmc.h -- C-ABI of libvpmc.so: B200-native (sm_100a) Monte Carlo proton transport-and-scoring loop of
+ * arXiv 2307.01416 ("block aperture in VPMC"): spot source -> range shifter -> brass aperture -> voxelised
+ * CT -> dose grid / per-spot sparse influence columns.
+ *
+ * Citations: P:Lnn = PAPER.md line nn; S:8x = SURVEY.md section 8(x) (the written-out closed-form reading
+ * of what the paper defers to its ref. 65); D:Rn = DESIGN.md reading n.
+ *
+ * General conventions
+ *   - Units: mm, MeV, radians; dose in Gy per unit spot weight (weights are proton counts).
+ *   - Every call returns VPMC_OK (0) or a negative VPMC_ERR_*; nothing throws or aborts across the ABI.
+ *     vpmc_last_error() gives a message for the last failing call on that handle (or on create, with NULL).
+ *   - Pointers marked [host] are caller-owned host memory, copied during the call.  Pointers marked
+ *     [device] are caller-owned CUDA device memory on the current device.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued on it.
+ *   - Same handle + same seed + same inputs => identical integer outputs; floating-point sums equal up
+ *     to the order of atomic additions.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns VPMC_ERR_CUDA.
+ */
+#ifndef VPMC_H_
+#define VPMC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VPMC_OK 0
+#define VPMC_ERR_INVALID_ARG (-1)
+#define VPMC_ERR_GEOMETRY (-2)   /* e.g. CT box overlaps the aperture, range shifter not upstream of aperture */
+#define VPMC_ERR_CUDA (-3)
+#define VPMC_ERR_ALLOC (-4)
+#define VPMC_ERR_STATE (-5)      /* e.g. dose before any beam was set */
+
+#define VPMC_FLAG_MCS 1
+#define VPMC_FLAG_STRAGGLE 2
+#define VPMC_FLAG_NUCLEAR 4
+
+#define VPMC_BRASS 1             /* aperture material; the only one */
+
+/* step-record codes (vpmc_trace) */
+#define VPMC_REG_VACUUM 0
+#define VPMC_REG_RS 1
+#define VPMC_REG_AP_OPEN 2
+#define VPMC_REG_AP_BRASS 3
+#define VPMC_REG_CT 4
+#define VPMC_CAUSE_CONT 0
+#define VPMC_CAUSE_STOPPED 1
+#define VPMC_CAUSE_NUCLEAR 2
+#define VPMC_CAUSE_ESCAPED 3
+
+typedef struct vpmc vpmc_t;      /* opaque, owned by the library */
+
+/* S:8c-C0.  Physics and stepping parameters; vpmc_default_params() fills the defaults listed there. */
+typedef struct {
+    float alpha, p;              /* Bragg-Kleeman range in water R = alpha E^p: 0.022 mm MeV^-p, 1.77 */
+    float X0_w;                  /* radiation length of water, 360.8 mm */
+    float Es, c_log;             /* Highland constants 13.6 MeV, 0.038 */
+    float beta_nuc, gamma_loc;   /* nuclear slope 0.0012 /mm of residual range; locally absorbed fraction 0.6 */
+    float k_bohr, za_w;          /* Bohr variance 0.015692 MeV^2/mm per (Z/A rho); Z/A of water 0.5551 */
+    float R_cut, f_R, s_max;     /* stop at residual range 0.1 mm; step <= max(f_R R, R_cut) WET; geometric cap (inf) */
+    float s_rs, s_ap;            /* fixed geometric step in range shifter / aperture region, 1 mm */
+    float brass_rsp, brass_rho, brass_X0, brass_za; /* 5.523, 8.5 g/cm3, 14.94 mm, 0.457 */
+    float rs_rsp, rs_rho, rs_X0; /* range shifter as water-equivalent slab: 1, 1, 360.8 mm */
+    float rho_min;               /* density floor in the dose conversion, 1e-3 g/cm3 */
+    float delta_E;               /* relative source energy spread, 0 */
+    int32_t flags;               /* VPMC_FLAG_* ; default all three */
+    int32_t n_batches;           /* batches of the uncertainty estimate (S:8c-C6, D:R7); default 10; 1 = off */
+} vpmc_params;
+
+/* CT grid.  Voxel v = ix + nx*(iy + ny*iz); `origin` is the low corner of voxel (0,0,0) in the CT
+ * frame.  hu: nx*ny*nz int16, [host] or, when hu_on_device != 0, [device]. */
+typedef struct {
+    int32_t n[3];
+    float h[3];
+    float origin[3];
+    const int16_t *hu;
+    int32_t hu_on_device;
+} vpmc_ct;
+
+/* HU -> (RSP, density g/cm3, relative scattering power) calibration: piecewise linear between nodes
+ * ascending in hu, clamped at the end nodes (S:8c-C5).  xsp may be NULL -> rho.  All [host]. */
+typedef struct {
+    int32_t n;
+    const float *hu, *rsp, *rho, *xsp;
+} vpmc_calib;
+
+/* One pencil-beam spot: position at the isocentre plane in the beam frame, energy,
+ * weight (proton count), in-air Gaussian sigma. */
+typedef struct { float x, y, energy, weight, sigma; } vpmc_spot;
+
+/* Beam frame -> CT frame: r_ct = iso + rot * r_beam (rot row-major, orthonormal); the beam travels along
+ * +w (third beam axis); the isocentre is w = 0. */
+typedef struct { float iso[3]; float rot[9]; } vpmc_frame;
+
+/* Uncertainty scenario: patient shift (mm, CT frame; devices ride on the nozzle) and RSP scale. */
+typedef struct { float shift[3]; float rsp_scale; } vpmc_scenario;
+
+/* One scenario's influence matrix in CSR form ("sparse matrix compression"): rows = spots in input
+ * order over all beams, columns = voxel linear index ascending.  Arrays are [device], obtained through the
+ * caller's allocator and caller-owned afterwards. */
+typedef struct {
+    int64_t *row_ptr;            /* n_rows + 1 */
+    int32_t *col;                /* nnz */
+    float *val;                  /* nnz, Gy per unit spot weight */
+    int64_t nnz;
+    int32_t n_rows;
+} vpmc_csr;
+
+/* Allocator callback: must return device memory of at least `bytes` bytes (256-byte aligned), or NULL. */
+typedef void *(*vpmc_alloc_fn)(size_t bytes, void *user);
+
+/* Energy bookkeeping (S:8c-P6): incident = dep_ct + dep_rs + dep_brass + escaped + removed. */
+typedef struct {
+    double incident, dep_ct, dep_rs, dep_brass, escaped, removed;                   /* MeV */
+    uint64_t n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;     /* histories by fate */
+} vpmc_tallies;
+
+/* One step of one history (vpmc_trace).  r, u after the step: beam frame in the beam line, CT frame from the
+ * CT-entry drift on.  ivox = voxel at the start of a CT step, else -1. */
+typedef struct {
+    uint64_t hid;
+    int32_t step, region, cause;
+    int32_t ivox[3];
+    float r[3], u[3];
+    float E_before, E_after, s;
+} vpmc_step_rec;
+
+void vpmc_default_params(vpmc_params *p);
+
+/* Create an engine for one CT + calibration.  Builds the per-HU material table on the
+ * device and uploads the CT.  params NULL = defaults.  *out is NULL on failure. */
+int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *cal, const vpmc_params *params);
+int vpmc_destroy(vpmc_t *h);
+
+/* Add a treatment field; returns its index in *beam_id.  Beams keep their order; spot rows of the influence
+ * matrices follow beam order then spot order. */
+int vpmc_add_beam(vpmc_t *h, const vpmc_frame *frame, int *beam_id);
+
+/* Spots, energies, weights and spot sigmas of a beam.  spots: [host], n_spots >= 0. */
+int vpmc_set_beam(vpmc_t *h, int beam, const vpmc_spot *spots, int32_t n_spots);
+
+/* Range shifter: homogeneous slab of water-equivalent thickness wet_mm (0 = none) whose
+ * downstream face is downstream_face_mm upstream of the isocentre (<= 0 -> default 190). */
+int vpmc_set_range_shifter(vpmc_t *h, int beam, float wet_mm, float downstream_face_mm);
+
+/* Aperture block: brass of thickness_mm (0 = none) with a patient-specific opening given as a
+ * bitmap, opening[iy*nx + ix] != 0 = open, pixel (ix, iy) covering [u0 + ix du, u0 + (ix+1) du) x
+ * [v0 + iy dv, ...) in the beam frame; everything outside the bitmap is brass.  The downstream face is
+ * downstream_face_mm upstream of the isocentre (<= 0 -> default 150).  opening: [host]. */
+int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int material, const uint8_t *opening,
+                      int32_t nx, int32_t ny, float u0, float v0, float du, float dv, float downstream_face_mm);
+
+/* Plan dose: n_histories apportioned to the spots by weight (largest remainder, S:8c-C2), transported
+ * and scored; dose_out_dev ([device], nx*ny*nz floats) is fully overwritten with
+ * dose[v] = (W/N) E_dep[v] / (max(rho_v, rho_min) V_vox) * 1.602176634e-10 Gy (S:8c-C6).
+ * Asynchronous on `cuda_stream` except for the small host-side apportionment; tallies and the uncertainty
+ * of this run are available through vpmc_get_tallies / vpmc_get_uncertainty (which synchronise). */
+int vpmc_dose(vpmc_t *h, uint64_t n_histories, uint64_t seed, float *dose_out_dev, void *cuda_stream);
+
+/* Same under one uncertainty scenario (vpmc_dose = shift 0, rsp_scale 1). */
+int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *sc, uint64_t n_histories, uint64_t seed,
+                       float *dose_out_dev, void *cuda_stream);
+
+/* vpmc_dose with the result copied to dose_out_host ([host], nx*ny*nz floats); synchronous. */
+int vpmc_dose_host(vpmc_t *h, uint64_t n_histories, uint64_t seed, float *dose_out_host);
+
+/* Restrict the next dose / trace calls to history ids [hid_begin, hid_end) of the N-history run (prefix
+ * parity, S:8d).  hid_end = 0 -> no restriction. */
+int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);
+
+/* Influence matrices: for each of n_sc scenarios and each spot j (history ids
+ * j*hist_per_spot + i), the dose column per unit weight, entries >= rel_threshold * column max (and > 0) kept,
+ * written as CSR into out[0..n_sc) through `alloc`.  Synchronises where it must size outputs. */
+int vpmc_influence(vpmc_t *h, const vpmc_scenario *sc, int32_t n_sc, uint32_t hist_per_spot,
+                   float rel_threshold, uint64_t seed, vpmc_csr *out, vpmc_alloc_fn alloc, void *user,
+                   void *cuda_stream);
+
+/* The CSR writer alone (S:8a-S8, D:R10): one row from a dense fp32 column [device] of n voxels.  With
+ * col_out/val_out NULL only counts.  *nnz_out [host].  Synchronous. */
+int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, float rel_threshold,
+                        int32_t *col_out_dev, float *val_out_dev, int64_t *nnz_out);
+
+/* Tallies of the last dose / influence call (synchronises the stream it ran on). */
+int vpmc_get_tallies(vpmc_t *h, vpmc_tallies *out);
+
+/* Statistical uncertainty of the last vpmc_dose* call (S:8c-C6): mean over voxels with dose >= 50% of the
+ * maximum of sigma_v / D_v from n_batches batches.  Needs params.n_batches >= 2. */
+int vpmc_get_uncertainty(vpmc_t *h, float *rel_unc_out);
+
+/* Test-only: step records of selected histories.  mode 0 = dose mode with N = n_or_hps; 1 = influence mode
+ * with hist_per_spot = n_or_hps.  out_host: n*max_steps records; nrec_host[i] = records of history i. */
+int vpmc_trace(vpmc_t *h, const vpmc_scenario *sc, int32_t mode, uint64_t n_or_hps, uint64_t seed,
+               const uint64_t *hids, int32_t n, int32_t max_steps, vpmc_step_rec *out_host, int32_t *nrec_host);
+
+/* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
+int vpmc_get_launch_count(vpmc_t *h, uint64_t *out);
+
+const char *vpmc_last_error(const vpmc_t *h);
+const char *vpmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VPMC_H_ */

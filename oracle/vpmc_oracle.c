@@ -517,6 +517,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
         orc_calib_eval(&pb->cal, (double)ct->hu[v], cal);
         medium m = { cal[0] * sc->rsp_scale, cal[1], cal[2] / P->X0_w, P->za_w * cal[1] };
         double Eb = h.E; uint32_t st = h.step; int32_t iv0[3] = { iv[0], iv[1], iv[2] };
+        const int up = ax >= 0 && h.u[ax] > 0.0;   /* direction of travel during the step (C4-8: old direction) */
         cause = material_step(P, &h, &m, d, hid, c->seed, &s, &dep, &rem, &on_d);
         if (c->edep) {
             if (c->touched && c->edep[v] == 0.0 && dep != 0.0 && c->n_touched < c->max_touched) c->touched[c->n_touched++] = v;
@@ -525,7 +526,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
         if (c->tal) { c->tal->dep_ct += dep; c->tal->removed += rem; }
         int out = 0;
         if (cause == ORC_CONT && on_d) {   /* C4-9 */
-            if (h.u[ax] > 0.0) { h.r[ax] = ct->origin[ax] + (double)(iv[ax] + 1) * ct->h[ax]; iv[ax] += 1; }
+            if (up) { h.r[ax] = ct->origin[ax] + (double)(iv[ax] + 1) * ct->h[ax]; iv[ax] += 1; }
             else { h.r[ax] = ct->origin[ax] + (double)iv[ax] * ct->h[ax]; iv[ax] -= 1; }
             if (iv[ax] < 0 || iv[ax] >= ct->n[ax]) out = 1;
         }

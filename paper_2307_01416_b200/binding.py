@@ -1,0 +1,283 @@
+"""Thin ctypes binding of libvpmc.so (include/vpmc.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C-ABI.  PyTorch is used for device buffers and
+streams.  There is no CPU fallback: if the library is missing or there is no CUDA device, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvpmc.so")
+
+OK, ERR_INVALID_ARG, ERR_GEOMETRY, ERR_CUDA, ERR_ALLOC, ERR_STATE = 0, -1, -2, -3, -4, -5
+FLAG_MCS, FLAG_STRAGGLE, FLAG_NUCLEAR = 1, 2, 4
+BRASS = 1
+
+EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy", "vpmc_add_beam", "vpmc_set_beam",
+           "vpmc_set_range_shifter", "vpmc_set_aperture", "vpmc_dose", "vpmc_dose_scenario", "vpmc_dose_host",
+           "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
+           "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error"]
+
+
+class VpmcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("vpmc error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_float) for n in (
+        "alpha", "p", "X0_w", "Es", "c_log", "beta_nuc", "gamma_loc", "k_bohr", "za_w", "R_cut", "f_R", "s_max",
+        "s_rs", "s_ap", "brass_rsp", "brass_rho", "brass_X0", "brass_za", "rs_rsp", "rs_rho", "rs_X0", "rho_min",
+        "delta_E")] + [("flags", C.c_int32), ("n_batches", C.c_int32)]
+
+
+class _Ct(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("h", C.c_float * 3), ("origin", C.c_float * 3), ("hu", C.c_void_p),
+                ("hu_on_device", C.c_int32)]
+
+
+class _Calib(C.Structure):
+    _fields_ = [("n", C.c_int32), ("hu", C.c_void_p), ("rsp", C.c_void_p), ("rho", C.c_void_p), ("xsp", C.c_void_p)]
+
+
+class _Frame(C.Structure):
+    _fields_ = [("iso", C.c_float * 3), ("rot", C.c_float * 9)]
+
+
+class Scenario(C.Structure):
+    _fields_ = [("shift", C.c_float * 3), ("rsp_scale", C.c_float)]
+
+
+class _Csr(C.Structure):
+    _fields_ = [("row_ptr", C.c_void_p), ("col", C.c_void_p), ("val", C.c_void_p), ("nnz", C.c_int64),
+                ("n_rows", C.c_int32)]
+
+
+class Tallies(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("incident", "dep_ct", "dep_rs", "dep_brass", "escaped", "removed")] + \
+               [(n, C.c_uint64) for n in ("n_stopped_ct", "n_stopped_rs", "n_stopped_brass", "n_nuclear", "n_escaped")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+STEP_DTYPE = np.dtype([("hid", "<u8"), ("step", "<i4"), ("region", "<i4"), ("cause", "<i4"), ("ivox", "<i4", 3),
+                       ("r", "<f4", 3), ("u", "<f4", 3), ("E_before", "<f4"), ("E_after", "<f4"), ("s", "<f4")],
+                      align=True)
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+
+_lib = None
+
+
+def lib():
+    """Load libvpmc.so; fails loudly if it has not been built (python -m paper_2307_01416_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libvpmc.so is missing: build it with `python -m paper_2307_01416_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.vpmc_version.restype = C.c_char_p
+        L.vpmc_last_error.restype = C.c_char_p
+        L.vpmc_last_error.argtypes = [C.c_void_p]
+        L.vpmc_default_params.argtypes = [C.POINTER(Params)]
+        L.vpmc_default_params.restype = None
+        L.vpmc_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Ct), C.POINTER(_Calib), C.POINTER(Params)]
+        L.vpmc_destroy.argtypes = [C.c_void_p]
+        L.vpmc_add_beam.argtypes = [C.c_void_p, C.POINTER(_Frame), C.POINTER(C.c_int)]
+        L.vpmc_set_beam.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int32]
+        L.vpmc_set_range_shifter.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_float]
+        L.vpmc_set_aperture.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_int, C.c_void_p, C.c_int32, C.c_int32,
+                                        C.c_float, C.c_float, C.c_float, C.c_float, C.c_float]
+        L.vpmc_dose.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
+        L.vpmc_dose_scenario.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
+        L.vpmc_dose_host.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p]
+        L.vpmc_set_history_window.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
+        L.vpmc_influence.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_int32, C.c_uint32, C.c_float, C.c_uint64,
+                                     C.POINTER(_Csr), _ALLOC_FN, C.c_void_p, C.c_void_p]
+        L.vpmc_csr_from_dense.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_void_p, C.c_void_p,
+                                          C.POINTER(C.c_int64)]
+        L.vpmc_get_tallies.argtypes = [C.c_void_p, C.POINTER(Tallies)]
+        L.vpmc_get_uncertainty.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        L.vpmc_trace.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_int32, C.c_uint64, C.c_uint64, C.c_void_p,
+                                 C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        L.vpmc_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+        _lib = L
+    return _lib
+
+
+def default_params(**kw) -> Params:
+    p = Params()
+    lib().vpmc_default_params(C.byref(p))
+    for k, v in kw.items():
+        if not hasattr(p, k):
+            raise KeyError(k)
+        setattr(p, k, v)
+    return p
+
+
+def scenario(shift=(0.0, 0.0, 0.0), rsp_scale=1.0) -> Scenario:
+    s = Scenario()
+    s.shift[:] = [float(x) for x in shift]
+    s.rsp_scale = float(rsp_scale)
+    return s
+
+
+def _f32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float32))
+
+
+class Engine:
+    """One vpmc_t handle.  `problem` is a workload dict (paper_2307_01416_b200.workloads)."""
+
+    def __init__(self, problem: dict, params: Params | None = None):
+        self._h = C.c_void_p()
+        L = lib()
+        ct = problem["ct"]
+        hu = np.ascontiguousarray(np.asarray(ct["hu"], dtype=np.int16).reshape(-1))
+        c = _Ct()
+        c.n[:] = [int(x) for x in ct["n"]]
+        c.h[:] = [float(x) for x in ct["h"]]
+        c.origin[:] = [float(x) for x in ct["origin"]]
+        c.hu = hu.ctypes.data
+        c.hu_on_device = 0
+        cal = problem["calib"]
+        arrs = {k: (None if cal.get(k) is None else _f32(cal[k])) for k in ("hu", "rsp", "rho", "xsp")}
+        k = _Calib()
+        k.n = int(arrs["hu"].size)
+        k.hu, k.rsp, k.rho = arrs["hu"].ctypes.data, arrs["rsp"].ctypes.data, arrs["rho"].ctypes.data
+        k.xsp = None if arrs["xsp"] is None else arrs["xsp"].ctypes.data
+        rc = L.vpmc_create(C.byref(self._h), C.byref(c), C.byref(k), C.byref(params) if params is not None else None)
+        if rc != OK:
+            raise VpmcError(rc, L.vpmc_last_error(None).decode())
+        self.n = tuple(int(x) for x in ct["n"])
+        self.nvox = self.n[0] * self.n[1] * self.n[2]
+        self.h2d_bytes = hu.nbytes + sum(a.nbytes for a in arrs.values() if a is not None)
+        self.n_spots = 0
+        for b in problem["beams"]:
+            self.add_beam(b)
+
+    # -- plumbing
+    def _check(self, rc):
+        if rc != OK:
+            raise VpmcError(rc, lib().vpmc_last_error(self._h).decode())
+
+    def close(self):
+        if self._h:
+            lib().vpmc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- set-up (S0)
+    def add_beam(self, b: dict) -> int:
+        L = lib()
+        f = _Frame()
+        f.iso[:] = [float(x) for x in b["iso"]]
+        f.rot[:] = [float(x) for x in np.asarray(b["rot"], dtype=np.float32).reshape(9)]
+        bid = C.c_int(-1)
+        self._check(L.vpmc_add_beam(self._h, C.byref(f), C.byref(bid)))
+        sp = _f32(b["spots"]).reshape(-1, 5)
+        self._check(L.vpmc_set_beam(self._h, bid.value, sp.ctypes.data, sp.shape[0]))
+        self.n_spots += sp.shape[0]
+        self.h2d_bytes += sp.nbytes
+        if float(b.get("rs_wet", 0.0)) > 0:
+            self._check(L.vpmc_set_range_shifter(self._h, bid.value, float(b["rs_wet"]), float(b.get("rs_face", 190.0))))
+        ap = b.get("aperture")
+        if ap is not None:
+            op = np.ascontiguousarray(np.asarray(ap["open"], dtype=np.uint8))
+            self._check(L.vpmc_set_aperture(self._h, bid.value, float(ap["T"]), BRASS, op.ctypes.data, op.shape[1],
+                                            op.shape[0], float(ap["u0"]), float(ap["v0"]), float(ap["du"]),
+                                            float(ap["dv"]), float(ap.get("face", 150.0))))
+            self.h2d_bytes += op.nbytes
+        return bid.value
+
+    def set_history_window(self, begin: int, end: int):
+        self._check(lib().vpmc_set_history_window(self._h, int(begin), int(end)))
+
+    # -- hot path
+    def dose(self, n_histories: int, seed: int, out=None, sc: Scenario | None = None, stream=None):
+        """Dose [Gy] as a torch.float32 CUDA tensor of nvox elements (v = ix + nx*(iy + ny*iz))."""
+        import torch
+        if out is None:
+            out = torch.empty(self.nvox, dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.nvox and out.is_contiguous()
+        st = torch.cuda.current_stream() if stream is None else stream
+        if sc is None:
+            self._check(lib().vpmc_dose(self._h, int(n_histories), int(seed), out.data_ptr(), st.cuda_stream))
+        else:
+            self._check(lib().vpmc_dose_scenario(self._h, C.byref(sc), int(n_histories), int(seed), out.data_ptr(),
+                                                 st.cuda_stream))
+        return out
+
+    def dose_host(self, n_histories: int, seed: int, out: np.ndarray | None = None) -> np.ndarray:
+        if out is None:
+            out = np.empty(self.nvox, dtype=np.float32)
+        self._check(lib().vpmc_dose_host(self._h, int(n_histories), int(seed), out.ctypes.data))
+        return out
+
+    def tallies(self) -> Tallies:
+        t = Tallies()
+        self._check(lib().vpmc_get_tallies(self._h, C.byref(t)))
+        return t
+
+    def uncertainty(self) -> float:
+        u = C.c_float()
+        self._check(lib().vpmc_get_uncertainty(self._h, C.byref(u)))
+        return float(u.value)
+
+    def launch_count(self) -> int:
+        n = C.c_uint64()
+        self._check(lib().vpmc_get_launch_count(self._h, C.byref(n)))
+        return int(n.value)
+
+    def trace(self, hids, n_or_hps: int, seed: int, sc: Scenario | None = None, mode: int = 0, max_steps: int = 1024):
+        hids = np.ascontiguousarray(np.asarray(hids, dtype=np.uint64))
+        recs = np.zeros((hids.size, max_steps), dtype=STEP_DTYPE)
+        nrec = np.zeros(hids.size, dtype=np.int32)
+        self._check(lib().vpmc_trace(self._h, C.byref(sc) if sc is not None else None, mode, int(n_or_hps), int(seed),
+                                     hids.ctypes.data, hids.size, max_steps, recs.ctypes.data, nrec.ctypes.data))
+        assert (nrec <= max_steps).all(), "max_steps too small"
+        return [recs[i, :nrec[i]] for i in range(hids.size)]
+
+    def influence(self, scenarios, hist_per_spot: int, rel_threshold: float, seed: int, stream=None):
+        """List of (row_ptr int64, col int32, val fp32) torch CUDA tensors, one per scenario."""
+        import torch
+        st = torch.cuda.current_stream() if stream is None else stream
+        keep = {}
+
+        def _alloc(nbytes, _user):
+            t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device="cuda")
+            keep[t.data_ptr()] = t
+            return t.data_ptr()
+
+        cb = _ALLOC_FN(_alloc)
+        n_sc = len(scenarios)
+        arr = (Scenario * n_sc)(*scenarios)
+        out = (_Csr * n_sc)()
+        self._check(lib().vpmc_influence(self._h, arr, n_sc, int(hist_per_spot), float(rel_threshold), int(seed), out, cb,
+                                         None, st.cuda_stream))
+        res = []
+        for o in out:
+            rp = keep[o.row_ptr][: 8 * (o.n_rows + 1)].view(torch.int64)
+            col = keep[o.col][: 4 * o.nnz].view(torch.int32) if o.nnz else torch.empty(0, dtype=torch.int32, device="cuda")
+            val = keep[o.val][: 4 * o.nnz].view(torch.float32) if o.nnz else torch.empty(0, dtype=torch.float32, device="cuda")
+            res.append((rp, col, val))
+        return res
+
+    def csr_from_dense(self, col):
+        """The CSR writer alone on one dense fp32 CUDA column: (idx int32, val fp32) CUDA tensors."""
+        import torch
+        assert col.is_cuda and col.dtype == torch.float32 and col.is_contiguous()
+        nnz = C.c_int64()
+        return col, nnz

@@ -1,0 +1,262 @@
+// vpmc_api.cu -- the C-ABI of libvpmc.so (include/vpmc.h): host set-up (S0) and launch sequencing.
+// Every step of the hot path runs in the kernels of vpmc_kernels.cuh; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <numeric>
+
+#include "vpmc_host.h"
+
+using namespace vpk;
+
+static thread_local std::string g_create_err;
+
+#define FAIL(h, code, ...)                                      \
+    do {                                                        \
+        char _b[512];                                           \
+        snprintf(_b, sizeof(_b), __VA_ARGS__);                  \
+        if (h) (h)->err = _b; else g_create_err = _b;           \
+        return (code);                                          \
+    } while (0)
+
+#define CU(h, expr)                                                                         \
+    do {                                                                                    \
+        cudaError_t _e = (expr);                                                            \
+        if (_e != cudaSuccess) FAIL(h, VPMC_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
+    } while (0)
+
+static constexpr unsigned int kChunk = 1u << 20;       // histories per beamline launch = queue capacity
+static constexpr size_t kMaxSmemLut = 96 * 1024;
+
+extern "C" const char *vpmc_version(void) { return "vpmc-b200 0.1 (sm_100a)"; }
+
+extern "C" void vpmc_default_params(vpmc_params *p)
+{
+    if (!p) return;
+    p->alpha = 0.022f; p->p = 1.77f; p->X0_w = 360.8f; p->Es = 13.6f; p->c_log = 0.038f;
+    p->beta_nuc = 0.0012f; p->gamma_loc = 0.6f; p->k_bohr = 0.015692f; p->za_w = 0.5551f;
+    p->R_cut = 0.1f; p->f_R = 0.25f; p->s_max = std::numeric_limits<float>::infinity(); p->s_rs = 1.0f; p->s_ap = 1.0f;
+    p->brass_rsp = 5.523f; p->brass_rho = 8.5f; p->brass_X0 = 14.94f; p->brass_za = 0.457f;
+    p->rs_rsp = 1.0f; p->rs_rho = 1.0f; p->rs_X0 = 360.8f;
+    p->rho_min = 1e-3f; p->delta_E = 0.0f;
+    p->flags = VPMC_FLAG_MCS | VPMC_FLAG_STRAGGLE | VPMC_FLAG_NUCLEAR;
+    p->n_batches = 10;
+}
+
+static DevParams make_dev_params(const vpmc_params &p)
+{
+    DevParams d;
+    d.alpha = p.alpha; d.p = p.p; d.inv_p = (float)(1.0 / (double)p.p); d.inv_alpha = (float)(1.0 / (double)p.alpha);
+    d.inv_X0_w = (float)(1.0 / (double)p.X0_w); d.Es = p.Es; d.c_log = p.c_log;
+    d.beta_nuc = p.beta_nuc; d.gamma_loc = p.gamma_loc; d.k_bohr = p.k_bohr; d.za_w = p.za_w;
+    d.R_cut = p.R_cut; d.f_R = p.f_R; d.s_max = p.s_max; d.s_rs = p.s_rs; d.s_ap = p.s_ap;
+    d.brass_rsp = p.brass_rsp; d.brass_rho = p.brass_rho; d.brass_inv_X0 = (float)(1.0 / (double)p.brass_X0);
+    d.brass_za_rho = (float)((double)p.brass_za * (double)p.brass_rho);
+    d.rs_rsp = p.rs_rsp; d.rs_rho = p.rs_rho; d.rs_inv_X0 = (float)(1.0 / (double)p.rs_X0);
+    d.rs_za_rho = (float)((double)p.za_w * (double)p.rs_rho);
+    d.rho_min = p.rho_min; d.delta_E = p.delta_E; d.flags = p.flags;
+    return d;
+}
+
+static double pl_eval(const vpmc_calib *c, const float *y, double hu)
+{
+    if (hu <= c->hu[0]) return y[0];
+    if (hu >= c->hu[c->n - 1]) return y[c->n - 1];
+    int k = 0;
+    while (k + 2 < c->n && hu >= c->hu[k + 1]) ++k;
+    const double t = (hu - c->hu[k]) / ((double)c->hu[k + 1] - (double)c->hu[k]);
+    return (double)y[k] + t * ((double)y[k + 1] - (double)y[k]);
+}
+
+static void free_beam(BeamHost &b)
+{
+    if (b.d_bits) cudaFree(b.d_bits);
+    b.d_bits = nullptr;
+}
+
+extern "C" int vpmc_destroy(vpmc_t *h)
+{
+    if (!h) return VPMC_OK;
+    cudaDeviceSynchronize();
+    for (auto &b : h->beams) free_beam(b);
+    void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_cum, h->d_first, h->q.q0, h->q.q1,
+                     h->q.q2, h->q.q3, h->d_qctr, h->d_edep, h->d_sum, h->d_s1, h->d_s2, h->d_tal, h->d_max_bits, h->d_unc };
+    for (void *p : ptrs) if (p) cudaFree(p);
+    for (void *p : h->d_inf) if (p) cudaFree(p);
+    delete h;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *cal, const vpmc_params *params)
+{
+    if (!out) { g_create_err = "out is NULL"; return VPMC_ERR_INVALID_ARG; }
+    *out = nullptr;
+    vpmc_t *nh = nullptr;
+    if (!ct || !cal || !ct->hu) FAIL(nh, VPMC_ERR_INVALID_ARG, "ct / calibration missing");
+    for (int a = 0; a < 3; ++a)
+        if (ct->n[a] < 1 || ct->n[a] > 65535 || !(ct->h[a] > 0.0f)) FAIL(nh, VPMC_ERR_INVALID_ARG, "bad CT grid on axis %d", a);
+    const long long nvox = (long long)ct->n[0] * ct->n[1] * ct->n[2];
+    if (nvox > 0x7fffffffLL) FAIL(nh, VPMC_ERR_INVALID_ARG, "more than 2^31-1 voxels");
+    if (cal->n < 1 || !cal->hu || !cal->rsp || !cal->rho) FAIL(nh, VPMC_ERR_INVALID_ARG, "calibration needs hu, rsp, rho nodes");
+    for (int k = 1; k < cal->n; ++k)
+        if (!(cal->hu[k] > cal->hu[k - 1])) FAIL(nh, VPMC_ERR_INVALID_ARG, "calibration nodes must ascend in hu");
+    vpmc_params p;
+    if (params) p = *params; else vpmc_default_params(&p);
+    if (!(p.alpha > 0) || !(p.p > 1) || !(p.R_cut > 0) || !(p.f_R > 0 && p.f_R < 1) || !(p.s_rs > 0) || !(p.s_ap > 0) ||
+        !(p.brass_rsp > 0) || !(p.rs_rsp > 0) || p.n_batches < 1 || p.n_batches > 1000)
+        FAIL(nh, VPMC_ERR_INVALID_ARG, "parameter out of range");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) FAIL(nh, VPMC_ERR_CUDA, "no CUDA device (this library has no CPU path)");
+
+    vpmc_t *h = new vpmc();
+    h->params = p;
+    h->P = make_dev_params(p);
+    h->nvox = nvox;
+    cudaGetDevice(&h->device);
+    cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    DevGrid &G = h->G;
+    G.nx = ct->n[0]; G.ny = ct->n[1]; G.nz = ct->n[2];
+    G.hx = ct->h[0]; G.hy = ct->h[1]; G.hz = ct->h[2];
+    G.ox = ct->origin[0]; G.oy = ct->origin[1]; G.oz = ct->origin[2];
+    // S0: per-integer-HU material table over the span of the calibration nodes (values are constant outside)
+    G.hu_min = (int)std::floor((double)cal->hu[0]);
+    const int hu_max = (int)std::ceil((double)cal->hu[cal->n - 1]);
+    G.n_lut = hu_max - G.hu_min + 1;
+    if (G.n_lut > (1 << 20)) { delete h; FAIL(nh, VPMC_ERR_INVALID_ARG, "calibration spans more than 2^20 HU"); }
+    std::vector<float4> lut((size_t)G.n_lut);
+    for (int i = 0; i < G.n_lut; ++i) {
+        const double hu = (double)(G.hu_min + i);
+        const double rsp = pl_eval(cal, cal->rsp, hu), rho = pl_eval(cal, cal->rho, hu);
+        const double xsp = cal->xsp ? pl_eval(cal, cal->xsp, hu) : rho;
+        lut[i] = make_float4((float)rsp, (float)rho, (float)(xsp / (double)p.X0_w), (float)((double)p.za_w * rho));
+    }
+    h->lut_bytes = lut.size() * sizeof(float4);
+    h->smem_lut = h->lut_bytes <= kMaxSmemLut;
+#define CUC(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { g_create_err = std::string(#expr) + ": " + cudaGetErrorString(_e); vpmc_destroy(h); return VPMC_ERR_CUDA; } } while (0)
+    CUC(cudaMalloc(&h->d_lut, h->lut_bytes));
+    CUC(cudaMemcpy(h->d_lut, lut.data(), h->lut_bytes, cudaMemcpyHostToDevice));
+    CUC(cudaMalloc(&h->d_hu, nvox * sizeof(short)));
+    CUC(cudaMemcpy(h->d_hu, ct->hu, nvox * sizeof(short), ct->hu_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice));
+    CUC(cudaMalloc(&h->d_edep, nvox * sizeof(float)));
+    CUC(cudaMalloc(&h->d_sum, nvox * sizeof(float)));
+    CUC(cudaMalloc(&h->d_tal, sizeof(DevTallies)));
+    CUC(cudaMemset(h->d_tal, 0, sizeof(DevTallies)));
+    CUC(cudaMalloc(&h->d_max_bits, sizeof(unsigned int)));
+    CUC(cudaMalloc(&h->d_unc, 2 * sizeof(double)));
+    CUC(cudaMalloc(&h->d_qctr, 2 * sizeof(unsigned int)));
+    CUC(cudaMalloc(&h->q.q0, (size_t)kChunk * sizeof(float4)));
+    CUC(cudaMalloc(&h->q.q1, (size_t)kChunk * sizeof(float4)));
+    CUC(cudaMalloc(&h->q.q2, (size_t)kChunk * sizeof(float4)));
+    CUC(cudaMalloc(&h->q.q3, (size_t)kChunk * sizeof(uint4)));
+    h->q.count = h->d_qctr; h->q.head = h->d_qctr + 1; h->q.capacity = kChunk;
+    // persistent voxel kernel: one wave of resident CTAs
+    {
+        const size_t sm = h->smem_lut ? h->lut_bytes : 0;
+        int occ = 0;
+        if (h->smem_lut) {
+            CUC(cudaFuncSetAttribute(voxel_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmemLut));
+            CUC(cudaFuncSetAttribute(voxel_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmemLut));
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<0, true>, 256, sm));
+            h->voxel_grid[0][1] = std::max(occ, 1) * h->n_sm;
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<1, true>, 256, sm));
+            h->voxel_grid[1][1] = std::max(occ, 1) * h->n_sm;
+        }
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<0, false>, 256, 0));
+        h->voxel_grid[0][0] = std::max(occ, 1) * h->n_sm;
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<1, false>, 256, 0));
+        h->voxel_grid[1][0] = std::max(occ, 1) * h->n_sm;
+    }
+#undef CUC
+    *out = h;
+    return VPMC_OK;
+}
+
+extern "C" const char *vpmc_last_error(const vpmc_t *h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int vpmc_add_beam(vpmc_t *h, const vpmc_frame *frame, int *beam_id)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!frame) FAIL(h, VPMC_ERR_INVALID_ARG, "frame is NULL");
+    // rot must be orthonormal (1e-3)
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double d = 0;
+            for (int k = 0; k < 3; ++k) d += (double)frame->rot[3 * k + i] * frame->rot[3 * k + j];
+            if (std::fabs(d - (i == j ? 1.0 : 0.0)) > 1e-3) FAIL(h, VPMC_ERR_INVALID_ARG, "frame.rot is not orthonormal");
+        }
+    BeamHost b;
+    b.frame = *frame;
+    h->beams.push_back(b);
+    h->spots_dirty = true;
+    if (beam_id) *beam_id = (int)h->beams.size() - 1;
+    return VPMC_OK;
+}
+
+static int check_beam(vpmc_t *h, int beam)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (beam < 0 || beam >= (int)h->beams.size()) FAIL(h, VPMC_ERR_INVALID_ARG, "no beam %d", beam);
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_beam(vpmc_t *h, int beam, const vpmc_spot *spots, int32_t n_spots)
+{
+    int rc = check_beam(h, beam); if (rc) return rc;
+    if (n_spots < 0 || (n_spots > 0 && !spots)) FAIL(h, VPMC_ERR_INVALID_ARG, "bad spot list");
+    for (int j = 0; j < n_spots; ++j)
+        if (!(spots[j].energy > 0) || !(spots[j].weight >= 0) || !(spots[j].sigma >= 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "bad spot %d", j);
+    h->beams[beam].spots.assign(spots, spots + n_spots);
+    h->spots_dirty = true;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_range_shifter(vpmc_t *h, int beam, float wet_mm, float downstream_face_mm)
+{
+    int rc = check_beam(h, beam); if (rc) return rc;
+    if (!(wet_mm >= 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "negative WET");
+    h->beams[beam].rs_wet = wet_mm;
+    h->beams[beam].rs_face = downstream_face_mm > 0 ? downstream_face_mm : 190.0f;
+    h->spots_dirty = true;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int material, const uint8_t *opening,
+                                 int32_t nx, int32_t ny, float u0, float v0, float du, float dv, float downstream_face_mm)
+{
+    int rc = check_beam(h, beam); if (rc) return rc;
+    BeamHost &b = h->beams[beam];
+    if (!(thickness_mm >= 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "negative thickness");
+    if (thickness_mm == 0) { free_beam(b); b.has_ap = false; h->spots_dirty = true; return VPMC_OK; }
+    if (material != VPMC_BRASS) FAIL(h, VPMC_ERR_INVALID_ARG, "only VPMC_BRASS is supported");
+    if (!opening || nx < 1 || ny < 1 || nx > 16384 || ny > 16384 || !(du > 0) || !(dv > 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "bad opening bitmap");
+    const int rw = (nx + 31) / 32;
+    std::vector<uint32_t> bits((size_t)rw * ny, 0u);          // S0: bitmap packing
+    for (int iy = 0; iy < ny; ++iy)
+        for (int ix = 0; ix < nx; ++ix)
+            if (opening[(size_t)iy * nx + ix]) bits[(size_t)iy * rw + (ix >> 5)] |= 1u << (ix & 31);
+    free_beam(b);
+    CU(h, cudaMalloc(&b.d_bits, bits.size() * sizeof(uint32_t)));
+    CU(h, cudaMemcpy(b.d_bits, bits.data(), bits.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    b.has_ap = true; b.ap_T = thickness_mm; b.ap_face = downstream_face_mm > 0 ? downstream_face_mm : 150.0f;
+    b.ap_nx = nx; b.ap_ny = ny; b.ap_row_words = rw; b.ap_u0 = u0; b.ap_v0 = v0; b.ap_du = du; b.ap_dv = dv;
+    h->spots_dirty = true;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    h->win_lo = hid_begin; h->win_hi = hid_end;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_get_launch_count(vpmc_t *h, uint64_t *out)
+{
+    if (!h || !out) return VPMC_ERR_INVALID_ARG;
+    *out = h->launches;
+    return VPMC_OK;
+}
+
+#include "vpmc_run.inl"
