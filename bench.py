@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- histories/s of the VPMC hot path on B200 (BASELINE.json metric) + seconds per dose at 0.5 %.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A "step" is one pass of the whole hot path (S1-S6b + dose conversion + batch-uncertainty passes) over one batch of
+synthetic input: the 8 plans of BASELINE.json configs[1] (water 100x100x150 @ 2 mm, 30 mm brass with a 1/2/3/4 cm
+opening, each with and without a 45 mm WET range shifter, 825-3993 spots, 10^7 histories per plan = 8x10^7 per step).
+`value` = histories/s with every input resident in HBM; `e2e` = the same through the C-ABI with host buffers
+(vpmc_create + set_* from pinned host arrays, vpmc_dose_host back to pinned host memory, vpmc_destroy).
+N > 1 (torchrun): every rank runs the same plans under its own Philox key (weak scaling) and the dose grids are
+averaged with one NCCL all-reduce per plan.  `--impl reference` times the CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "proton histories/s"
+SEED = 2
+# dominant kernel = voxel_kernel; ALU-bound.  Thread-instructions per CT step, from the committed
+# ncu capture (profiles/): smsp__thread_inst_executed.sum / CT steps of the launch.
+INST_PER_CT_STEP = 530.0
+ALG_BYTES_PER_CT_STEP = 10.0           # 2 B HU read + 4 B read + 4 B write of the dose add
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is not None:
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 8 or not c[0].isdigit() or int(c[0]) != self.idx:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[4:8]):
+                if v == "Active":
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def pinned(a):
+    """numpy view of a pinned host copy of array a."""
+    import torch
+    t = torch.from_numpy(a.copy()).pin_memory()
+    return t.numpy()
+
+
+def pin_problem(w):
+    w = dict(w)
+    w["ct"] = dict(w["ct"]); w["ct"]["hu"] = pinned(w["ct"]["hu"])
+    beams = []
+    for b in w["beams"]:
+        b = dict(b); b["spots"] = pinned(b["spots"])
+        if b.get("aperture") is not None:
+            b["aperture"] = dict(b["aperture"]); b["aperture"]["open"] = pinned(b["aperture"]["open"])
+        beams.append(b)
+    w["beams"] = beams
+    return w
+
+
+def run_reference(args):
+    """The CPU oracle on the same workload/metric; each step = a bounded sample of the plans."""
+    from oracle import cpu_bench
+    from paper_2307_01416_b200 import workloads as wl
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    plans = wl.config2_plans()
+    per_plan = args.ref_sample // len(plans)
+    rates, cores = [], cpu_bench.n_cores()
+    t_all = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        done, busy = 0, 0.0
+        for (d, rs) in plans:
+            r, cores, _ = cpu_bench.time_oracle("config2", {"opening_mm": d, "range_shifter": rs}, args.histories, SEED, per_plan)
+            busy += per_plan / r
+            done += per_plan
+        if it >= args.warmup:
+            rates.append(done / busy)
+            t_all.append(time.perf_counter() - t0)
+    v = sum(rates) / len(rates)
+    sample = "%d histories per plan over %d plans per step, ids spread over the %d-history run" % (per_plan, len(plans), args.histories)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "histories/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(t_all) / len(t_all), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: 8 water-phantom plans, bounded sample", "histories_per_plan": args.histories},
+        "cpu_baseline": {"value": v, "unit": "histories/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "histories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200")
+    ap.add_argument("--histories", type=int, default=10_000_000, help="histories per plan (BASELINE.json: 1e7)")
+    ap.add_argument("--ref-sample", type=int, default=800_000, help="oracle histories per reference step")
+    ap.add_argument("--cpu-sample", type=int, default=1_600_000, help="oracle histories of the cpu_baseline leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-dose-at-unc", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    run_b200(args)
+
+
+# run_b200 is appended below
+
+
+def run_b200(args):
+    import numpy as np
+    import torch
+    from paper_2307_01416_b200 import binding, dist, workloads as wl
+
+    rank, local_rank, world = dist.init()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
+    N = int(args.histories)
+    seed = dist.rank_seed(SEED, rank)
+    plans = wl.config2_plans()
+    problems = [wl.config2(d, rs, N, SEED) for (d, rs) in plans]
+
+    # ---- set-up (S0), not part of histories/s
+    t0 = time.perf_counter()
+    engines = [binding.Engine(p) for p in problems]
+    doses = [torch.empty(e.nvox, dtype=torch.float32, device=dev) for e in engines]
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for e, d in zip(engines, doses):
+            e.dose(N, seed, out=d, stream=stream)
+            dist.combine_dose(d, world)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    for e in engines:
+        e.set_timing(True)
+        e.timing()
+    launches0 = sum(e.launch_count() for e in engines)
+    dist.barrier(world)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local_rank)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.zero_()                                   # L2 flush between timed iterations (not timed)
+        ev[k][0].record(stream)
+        step()
+        ev[k][1].record(stream)
+    torch.cuda.synchronize()
+    dist.barrier(world)
+    clocks = sampler.stop()
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t_ms = dist.max_over_ranks(t_ms, world, dev)
+    launches = sum(e.launch_count() for e in engines) - launches0
+    hist_per_step = N * len(plans) * world
+    value = hist_per_step * args.steps / (t_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (voxel_kernel), live CUDA-event durations from the library
+    tm = {"beamline": [0.0, 0], "voxel": [0.0, 0], "scoring": [0.0, 0], "writer": [0.0, 0]}
+    steps_ct = 0
+    for e in engines:
+        for k, (ms, n) in e.timing().items():
+            tm[k][0] += ms; tm[k][1] += n
+        e.set_timing(False)
+        steps_ct += e.tallies().n_steps_ct               # of the last dose() call = one timed step's share
+    vox_ms, vox_n = tm["voxel"]
+    ct_steps_per_launch = steps_ct * args.steps / max(vox_n, 1)
+    avg_launch_s = vox_ms * 1e-3 / max(vox_n, 1)
+    peak_ginst = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e9        # lane-instructions/s at the max SM clock
+    achieved_ginst = INST_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9
+    roofline = {"bound": "alu", "kernel": "voxel_kernel", "achieved": achieved_ginst, "peak": peak_ginst,
+                "unit": "Glane-inst/s", "frac": achieved_ginst / peak_ginst, "traffic": None,
+                "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (%s sm_max_mhz)" % (sm_max_mhz, peak_kind),
+                "inst_per_ct_step": INST_PER_CT_STEP, "ct_steps_per_launch": ct_steps_per_launch,
+                "avg_launch_ms": avg_launch_s * 1e3, "launches": vox_n,
+                "share_of_step": {k: v[0] / max(t_ms, 1e-9) for k, v in tm.items()},
+                "hbm": {"achieved": ALG_BYTES_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9, "peak": hbm_gbs,
+                        "unit": "GB/s", "frac": ALG_BYTES_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9 / hbm_gbs,
+                        "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"}}
+
+    # ---- e2e: host buffers in, host dose out, through the C-ABI, H2D/D2H inside the timed region
+    pinned_problems = [pin_problem(p) for p in problems]
+    host_out = [pinned(np.empty(e.nvox, dtype=np.float32)) for e in engines]
+    for e in engines:
+        e.close()
+    del engines
+
+    def e2e_step():
+        h2d = d2h = 0
+        for p, out in zip(pinned_problems, host_out):
+            e = binding.Engine(p)
+            e.dose_host(N, seed, out=out)
+            h2d += e.h2d_bytes; d2h += out.nbytes
+            e.close()
+        return h2d, d2h
+
+    e2e_step()
+    dist.barrier(world)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        h2d, d2h = e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = dist.max_over_ranks(time.perf_counter() - t0, world, dev)
+    e2e = {"value": hist_per_step * args.steps / e2e_s, "unit": "histories/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+
+    out = {"metric": METRIC, "value": value, "unit": "histories/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": "BASELINE.json configs[1]: water 100x100x150 @ 2 mm, 8 plans (opening 1/2/3/4 cm x RS off/on), "
+                                  "825-3993 spots", "histories_per_plan": N, "plans_per_step": len(plans),
+                      "n_batches": 10, "l2_flush_between_steps": True, "parallelism": "replicas x%d + dose all-reduce" % world,
+                      "setup_s": setup_s},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+
+    if rank == 0 and world == 1 and not args.no_dose_at_unc:
+        out["dose_at_0p5pct"] = dose_at_uncertainty(binding, wl)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import cpu_bench
+        per_plan = args.cpu_sample // len(plans)
+        busy, done, cores = 0.0, 0, 1
+        for (d, rs) in plans:
+            r, cores, _ = cpu_bench.time_oracle("config2", {"opening_mm": d, "range_shifter": rs}, N, SEED, per_plan)
+            busy += per_plan / r; done += per_plan
+        out["cpu_baseline"] = {"value": done / busy, "unit": "histories/s", "cores": cores, "kind": "oracle",
+                               "sample": "%d histories per plan over the %d plans, ids spread over the %d-history run, "
+                                         "%d single-threaded oracle processes" % (per_plan, len(plans), N, cores)}
+    if rank == 0:
+        print(json.dumps(out))
+
+
+def dose_at_uncertainty(binding, wl, target=0.005):
+    """Second half of the metric: seconds per dose at 0.5 % statistical uncertainty (SURVEY.md 8(c)-C6 estimator):
+    set-up + a pilot run + the run sized from the pilot by N = N0 (u0/target)^2; the final run's own estimate is reported."""
+    import torch
+    p = wl.config2(20, False)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e = binding.Engine(p)
+    n0 = 1_000_000
+    d = e.dose(n0, SEED)
+    u0 = e.uncertainty()
+    n = int(min(max(n0 * (u0 / target) ** 2 * 1.05, n0), 2e9))
+    d = e.dose(n, SEED + 1, out=d)
+    u = e.uncertainty()
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    e.close()
+    return {"workload": "config2 opening 2 cm, no range shifter", "seconds": sec, "histories": n + n0, "uncertainty": u,
+            "pilot_uncertainty": u0, "target": target}
+
+
+if __name__ == "__main__":
+    main()

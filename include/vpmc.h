@@ -116,6 +116,7 @@ typedef void *(*vpmc_alloc_fn)(size_t bytes, void *user);
 typedef struct {
     double incident, dep_ct, dep_rs, dep_brass, escaped, removed;                   /* MeV */
     uint64_t n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;     /* histories by fate */
+    uint64_t n_steps_ct, n_steps_dev;   /* steps taken in the CT / in the beam line (drifts included) */
 } vpmc_tallies;
 
 /* One step of one history (vpmc_trace).  r, u after the step: beam frame in the beam line, CT frame from the
@@ -194,6 +195,13 @@ int vpmc_get_uncertainty(vpmc_t *h, float *rel_unc_out);
  * with hist_per_spot = n_or_hps.  out_host: n*max_steps records; nrec_host[i] = records of history i. */
 int vpmc_trace(vpmc_t *h, const vpmc_scenario *sc, int32_t mode, uint64_t n_or_hps, uint64_t seed,
                const uint64_t *hids, int32_t n, int32_t max_steps, vpmc_step_rec *out_host, int32_t *nrec_host);
+
+/* Per-kernel-class device timing (bench.py's roofline): when on, every launch is bracketed by CUDA events on its
+ * stream.  vpmc_get_timing synchronises, returns accumulated milliseconds and launch counts per class
+ * (0 beam line S1-S3, 1 voxel stepping S4-S6b, 2 dose scoring passes S6, 3 influence/CSR writer S7-S8) and resets. */
+#define VPMC_N_KERNEL_CLASSES 4
+int vpmc_set_timing(vpmc_t *h, int on);
+int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out);
 
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int vpmc_get_launch_count(vpmc_t *h, uint64_t *out);

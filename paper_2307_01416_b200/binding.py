@@ -20,7 +20,8 @@ BRASS = 1
 EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy", "vpmc_add_beam", "vpmc_set_beam",
            "vpmc_set_range_shifter", "vpmc_set_aperture", "vpmc_dose", "vpmc_dose_scenario", "vpmc_dose_host",
            "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
-           "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error"]
+           "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
+           "vpmc_get_timing"]
 
 
 class VpmcError(RuntimeError):
@@ -60,7 +61,8 @@ class _Csr(C.Structure):
 
 class Tallies(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("incident", "dep_ct", "dep_rs", "dep_brass", "escaped", "removed")] + \
-               [(n, C.c_uint64) for n in ("n_stopped_ct", "n_stopped_rs", "n_stopped_brass", "n_nuclear", "n_escaped")]
+               [(n, C.c_uint64) for n in ("n_stopped_ct", "n_stopped_rs", "n_stopped_brass", "n_nuclear", "n_escaped",
+                                          "n_steps_ct", "n_steps_dev")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -108,6 +110,8 @@ def lib():
         L.vpmc_trace.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_int32, C.c_uint64, C.c_uint64, C.c_void_p,
                                  C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.vpmc_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+        L.vpmc_set_timing.argtypes = [C.c_void_p, C.c_int]
+        L.vpmc_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
 
@@ -240,6 +244,16 @@ class Engine:
         n = C.c_uint64()
         self._check(lib().vpmc_get_launch_count(self._h, C.byref(n)))
         return int(n.value)
+
+    def set_timing(self, on: bool):
+        self._check(lib().vpmc_set_timing(self._h, 1 if on else 0))
+
+    def timing(self):
+        """{class: (milliseconds, launches)} accumulated since the last call; classes beamline/voxel/scoring/writer."""
+        ms = (C.c_double * 4)()
+        n = (C.c_uint64 * 4)()
+        self._check(lib().vpmc_get_timing(self._h, ms, n))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("beamline", "voxel", "scoring", "writer"))}
 
     def trace(self, hids, n_or_hps: int, seed: int, sc: Scenario | None = None, mode: int = 0, max_steps: int = 1024):
         hids = np.ascontiguousarray(np.asarray(hids, dtype=np.uint64))

@@ -252,6 +252,43 @@ extern "C" int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t h
     return VPMC_OK;
 }
 
+// ---- per-kernel-class timing (events on the launching stream) ----
+struct TimedScope {
+    vpmc_t *h; cudaStream_t st; int cls; cudaEvent_t a = nullptr, b = nullptr;
+    TimedScope(vpmc_t *h_, cudaStream_t st_, int cls_) : h(h_), st(st_), cls(cls_)
+    {
+        if (h->timing && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) cudaEventRecord(a, st);
+        else a = nullptr;
+    }
+    ~TimedScope()
+    {
+        if (a) { cudaEventRecord(b, st); h->timed.push_back({ a, b, cls }); }
+    }
+};
+
+extern "C" int vpmc_set_timing(vpmc_t *h, int on)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    h->timing = on != 0;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!ms_out || !launches_out) FAIL(h, VPMC_ERR_INVALID_ARG, "NULL argument");
+    for (int i = 0; i < VPMC_N_KERNEL_CLASSES; ++i) { ms_out[i] = 0.0; launches_out[i] = 0; }
+    for (auto &t : h->timed) {
+        CU(h, cudaEventSynchronize(t.b));
+        float ms = 0.0f;
+        CU(h, cudaEventElapsedTime(&ms, t.a, t.b));
+        ms_out[t.cls] += ms; launches_out[t.cls] += 1;
+        cudaEventDestroy(t.a); cudaEventDestroy(t.b);
+    }
+    h->timed.clear();
+    return VPMC_OK;
+}
+
 extern "C" int vpmc_get_launch_count(vpmc_t *h, uint64_t *out)
 {
     if (!h || !out) return VPMC_ERR_INVALID_ARG;

@@ -68,5 +68,8 @@ struct vpmc {
     unsigned long long win_lo = 0, win_hi = 0;
     cudaStream_t last_stream = nullptr;
     unsigned long long launches = 0;
+    bool timing = false;
+    struct Timed { cudaEvent_t a, b; int cls; };
+    std::vector<Timed> timed;
     std::string err;
 };

@@ -61,24 +61,24 @@ __device__ __forceinline__ unsigned warp_sum(unsigned v)
     return v;
 }
 
-// block-level reduction of the per-thread tallies, then 11 global atomics per block
+// block-level reduction of the per-thread tallies, then 13 global atomics per block
 __device__ void flush_tallies(const Tally &t, DevTallies *g)
 {
     __shared__ double sd[6];
-    __shared__ unsigned int sc[5];
+    __shared__ unsigned int sc[7];
     if (threadIdx.x < 6) sd[threadIdx.x] = 0.0;
-    if (threadIdx.x < 5) sc[threadIdx.x] = 0u;
+    if (threadIdx.x < 7) sc[threadIdx.x] = 0u;
     __syncthreads();
     const double d[6] = { t.incident, t.dep_ct, t.dep_rs, t.dep_brass, t.escaped, t.removed };
-    const unsigned c[5] = { t.n_stopped_ct, t.n_stopped_rs, t.n_stopped_brass, t.n_nuclear, t.n_escaped };
+    const unsigned c[7] = { t.n_stopped_ct, t.n_stopped_rs, t.n_stopped_brass, t.n_nuclear, t.n_escaped, t.n_steps_ct, t.n_steps_dev };
     const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int i = 0; i < 6; ++i) { const double v = warp_sum(d[i]); if (lane == 0 && v != 0.0) atomicAdd(&sd[i], v); }
 #pragma unroll
-    for (int i = 0; i < 5; ++i) { const unsigned v = warp_sum(c[i]); if (lane == 0 && v) atomicAdd(&sc[i], v); }
+    for (int i = 0; i < 7; ++i) { const unsigned v = warp_sum(c[i]); if (lane == 0 && v) atomicAdd(&sc[i], v); }
     __syncthreads();
     if (threadIdx.x < 6 && sd[threadIdx.x] != 0.0) atomicAdd(&g->incident + threadIdx.x, sd[threadIdx.x]);
-    if (threadIdx.x < 5 && sc[threadIdx.x]) atomicAdd(&g->n_stopped_ct + threadIdx.x, (unsigned long long)sc[threadIdx.x]);
+    if (threadIdx.x < 7 && sc[threadIdx.x]) atomicAdd(&g->n_stopped_ct + threadIdx.x, (unsigned long long)sc[threadIdx.x]);
 }
 
 // item -> (global spot, history id)
@@ -119,6 +119,7 @@ beamline_kernel(const DevParams P, const DevGrid G, const WorkMap wm, const floa
         const float sh[3] = { shift.x, shift.y, shift.z };
         float w_now;
         if (beamline(P, b, h, t, tr, k0, k1, w_now) == CONT) alive = enter_ct(G, b, sh, w_now, h, iv, t, tr) == CONT;
+        t.n_steps_dev = h.step;
     }
     // S6b, first stage: only survivors enter the voxel queue (warp-aggregated slot claim)
     const unsigned mask = __ballot_sync(0xffffffffu, alive);
@@ -225,6 +226,7 @@ voxel_kernel(const DevParams P, const DevGrid G, const Queue q, const short *__r
             const int vx = ix, vy = iy, vz = iz;      // voxel of the deposit = voxel at the start of the step
             if (SMEM_LUT) cause = ct_step(P, G, hu, LutShared{ lut_s }, rsp_scale, h, ix, iy, iz, v, o, tr, k0, k1);
             else cause = ct_step(P, G, hu, LutGlobal{ lut_g }, rsp_scale, h, ix, iy, iz, v, o, tr, k0, k1);
+            t.n_steps_ct += (cause != STOPPED);
             if (o.dep != 0.0f) {
                 if (MODE == 0) {
                     atomicAdd(edep + v, o.dep);

@@ -116,8 +116,12 @@ static int launch_chunk(vpmc_t *h, const WorkMap &wm0, unsigned long long item0,
     CU(h, cudaMemsetAsync(h->d_qctr, 0, 2 * sizeof(unsigned int), st));
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const float3 shift = make_float3(sc.shift[0], sc.shift[1], sc.shift[2]);
-    beamline_kernel<<<(n + 255) / 256, 256, 0, st>>>(h->P, h->G, wm, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, shift, k0, k1, h->q, h->d_tal);
+    {
+        TimedScope ts(h, st, 0);
+        beamline_kernel<<<(n + 255) / 256, 256, 0, st>>>(h->P, h->G, wm, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, shift, k0, k1, h->q, h->d_tal);
+    }
     CU(h, cudaGetLastError());
+    TimedScope ts(h, st, 1);
     if (h->smem_lut)
         voxel_kernel<MODE, true><<<h->voxel_grid[MODE][1], 256, h->lut_bytes, st>>>(h->P, h->G, h->q, h->d_hu, h->d_lut, sc.rsp_scale, edep, cb, col0, wm.hps, k0, k1, h->d_tal);
     else
@@ -190,6 +194,7 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
             rc = launch_chunk<0>(h, wm, i0, n, sc, seed, h->d_edep, cb, 0, st); if (rc) return rc;
         }
         const float f = (float)((double)n_total / (double)nb);
+        TimedScope ts(h, st, 2);
         batch_accumulate_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->d_edep, h->d_sum, h->d_s1, h->d_s2, h->nvox, f, with_unc ? 1 : 0);
         CU(h, cudaGetLastError());
         h->launches += 1;
@@ -199,6 +204,7 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     for (double x : h->spot_w) W += x;
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef = (float)((n_histories ? W / (double)n_histories : 0.0) / V * 1.602176634e-10);
+    TimedScope ts(h, st, 2);
     dose_convert_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->d_sum, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef, dose_out_dev, h->nvox, h->d_max_bits);
     CU(h, cudaGetLastError());
     h->launches += 1;

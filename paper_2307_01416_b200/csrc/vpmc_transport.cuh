@@ -9,12 +9,14 @@ namespace vpk {
 struct DevTallies {
     double incident, dep_ct, dep_rs, dep_brass, escaped, removed;
     unsigned long long n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;
+    unsigned long long n_steps_ct, n_steps_dev;
 };
 
 // per-thread partial tallies
 struct Tally {
     double incident = 0, dep_ct = 0, dep_rs = 0, dep_brass = 0, escaped = 0, removed = 0;
     unsigned int n_stopped_ct = 0, n_stopped_rs = 0, n_stopped_brass = 0, n_nuclear = 0, n_escaped = 0;
+    unsigned int n_steps_ct = 0, n_steps_dev = 0;
 };
 
 struct StepRec {   // == vpmc_step_rec
