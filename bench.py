@@ -150,6 +150,8 @@ def main():
     ap.add_argument("--histories", type=int, default=10_000_000, help="histories per plan (BASELINE.json: 1e7)")
     ap.add_argument("--ref-sample", type=int, default=800_000, help="oracle histories per reference step")
     ap.add_argument("--cpu-sample", type=int, default=1_600_000, help="oracle histories of the cpu_baseline leg")
+    ap.add_argument("--plans", default="", help="subset of the 8 plans as opening_mm:rs pairs, e.g. 20:0,20:1 (profiling)")
+    ap.add_argument("--n-batches", type=int, default=10, help="batches of the uncertainty estimate (vpmc_params.n_batches)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-dose-at-unc", action="store_true")
     args = ap.parse_args()
@@ -174,11 +176,14 @@ def run_b200(args):
     N = int(args.histories)
     seed = dist.rank_seed(SEED, rank)
     plans = wl.config2_plans()
+    if args.plans:
+        plans = [(int(x.split(":")[0]), bool(int(x.split(":")[1]))) for x in args.plans.split(",")]
     problems = [wl.config2(d, rs, N, SEED) for (d, rs) in plans]
+    params = binding.default_params(n_batches=args.n_batches)
 
     # ---- set-up (S0), not part of histories/s
     t0 = time.perf_counter()
-    engines = [binding.Engine(p) for p in problems]
+    engines = [binding.Engine(p, params) for p in problems]
     doses = [torch.empty(e.nvox, dtype=torch.float32, device=dev) for e in engines]
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
@@ -249,7 +254,7 @@ def run_b200(args):
     def e2e_step():
         h2d = d2h = 0
         for p, out in zip(pinned_problems, host_out):
-            e = binding.Engine(p)
+            e = binding.Engine(p, params)
             e.dose_host(N, seed, out=out)
             h2d += e.h2d_bytes; d2h += out.nbytes
             e.close()
@@ -270,7 +275,7 @@ def run_b200(args):
            "dtype": "f32", "data": "synthetic",
            "config": {"workload": "BASELINE.json configs[1]: water 100x100x150 @ 2 mm, 8 plans (opening 1/2/3/4 cm x RS off/on), "
                                   "825-3993 spots", "histories_per_plan": N, "plans_per_step": len(plans),
-                      "n_batches": 10, "l2_flush_between_steps": True, "parallelism": "replicas x%d + dose all-reduce" % world,
+                      "n_batches": args.n_batches, "l2_flush_between_steps": True, "parallelism": "replicas x%d + dose all-reduce" % world,
                       "setup_s": setup_s},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
 

@@ -57,6 +57,9 @@ static DevParams make_dev_params(const vpmc_params &p)
     d.rs_rsp = p.rs_rsp; d.rs_rho = p.rs_rho; d.rs_inv_X0 = (float)(1.0 / (double)p.rs_X0);
     d.rs_za_rho = (float)((double)p.za_w * (double)p.rs_rho);
     d.rho_min = p.rho_min; d.delta_E = p.delta_E; d.flags = p.flags;
+    const double pp = (double)p.p;
+    d.pc2 = (float)(pp * (pp - 1) / 2); d.pc3 = (float)(pp * (pp - 1) * (pp - 2) / 6);
+    d.pc4 = (float)(pp * (pp - 1) * (pp - 2) * (pp - 3) / 24); d.pc5 = (float)(pp * (pp - 1) * (pp - 2) * (pp - 3) * (pp - 4) / 120);
     return d;
 }
 

@@ -206,7 +206,7 @@ voxel_kernel(const DevParams P, const DevGrid G, const Queue q, const short *__r
                     const float4 a = q.q0[slot], b = q.q1[slot], c = q.q2[slot];
                     const uint4 e = q.q3[slot];
                     h.rx = a.x; h.ry = a.y; h.rz = a.z; h.E = a.w;
-                    h.ux = b.x; h.uy = b.y; h.uz = b.z; h.t_rad = b.w;
+                    h.ux = b.x; h.uy = b.y; h.uz = b.z; h.t_rad = b.w; h.A_rad = highland_A(b.w, P.c_log);
                     h.tau = c.x; h.tau_star = c.y; h.step = __float_as_uint(c.z);
                     h.R = __longlong_as_double((long long)(((unsigned long long)e.w << 32) | __float_as_uint(c.w)));
                     h.hid_lo = e.x; h.hid_hi = e.y;

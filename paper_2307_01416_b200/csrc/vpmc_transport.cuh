@@ -81,7 +81,7 @@ __device__ __forceinline__ void sample_source(const DevParams &P, const float4 s
     h.E = E0; h.R = R0;
     const float4 b = draw4(h, 0u, 2u, k0, k1);
     h.tau_star = -logf(b.x);
-    h.tau = 0.0f; h.t_rad = 0.0f; h.step = 0u;
+    h.tau = 0.0f; h.t_rad = 0.0f; h.A_rad = 0.0f; h.step = 0u;
     h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f;
 }
 
