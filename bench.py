@@ -228,13 +228,14 @@ def run_b200(args):
         for k, (ms, n) in e.timing().items():
             tm[k][0] += ms; tm[k][1] += n
         e.set_timing(False)
-        steps_ct += e.tallies().n_steps_ct               # of the last dose() call = one timed step's share
-    vox_ms, vox_n = tm["voxel"]
+        tl = e.tallies()
+        steps_ct += tl.n_steps_ct + tl.n_steps_dev       # of the last dose() call = one timed step's share
+    vox_ms, vox_n = tm["beamline"][0] + tm["voxel"][0], tm["voxel"][1]
     ct_steps_per_launch = steps_ct * args.steps / max(vox_n, 1)
     avg_launch_s = vox_ms * 1e-3 / max(vox_n, 1)
     peak_ginst = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e9        # lane-instructions/s at the max SM clock
     achieved_ginst = INST_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9
-    roofline = {"bound": "alu", "kernel": "voxel_kernel", "achieved": achieved_ginst, "peak": peak_ginst,
+    roofline = {"bound": "alu", "kernel": "beam_kernel + voxel_kernel<0>", "achieved": achieved_ginst, "peak": peak_ginst,
                 "unit": "Glane-inst/s", "frac": achieved_ginst / peak_ginst, "traffic": None,
                 "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (%s sm_max_mhz)" % (sm_max_mhz, peak_kind),
                 "inst_per_ct_step": INST_PER_CT_STEP, "ct_steps_per_launch": ct_steps_per_launch,

@@ -174,7 +174,9 @@ int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);
 
 /* Influence matrices: for each of n_sc scenarios and each spot j (history ids
  * j*hist_per_spot + i), the dose column per unit weight, entries >= rel_threshold * column max (and > 0) kept,
- * written as CSR into out[0..n_sc) through `alloc`.  Synchronises where it must size outputs. */
+ * written as CSR into out[0..n_sc) through `alloc` (three calls per scenario: row_ptr, col, val).  Synchronises
+ * where it must size outputs.  Tallies afterwards cover every history of every scenario once (the pilot and replay
+ * passes that only size the per-column boxes are not counted).  On error out[] may be partially filled. */
 int vpmc_influence(vpmc_t *h, const vpmc_scenario *sc, int32_t n_sc, uint32_t hist_per_spot,
                    float rel_threshold, uint64_t seed, vpmc_csr *out, vpmc_alloc_fn alloc, void *user,
                    void *cuda_stream);
@@ -183,6 +185,10 @@ int vpmc_influence(vpmc_t *h, const vpmc_scenario *sc, int32_t n_sc, uint32_t hi
  * col_out/val_out NULL only counts.  *nnz_out [host].  Synchronous. */
 int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, float rel_threshold,
                         int32_t *col_out_dev, float *val_out_dev, int64_t *nnz_out);
+
+/* Upper bound in bytes on the per-group scratch of vpmc_influence (the dense per-column boxes of one group of spots);
+ * 0 = automatic (a third of the free device memory, at most 24 GiB).  Smaller limits only mean more groups. */
+int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes);
 
 /* Tallies of the last dose / influence call (synchronises the stream it ran on). */
 int vpmc_get_tallies(vpmc_t *h, vpmc_tallies *out);
@@ -198,7 +204,8 @@ int vpmc_trace(vpmc_t *h, const vpmc_scenario *sc, int32_t mode, uint64_t n_or_h
 
 /* Per-kernel-class device timing (bench.py's roofline): when on, every launch is bracketed by CUDA events on its
  * stream.  vpmc_get_timing synchronises, returns accumulated milliseconds and launch counts per class
- * (0 beam line S1-S3, 1 voxel stepping S4-S6b, 2 dose scoring passes S6, 3 influence/CSR writer S7-S8) and resets. */
+ * (0 beam_kernel S1-S3, 1 voxel_kernel S4-S7 incl. the influence pilot, 2 dose conversion / uncertainty passes S6,
+ * 3 CSR writer passes S8) and resets. */
 #define VPMC_N_KERNEL_CLASSES 4
 int vpmc_set_timing(vpmc_t *h, int on);
 int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out);

@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libvpmc.so")
+LIB_PATH = os.environ.get("VPMC_LIB", os.path.join(_HERE, "libvpmc.so"))   # VPMC_LIB: another build of the same library
 
 OK, ERR_INVALID_ARG, ERR_GEOMETRY, ERR_CUDA, ERR_ALLOC, ERR_STATE = 0, -1, -2, -3, -4, -5
 FLAG_MCS, FLAG_STRAGGLE, FLAG_NUCLEAR = 1, 2, 4
@@ -21,7 +21,7 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_set_range_shifter", "vpmc_set_aperture", "vpmc_dose", "vpmc_dose_scenario", "vpmc_dose_host",
            "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
-           "vpmc_get_timing"]
+           "vpmc_get_timing", "vpmc_set_workspace_limit"]
 
 
 class VpmcError(RuntimeError):
@@ -112,6 +112,7 @@ def lib():
         L.vpmc_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
         L.vpmc_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.vpmc_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+        L.vpmc_set_workspace_limit.argtypes = [C.c_void_p, C.c_uint64]
         _lib = L
     return _lib
 
@@ -249,7 +250,7 @@ class Engine:
         self._check(lib().vpmc_set_timing(self._h, 1 if on else 0))
 
     def timing(self):
-        """{class: (milliseconds, launches)} accumulated since the last call; classes beamline/voxel/scoring/writer."""
+        """{class: (milliseconds, launches)} accumulated since the last call; classes beamline / voxel / scoring / writer."""
         ms = (C.c_double * 4)()
         n = (C.c_uint64 * 4)()
         self._check(lib().vpmc_get_timing(self._h, ms, n))
@@ -289,9 +290,20 @@ class Engine:
             res.append((rp, col, val))
         return res
 
-    def csr_from_dense(self, col):
+    def set_workspace_limit(self, nbytes: int):
+        self._check(lib().vpmc_set_workspace_limit(self._h, int(nbytes)))
+
+    def csr_from_dense(self, col, rel_threshold: float):
         """The CSR writer alone on one dense fp32 CUDA column: (idx int32, val fp32) CUDA tensors."""
         import torch
         assert col.is_cuda and col.dtype == torch.float32 and col.is_contiguous()
         nnz = C.c_int64()
-        return col, nnz
+        self._check(lib().vpmc_csr_from_dense(self._h, col.data_ptr(), col.numel(), float(rel_threshold), None, None,
+                                              C.byref(nnz)))
+        idx = torch.empty(max(nnz.value, 1), dtype=torch.int32, device=col.device)
+        val = torch.empty(max(nnz.value, 1), dtype=torch.float32, device=col.device)
+        n2 = C.c_int64()
+        self._check(lib().vpmc_csr_from_dense(self._h, col.data_ptr(), col.numel(), float(rel_threshold), idx.data_ptr(),
+                                              val.data_ptr(), C.byref(n2)))
+        assert n2.value == nnz.value
+        return idx[: nnz.value], val[: nnz.value]

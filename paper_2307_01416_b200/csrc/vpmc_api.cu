@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <numeric>
@@ -27,10 +28,23 @@ static thread_local std::string g_create_err;
         if (_e != cudaSuccess) FAIL(h, VPMC_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
     } while (0)
 
-static constexpr unsigned int kChunk = 1u << 20;       // histories per beamline launch = queue capacity
-static constexpr size_t kMaxSmemLut = 96 * 1024;
+static constexpr size_t kMaxSmemLut = 96 * 1024;      // larger material tables are read through L1 instead
+static constexpr unsigned long long kChunk = 1ull << 23;   // work items per pass of the pipeline = queue capacity
 
-extern "C" const char *vpmc_version(void) { return "vpmc-b200 0.1 (sm_100a)"; }
+// grow-only device buffer
+static int ensure(vpmc_t *h, DevBuf &b, size_t bytes);
+
+static int ensure(vpmc_t *h, DevBuf &b, size_t bytes)
+{
+    if (b.bytes >= bytes && b.p) return VPMC_OK;
+    if (b.p) { cudaFree(b.p); b.p = nullptr; b.bytes = 0; }
+    const size_t want = std::max<size_t>(bytes, 256);
+    if (cudaMalloc(&b.p, want) != cudaSuccess) { cudaGetLastError(); b.p = nullptr; FAIL(h, VPMC_ERR_ALLOC, "out of device memory (%zu bytes)", want); }
+    b.bytes = want;
+    return VPMC_OK;
+}
+
+extern "C" const char *vpmc_version(void) { return "vpmc-b200 0.2 (sm_100a)"; }
 
 extern "C" void vpmc_default_params(vpmc_params *p)
 {
@@ -52,9 +66,10 @@ static DevParams make_dev_params(const vpmc_params &p)
     d.inv_X0_w = (float)(1.0 / (double)p.X0_w); d.Es = p.Es; d.c_log = p.c_log;
     d.beta_nuc = p.beta_nuc; d.gamma_loc = p.gamma_loc; d.k_bohr = p.k_bohr; d.za_w = p.za_w;
     d.R_cut = p.R_cut; d.f_R = p.f_R; d.s_max = p.s_max; d.s_rs = p.s_rs; d.s_ap = p.s_ap;
-    d.brass_rsp = p.brass_rsp; d.brass_rho = p.brass_rho; d.brass_inv_X0 = (float)(1.0 / (double)p.brass_X0);
+    d.brass_rsp = p.brass_rsp; d.brass_inv_rsp = (float)(1.0 / (double)p.brass_rsp); d.brass_rho = p.brass_rho;
+    d.brass_inv_X0 = (float)(1.0 / (double)p.brass_X0);
     d.brass_za_rho = (float)((double)p.brass_za * (double)p.brass_rho);
-    d.rs_rsp = p.rs_rsp; d.rs_rho = p.rs_rho; d.rs_inv_X0 = (float)(1.0 / (double)p.rs_X0);
+    d.rs_rsp = p.rs_rsp; d.rs_inv_rsp = (float)(1.0 / (double)p.rs_rsp); d.rs_rho = p.rs_rho; d.rs_inv_X0 = (float)(1.0 / (double)p.rs_X0);
     d.rs_za_rho = (float)((double)p.za_w * (double)p.rs_rho);
     d.rho_min = p.rho_min; d.delta_E = p.delta_E; d.flags = p.flags;
     const double pp = (double)p.p;
@@ -76,7 +91,8 @@ static double pl_eval(const vpmc_calib *c, const float *y, double hu)
 static void free_beam(BeamHost &b)
 {
     if (b.d_bits) cudaFree(b.d_bits);
-    b.d_bits = nullptr;
+    if (b.d_dist) cudaFree(b.d_dist);
+    b.d_bits = nullptr; b.d_dist = nullptr;
 }
 
 extern "C" int vpmc_destroy(vpmc_t *h)
@@ -84,10 +100,13 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     if (!h) return VPMC_OK;
     cudaDeviceSynchronize();
     for (auto &b : h->beams) free_beam(b);
-    void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_cum, h->d_first, h->q.q0, h->q.q1,
-                     h->q.q2, h->q.q3, h->d_qctr, h->d_edep, h->d_sum, h->d_s1, h->d_s2, h->d_tal, h->d_max_bits, h->d_unc };
+    void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_qctr, h->d_s1, h->d_s2, h->d_fb,
+                     h->d_tal, h->d_tal_scratch, h->d_max_bits, h->d_unc };
     for (void *p : ptrs) if (p) cudaFree(p);
-    for (void *p : h->d_inf) if (p) cudaFree(p);
+    DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
+                       &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
+                       &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc };
+    for (DevBuf *b : bufs) if (b->p) cudaFree(b->p);
     delete h;
     return VPMC_OK;
 }
@@ -133,7 +152,8 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
         const double hu = (double)(G.hu_min + i);
         const double rsp = pl_eval(cal, cal->rsp, hu), rho = pl_eval(cal, cal->rho, hu);
         const double xsp = cal->xsp ? pl_eval(cal, cal->xsp, hu) : rho;
-        lut[i] = make_float4((float)rsp, (float)rho, (float)(xsp / (double)p.X0_w), (float)((double)p.za_w * rho));
+        if (!(rsp > 0.0)) { delete h; FAIL(nh, VPMC_ERR_INVALID_ARG, "calibration gives RSP <= 0 at HU %d", G.hu_min + i); }
+        lut[i] = make_float4((float)rsp, (float)rho, (float)(xsp / (double)p.X0_w), (float)(1.0 / rsp));
     }
     h->lut_bytes = lut.size() * sizeof(float4);
     h->smem_lut = h->lut_bytes <= kMaxSmemLut;
@@ -142,34 +162,31 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     CUC(cudaMemcpy(h->d_lut, lut.data(), h->lut_bytes, cudaMemcpyHostToDevice));
     CUC(cudaMalloc(&h->d_hu, nvox * sizeof(short)));
     CUC(cudaMemcpy(h->d_hu, ct->hu, nvox * sizeof(short), ct->hu_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice));
-    CUC(cudaMalloc(&h->d_edep, nvox * sizeof(float)));
-    CUC(cudaMalloc(&h->d_sum, nvox * sizeof(float)));
     CUC(cudaMalloc(&h->d_tal, sizeof(DevTallies)));
     CUC(cudaMemset(h->d_tal, 0, sizeof(DevTallies)));
+    CUC(cudaMalloc(&h->d_tal_scratch, sizeof(DevTallies)));
     CUC(cudaMalloc(&h->d_max_bits, sizeof(unsigned int)));
     CUC(cudaMalloc(&h->d_unc, 2 * sizeof(double)));
-    CUC(cudaMalloc(&h->d_qctr, 2 * sizeof(unsigned int)));
-    CUC(cudaMalloc(&h->q.q0, (size_t)kChunk * sizeof(float4)));
-    CUC(cudaMalloc(&h->q.q1, (size_t)kChunk * sizeof(float4)));
-    CUC(cudaMalloc(&h->q.q2, (size_t)kChunk * sizeof(float4)));
-    CUC(cudaMalloc(&h->q.q3, (size_t)kChunk * sizeof(uint4)));
-    h->q.count = h->d_qctr; h->q.head = h->d_qctr + 1; h->q.capacity = kChunk;
-    // persistent voxel kernel: one wave of resident CTAs
+    CUC(cudaMalloc(&h->d_qctr, 4 * sizeof(unsigned int)));
+    CUC(cudaMalloc(&h->d_fb, 1024 * sizeof(float)));
+    // persistent kernels: one wave of resident CTAs each
     {
-        const size_t sm = h->smem_lut ? h->lut_bytes : 0;
+        h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
+        if (const char *e = getenv("VPMC_LUT")) { if (!strcmp(e, "global")) h->smem_lut = false; }
         int occ = 0;
-        if (h->smem_lut) {
-            CUC(cudaFuncSetAttribute(voxel_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmemLut));
-            CUC(cudaFuncSetAttribute(voxel_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmemLut));
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<0, true>, 256, sm));
-            h->voxel_grid[0][1] = std::max(occ, 1) * h->n_sm;
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<1, true>, 256, sm));
-            h->voxel_grid[1][1] = std::max(occ, 1) * h->n_sm;
-        }
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<0, false>, 256, 0));
-        h->voxel_grid[0][0] = std::max(occ, 1) * h->n_sm;
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_kernel<1, false>, 256, 0));
-        h->voxel_grid[1][0] = std::max(occ, 1) * h->n_sm;
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel, kBlock, 0));
+        h->grid_beam = std::max(occ, 1) * h->n_sm;
+        const void *fn[3][2] = { { (const void *)voxel_kernel<0, false>, (const void *)voxel_kernel<0, true> },
+                                 { (const void *)voxel_kernel<1, false>, (const void *)voxel_kernel<1, true> },
+                                 { (const void *)voxel_kernel<2, false>, (const void *)voxel_kernel<2, true> } };
+        for (int m = 0; m < 3; ++m)
+            for (int s = 0; s < 2; ++s) {
+                if (s == 1 && !h->smem_lut) continue;
+                const size_t sm = h->tally_smem + (s ? h->lut_bytes : 0);
+                if (s) CUC(cudaFuncSetAttribute(fn[m][s], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxSmemLut + h->tally_smem)));
+                CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn[m][s], kBlock, sm));
+                h->grid[m][s] = std::max(occ, 1) * h->n_sm;
+            }
     }
 #undef CUC
     *out = h;
@@ -189,6 +206,7 @@ extern "C" int vpmc_add_beam(vpmc_t *h, const vpmc_frame *frame, int *beam_id)
             for (int k = 0; k < 3; ++k) d += (double)frame->rot[3 * k + i] * frame->rot[3 * k + j];
             if (std::fabs(d - (i == j ? 1.0 : 0.0)) > 1e-3) FAIL(h, VPMC_ERR_INVALID_ARG, "frame.rot is not orthonormal");
         }
+    if (h->beams.size() >= 255) FAIL(h, VPMC_ERR_INVALID_ARG, "at most 255 beams");
     BeamHost b;
     b.frame = *frame;
     h->beams.push_back(b);
@@ -239,9 +257,37 @@ extern "C" int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int ma
     for (int iy = 0; iy < ny; ++iy)
         for (int ix = 0; ix < nx; ++ix)
             if (opening[(size_t)iy * nx + ix]) bits[(size_t)iy * rw + (ix >> 5)] |= 1u << (ix & 31);
+    // S0: safe-distance map.  Tile = 8 x 8 pixels; dist = Chebyshev distance in tiles to the nearest tile that is not
+    // fully open (everything outside the bitmap is brass), by the exact two-pass chamfer for the L-infinity metric.
+    const int ts = 1 << kApTileShift, ntx = (nx + ts - 1) / ts, nty = (ny + ts - 1) / ts;
+    std::vector<int> dist((size_t)ntx * nty, 0);
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            bool all = (tx + 1) * ts <= nx && (ty + 1) * ts <= ny;
+            for (int iy = ty * ts; all && iy < (ty + 1) * ts; ++iy)
+                for (int ix = tx * ts; ix < (tx + 1) * ts; ++ix)
+                    if (!opening[(size_t)iy * nx + ix]) { all = false; break; }
+            dist[(size_t)ty * ntx + tx] = all ? 255 : 0;
+        }
+    auto at = [&](int ty, int tx) { return (tx < 0 || ty < 0 || tx >= ntx || ty >= nty) ? 0 : dist[(size_t)ty * ntx + tx]; };
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            int &v = dist[(size_t)ty * ntx + tx];
+            v = std::min(v, std::min(std::min(at(ty - 1, tx - 1), at(ty - 1, tx)), std::min(at(ty - 1, tx + 1), at(ty, tx - 1))) + 1);
+        }
+    for (int ty = nty - 1; ty >= 0; --ty)
+        for (int tx = ntx - 1; tx >= 0; --tx) {
+            int &v = dist[(size_t)ty * ntx + tx];
+            v = std::min(v, std::min(std::min(at(ty + 1, tx + 1), at(ty + 1, tx)), std::min(at(ty + 1, tx - 1), at(ty, tx + 1))) + 1);
+        }
+    std::vector<unsigned char> dist8(dist.size());
+    for (size_t i = 0; i < dist.size(); ++i) dist8[i] = (unsigned char)std::min(dist[i], 255);
     free_beam(b);
     CU(h, cudaMalloc(&b.d_bits, bits.size() * sizeof(uint32_t)));
     CU(h, cudaMemcpy(b.d_bits, bits.data(), bits.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc(&b.d_dist, dist8.size()));
+    CU(h, cudaMemcpy(b.d_dist, dist8.data(), dist8.size(), cudaMemcpyHostToDevice));
+    b.ap_ntx = ntx; b.ap_nty = nty;
     b.has_ap = true; b.ap_T = thickness_mm; b.ap_face = downstream_face_mm > 0 ? downstream_face_mm : 150.0f;
     b.ap_nx = nx; b.ap_ny = ny; b.ap_row_words = rw; b.ap_u0 = u0; b.ap_v0 = v0; b.ap_du = du; b.ap_dv = dv;
     h->spots_dirty = true;

@@ -18,6 +18,15 @@ struct BeamHost {
     int ap_nx = 0, ap_ny = 0, ap_row_words = 0;
     float ap_u0 = 0, ap_v0 = 0, ap_du = 1, ap_dv = 1;
     uint32_t *d_bits = nullptr;       // packed opening bitmap on the device
+    unsigned char *d_dist = nullptr;  // safe-distance map of the opening (tiles of 8 x 8 pixels)
+    int ap_ntx = 0, ap_nty = 0;
+};
+
+// a device buffer that only grows
+struct DevBuf {
+    void *p = nullptr;
+    size_t bytes = 0;
+    template <class T> T *as() const { return static_cast<T *>(p); }
 };
 
 struct vpmc {
@@ -29,7 +38,7 @@ struct vpmc {
 
     // device-resident inputs
     short *d_hu = nullptr;
-    float4 *d_lut = nullptr;          // per-HU (rsp, rho, xsp/X0_w, za_w*rho)
+    float4 *d_lut = nullptr;          // per-HU (rsp, rho, xsp/X0_w, 1/rsp)
     std::vector<BeamHost> beams;
     bool spots_dirty = true;
     int n_spots = 0;
@@ -40,30 +49,30 @@ struct vpmc {
     std::vector<double> spot_w;       // weights in global spot order
     std::vector<int> spot_beam_h;
 
-    // work mapping
-    unsigned long long *d_cum = nullptr, *d_first = nullptr;
-    int map_capacity = 0;
-
-    // survivor queue
-    vpk::Queue q{};
-    unsigned int *d_qctr = nullptr;   // [0] count, [1] head
+    // work mapping (dose mode): [n_batches * n_spots + 1]
+    DevBuf cum, first;
+    DevBuf s0, s1, s2;                // source records of a chunk
+    DevBuf q0, q1, q2, q3, q4;        // survivor queue (grown to the chunk size in use)
+    unsigned int *d_qctr = nullptr;   // [0] queue count, [1] queue head, [2] source-record counter of beam_kernel
 
     // scoring
-    float *d_edep = nullptr;          // current batch E_dep (MeV)
-    float *d_sum = nullptr, *d_s1 = nullptr, *d_s2 = nullptr;
-    vpk::DevTallies *d_tal = nullptr;
+    DevBuf edep;                      // [n_batches][nvox] E_dep (MeV)
+    float *d_s1 = nullptr, *d_s2 = nullptr, *d_fb = nullptr;
+    vpk::DevTallies *d_tal = nullptr, *d_tal_scratch = nullptr;
     unsigned int *d_max_bits = nullptr;
     double *d_unc = nullptr;          // [0] sum, [1] count
     bool unc_valid = false;
 
-    // influence scratch (grown on demand)
-    void *d_inf[16] = { nullptr };
-    size_t inf_bytes[16] = { 0 };
+    // influence workspace (grown on demand)
+    DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_skip, inf_tilecnt, inf_colmax,
+        inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc;
+    size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
 
     // launch configuration
-    int voxel_grid[2][2] = { { 0, 0 }, { 0, 0 } };   // [mode][smem_lut]
+    int grid_beam = 0;                // resident CTAs of beam_kernel
+    int grid[3][2] = { { 0, 0 }, { 0, 0 }, { 0, 0 } };   // [mode][smem_lut] resident CTAs of voxel_kernel
     bool smem_lut = false;
-    size_t lut_bytes = 0;
+    size_t lut_bytes = 0, tally_smem = 0;
 
     unsigned long long win_lo = 0, win_hi = 0;
     cudaStream_t last_stream = nullptr;

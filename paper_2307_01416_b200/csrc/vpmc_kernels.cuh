@@ -1,46 +1,37 @@
-// vpmc_kernels.cuh -- the sm_100a kernels of the hot path and their launch-side
-// descriptors.  See DESIGN.md 5 for the launch structure:
-//   beamline_kernel   S1-S3: one thread per history; survivors are pushed (warp-aggregated) to a queue
-//   voxel_kernel      S4-S6b: persistent warps pull histories from the queue, refill dead lanes, score
-//   batch/dose/uncertainty kernels: S6 dose conversion and the C6 batch estimator
-//   influence kernels S7-S8: per-column private sub-volumes, threshold + scan + CSR emit
+// vpmc_kernels.cuh -- the sm_100a kernels of the hot path.  See DESIGN.md 5:
+//   beam_kernel       S1-S3: persistent warps carry histories through source, range shifter and aperture; lanes whose
+//                     history ended or left the beam line are refilled from a global item counter (warp-aggregated);
+//                     survivors are pushed to a queue
+//   voxel_kernel      S4-S7: persistent warps pull survivors from the queue, take the CT entry, step through the voxels
+//                     and score; MODE 0 the dose grid(s), MODE 1 per-column boxes, MODE 2 only column bounding boxes
+//   dose_finalize / uncertainty kernels: S6 dose conversion and the C6 batch estimator
+//   csr_* kernels     S8: threshold + count + scan + emit of the per-spot sparse columns
 #pragma once
 #include "vpmc_transport.cuh"
 
 namespace vpk {
 
-// history id <-> work item (C2)
+// work item -> (spot, history id, column / batch)   (C2)
 struct WorkMap {
     int mode;                         // 0 dose, 1 influence
     unsigned long long n_items;       // items of this launch
-    unsigned long long item0;         // first item of this launch within the batch
-    const unsigned long long *cum;    // dose: [n_spots+1] prefix of this batch's per-spot item counts
-    const unsigned long long *first;  // dose: [n_spots] first history id of this batch's sub-range of spot j
-    int n_spots;
-    unsigned int hps;                 // influence: histories per spot
-    int g0;                           // influence: first global spot (column) of this launch
+    // dose: entry e = batch * n_spots + spot; cum[e] = first item of the entry, first[e] = its first history id
+    const unsigned long long *cum;
+    const unsigned long long *first;
+    int n_entries, n_spots;
+    // influence: item k -> local column k / n_sub, history i = k % n_sub of global spot cols[c] (or g0 + c)
+    unsigned int hps, n_sub;
+    const int *cols;
+    int g0;
 };
 
-// survivors of the beam line, SoA of 16-byte records for coalesced access
-struct Queue {
-    float4 *q0;   // lx, ly, lz (local offsets in the entry voxel), E
-    float4 *q1;   // ux, uy, uz, t_rad    (CT frame)
-    float4 *q2;   // tau, tau_star, step (bits), R low word
-    uint4 *q3;    // hid_lo, hid_hi, voxel linear index, R high word
-    unsigned int *count;   // entries pushed
-    unsigned int *head;    // entries claimed by the voxel kernel
-    unsigned int capacity;
-};
-
-// influence-mode scoring target (S7): per-column private box in CT index space + overflow list
+// influence-mode scoring target (S7): per-column private box in CT index space
 struct ColumnBoxes {
     const int4 *lo;          // [n_cols] box low corner (ix, iy, iz, 0)
     const int4 *dim;         // [n_cols] box extent (bx, by, bz, 0)
     const unsigned long long *offset;   // [n_cols] offset of the box in `scratch`
-    float *scratch;          // concatenated boxes
-    unsigned int *ovf_count; // overflow entries appended
-    unsigned int ovf_capacity;
-    int *ovf_col; int *ovf_vox; float *ovf_val;
+    float *scratch;          // concatenated boxes (MeV)
+    int *bbox;               // [n_cols][6] min x,y,z, max x,y,z of deposits OUTSIDE the box (MODE 1) / of all (MODE 2)
 };
 
 __device__ __forceinline__ unsigned lanemask_lt()
@@ -54,265 +45,390 @@ __device__ __forceinline__ double warp_sum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
-__device__ __forceinline__ unsigned warp_sum(unsigned v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
 
-// block-level reduction of the per-thread tallies, then 13 global atomics per block
-__device__ void flush_tallies(const Tally &t, DevTallies *g)
-{
-    __shared__ double sd[6];
-    __shared__ unsigned int sc[7];
-    if (threadIdx.x < 6) sd[threadIdx.x] = 0.0;
-    if (threadIdx.x < 7) sc[threadIdx.x] = 0u;
-    __syncthreads();
-    const double d[6] = { t.incident, t.dep_ct, t.dep_rs, t.dep_brass, t.escaped, t.removed };
-    const unsigned c[7] = { t.n_stopped_ct, t.n_stopped_rs, t.n_stopped_brass, t.n_nuclear, t.n_escaped, t.n_steps_ct, t.n_steps_dev };
-    const int lane = threadIdx.x & 31;
-#pragma unroll
-    for (int i = 0; i < 6; ++i) { const double v = warp_sum(d[i]); if (lane == 0 && v != 0.0) atomicAdd(&sd[i], v); }
-#pragma unroll
-    for (int i = 0; i < 7; ++i) { const unsigned v = warp_sum(c[i]); if (lane == 0 && v) atomicAdd(&sc[i], v); }
-    __syncthreads();
-    if (threadIdx.x < 6 && sd[threadIdx.x] != 0.0) atomicAdd(&g->incident + threadIdx.x, sd[threadIdx.x]);
-    if (threadIdx.x < 7 && sc[threadIdx.x]) atomicAdd(&g->n_stopped_ct + threadIdx.x, (unsigned long long)sc[threadIdx.x]);
-}
-
-// item -> (global spot, history id)
-__device__ __forceinline__ void map_item(const WorkMap &wm, unsigned long long k, int &g, unsigned long long &hid)
+// item -> (global spot, history id, column or batch)
+__device__ __forceinline__ void map_item(const WorkMap &wm, unsigned long long k, int &g, unsigned long long &hid, int &col)
 {
     if (wm.mode == 0) {
-        int lo = 0, hi = wm.n_spots;           // largest g with cum[g] <= k and a non-empty range
+        int lo = 0, hi = wm.n_entries;           // largest e with cum[e] <= k (empty entries are skipped by the search)
         while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(wm.cum + mid) <= k) lo = mid; else hi = mid; }
-        g = lo;
-        hid = __ldg(wm.first + g) + (k - __ldg(wm.cum + g));
+        col = lo / wm.n_spots;                   // batch
+        g = lo - col * wm.n_spots;
+        hid = __ldg(wm.first + lo) + (k - __ldg(wm.cum + lo));
     } else {
-        const unsigned long long c = k / wm.hps;
-        g = wm.g0 + (int)c;
-        hid = (unsigned long long)g * wm.hps + (k - c * wm.hps);
+        const unsigned long long c = k / wm.n_sub;
+        col = (int)c;
+        g = wm.cols ? __ldg(wm.cols + c) : wm.g0 + (int)c;
+        hid = (unsigned long long)g * wm.hps + (k - c * wm.n_sub);
     }
 }
 
-// ------------------------------------------------------------------------------------------- S1-S3
-__global__ void __launch_bounds__(256)
-beamline_kernel(const DevParams P, const DevGrid G, const WorkMap wm, const float4 *__restrict__ spots,
-                const double *__restrict__ spot_R0, const int *__restrict__ spot_beam, const DevBeam *__restrict__ beams, const float3 shift,
-                const uint32_t k0, const uint32_t k1, const Queue q, DevTallies *tal)
+// ------------------------------------------------------------------------------------------- scorers (S6, S7)
+struct DoseScorer {            // MODE 0: E_dep[batch][v] += dE, fp32 RED into L2-resident grids
+    float *edep; unsigned long long nvox;
+    __device__ __forceinline__ void begin(const Hist &) {}
+    __device__ __forceinline__ void deposit(const Hist &h, float dep) { atomicAdd(edep + (size_t)h.col * nvox + h.g3, dep); }
+    __device__ __forceinline__ void end(const Hist &) {}
+};
+
+__device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int x1, int y1, int z1)
+{
+    atomicMin(bb + 0, x0); atomicMin(bb + 1, y0); atomicMin(bb + 2, z0);
+    atomicMax(bb + 3, x1); atomicMax(bb + 4, y1); atomicMax(bb + 5, z1);
+}
+
+struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it only grows the column's overflow bbox
+    ColumnBoxes cb;
+    __device__ __forceinline__ void begin(const Hist &) {}
+    __device__ __forceinline__ void deposit(const Hist &h, float dep)
+    {
+        const int c = h.col;
+        const int4 lo = __ldg(cb.lo + c), dm = __ldg(cb.dim + c);
+        const int bx = (int)h.g0 - lo.x, by = (int)h.g1 - lo.y, bz = (int)h.g2 - lo.z;
+        if ((unsigned)bx < (unsigned)dm.x && (unsigned)by < (unsigned)dm.y && (unsigned)bz < (unsigned)dm.z)
+            atomicAdd(cb.scratch + __ldg(cb.offset + c) + (bx + (unsigned long long)dm.x * (by + (unsigned long long)dm.y * bz)), dep);
+        else
+            bbox_merge(cb.bbox + 6 * c, (int)h.g0, (int)h.g1, (int)h.g2, (int)h.g0, (int)h.g1, (int)h.g2);
+    }
+    __device__ __forceinline__ void end(const Hist &) {}
+};
+
+struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits of each column
+    int *bbox;
+    int x0, y0, z0, x1, y1, z1;
+    __device__ __forceinline__ void begin(const Hist &) { x0 = y0 = z0 = 0x7fffffff; x1 = y1 = z1 = -1; }
+    __device__ __forceinline__ void deposit(const Hist &h, float)
+    {
+        x0 = min(x0, (int)h.g0); y0 = min(y0, (int)h.g1); z0 = min(z0, (int)h.g2);
+        x1 = max(x1, (int)h.g0); y1 = max(y1, (int)h.g1); z1 = max(z1, (int)h.g2);
+    }
+    __device__ __forceinline__ void end(const Hist &h) { if (x1 >= 0) bbox_merge(bbox + 6 * h.col, x0, y0, z0, x1, y1, z1); }
+};
+
+template <int MODE> struct ScorerOf;
+template <> struct ScorerOf<0> { typedef DoseScorer type; };
+template <> struct ScorerOf<1> { typedef BoxScorer type; };
+template <> struct ScorerOf<2> { typedef BoundsScorer type; };
+
+struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; };
+
+template <int MODE> __device__ __forceinline__ typename ScorerOf<MODE>::type make_scorer(const ScoreArgs &a);
+template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox }; }
+template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { return BoxScorer{ a.cb }; }
+template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; return s; }
+
+// ------------------------------------------------------------------------------------------- S1-S7
+// Pipeline of one chunk of work items:
+//   source_kernel  one thread per item: item -> spot, history id; S1 sampling; writes a 48-byte source record
+//   beam_kernel    persistent warps step histories through range shifter and aperture; a free lane is refilled by
+//                  LOADING the next source record (cheap, so lanes are refilled eagerly); survivors -> queue
+//   entry_kernel   one thread per survivor: beam frame -> CT frame, ray-box entry (fp64), record rewritten in place
+//   voxel_kernel   persistent warps step survivors through the voxels and score; refill = loading a record
+// The expensive once-per-history work (Philox + accurate log / sincos of the source, the fp64 CT entry) runs in plain
+// fully converged kernels; the persistent kernels contain nothing but the step loop.
+constexpr int kBlock = 256;
+constexpr int kWarps = kBlock / 32;
+#ifndef VPK_REFILL_MIN
+#define VPK_REFILL_MIN 4
+#endif
+constexpr int kRefillMin = VPK_REFILL_MIN;   // S6b: free lanes are refilled once at least this many of a warp's lanes are free
+
+#ifndef VPK_MIN_BLOCKS
+#define VPK_MIN_BLOCKS 3
+#endif
+
+// source records of a chunk, SoA of 16-byte words
+struct SourceBuf {
+    uint4 *s0;    // x hi, x lo, y hi, y lo (beam frame, fp32 pairs)
+    uint4 *s1;    // E, tau_star, col | beam << 24, region
+    uint4 *s2;    // R lo, R hi, hid_lo, hid_hi
+};
+
+// Histories that left the beam line alive, handed from beam_kernel to voxel_kernel: SoA of 16-byte records (80 B per
+// history), written and read coalesced.  beam_kernel writes the beam-frame state on the exit plane of the last device;
+// entry_kernel rewrites q0 (and the direction) as the CT state.
+struct Queue {
+    uint4 *q0;    // beam frame: x hi, x lo, y hi, y lo;  CT: local x, y, z (fp32), voxel index (0xffffffff = missed the CT)
+    float4 *q1;   // ux, uy, uz, E
+    float4 *q2;   // lx, ly, lz, t_rad
+    uint4 *q3;    // tau, tau_star, step, col | beam << 24
+    uint4 *q4;    // R lo, R hi, hid_lo, hid_hi
+    unsigned int *count;   // entries pushed
+    unsigned int *head;    // entries claimed by the voxel kernel
+    unsigned int capacity;
+};
+
+// per-warp flush of the tallies: lane counters into the warp's shared slots, then <= 13 global atomics per warp
+__device__ __forceinline__ void flush_warp_tallies(WarpTally *w, const LaneCounters &lc, DevTallies *tal, int lane)
+{
+    const double inc = warp_sum(lc.incident);
+    const unsigned nct = __reduce_add_sync(0xffffffffu, lc.n_ct), ndev = __reduce_add_sync(0xffffffffu, lc.n_dev);
+    __syncwarp();
+    if (lane == 0) { w->d[TD_INCIDENT] += inc; w->c[TC_STEPS_CT] += nct; w->c[TC_STEPS_DEV] += ndev; }
+    __syncwarp();
+    if (lane < TD_N && w->d[lane] != 0.0) atomicAdd(&tal->incident + lane, w->d[lane]);
+    if (lane < TC_N && w->c[lane]) atomicAdd(&tal->n_stopped_ct + lane, (unsigned long long)w->c[lane]);
+}
+
+// S1: items [item0, item0 + n) -> source records [0, n)
+__global__ void __launch_bounds__(kBlock)
+source_kernel(const Ctx c, const WorkMap wm, const unsigned long long item0, const float4 *__restrict__ spots,
+              const double *__restrict__ spot_R0, const int *__restrict__ spot_beam, const SourceBuf sb, DevTallies *tal)
 {
     const unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    Tally t;
-    Hist h;
-    int iv[3] = { 0, 0, 0 };
-    int g = 0;
-    bool alive = false;
+    double inc = 0.0;
     if (k < wm.n_items) {
-        unsigned long long hid;
-        map_item(wm, wm.item0 + k, g, hid);
+        Hist h;
+        int g; unsigned long long hid;
+        map_item(wm, item0 + k, g, hid, h.col);
         h.hid_lo = (uint32_t)hid; h.hid_hi = (uint32_t)(hid >> 32);
-        const DevBeam b = beams[__ldg(spot_beam + g)];
-        sample_source(P, __ldg(spots + g), __ldg(spot_R0 + g), h, k0, k1);
-        t.incident = (double)h.E;
-        NullTracer tr;
-        const float sh[3] = { shift.x, shift.y, shift.z };
-        float w_now;
-        if (beamline(P, b, h, t, tr, k0, k1, w_now) == CONT) alive = enter_ct(G, b, sh, w_now, h, iv, t, tr) == CONT;
-        t.n_steps_dev = h.step;
+        const int beam = __ldg(spot_beam + g);
+        sample_source(c.P, c.beams[beam], beam, __ldg(spots + g), __ldg(spot_R0 + g), h, c.k0, c.k1);
+        inc = (double)h.E;
+        const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
+        sb.s0[k] = make_uint4(h.g0, h.g1, h.g2, h.g3);
+        sb.s1[k] = make_uint4(__float_as_uint(h.E), __float_as_uint(h.tau_star), (unsigned)h.col | ((unsigned)beam << 24), (unsigned)(h.region & 0xff));
+        sb.s2[k] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
     }
-    // S6b, first stage: only survivors enter the voxel queue (warp-aggregated slot claim)
-    const unsigned mask = __ballot_sync(0xffffffffu, alive);
-    if (mask) {
-        unsigned base = 0;
-        const int leader = __ffs(mask) - 1;
-        if ((threadIdx.x & 31) == leader) base = atomicAdd(q.count, __popc(mask));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (alive) {
-            const unsigned slot = base + __popc(mask & lanemask_lt());
-            if (slot < q.capacity) {
-                q.q0[slot] = make_float4(h.rx, h.ry, h.rz, h.E);
-                q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.t_rad);
-                const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
-                q.q2[slot] = make_float4(h.tau, h.tau_star, __uint_as_float(h.step), __uint_as_float((unsigned)rb));
-                q.q3[slot] = make_uint4(h.hid_lo, h.hid_hi, (unsigned)(iv[0] + G.nx * (iv[1] + G.ny * iv[2])), (unsigned)(rb >> 32));
-            }
-        }
-    }
-    flush_tallies(t, tal);
+    inc = warp_sum(inc);
+    if ((threadIdx.x & 31) == 0 && inc != 0.0) atomicAdd(&tal->incident, inc);
 }
 
-// ------------------------------------------------------------------------------------------- S4-S6
-// One CT step of history h in voxel (ix,iy,iz): returns the cause; v = voxel of the deposit, o.dep its size.
-template <class Tracer, class Lut>
-__device__ __forceinline__ int ct_step(const DevParams &P, const DevGrid &G, const short *__restrict__ hu, const Lut &lut,
-                                       float rsp_scale, Hist &h, int &ix, int &iy, int &iz, long long &v, StepOut &o,
-                                       Tracer &tr, uint32_t k0, uint32_t k1)
+// S2-S3: persistent warps; every lane carries one history through the beam line with beam_step(); a lane whose history
+// ended or left the beam line loads the next source record (warp-aggregated claim on the item counter).  Survivors are
+// pushed to the queue with one atomic per warp and iteration.
+__global__ void __launch_bounds__(kBlock, VPK_MIN_BLOCKS)
+beam_kernel(const Ctx c, const unsigned int n_items, const SourceBuf sb, const Queue q, unsigned int *counter, DevTallies *tal)
 {
-    int ax;
-    const float d = face_distance(G, h, ax);
-    const bool up = (ax == 0 ? h.ux : (ax == 1 ? h.uy : h.uz)) > 0.0f;   // direction of travel during the step
-    v = ix + (long long)G.nx * (iy + (long long)G.ny * iz);
-    int t = (int)__ldg(hu + v) - G.hu_min;
-    t = min(max(t, 0), G.n_lut - 1);
-    const float4 mv = lut[t];
-    const Medium m = { mv.x * rsp_scale, mv.y, mv.z, mv.w };
-    const float Eb = h.E; const uint32_t st = h.step;
-    const int iv0[3] = { ix, iy, iz };
-    int cause = material_step(P, h, m, d, k0, k1, o);
-    if (cause == CONT && o.on_d && cross_face(G, h, ix, iy, iz, ax, up)) cause = ESCAPED;
-    tr.put(h, fmaf((float)ix, G.hx, G.ox), fmaf((float)iy, G.hy, G.oy), fmaf((float)iz, G.hz, G.oz), st, REG_CT, iv0,
-           Eb, h.E, o.s, cause);
-    return cause;
-}
-
-struct LutShared { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return p[i]; } };
-struct LutGlobal { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return __ldg(p + i); } };
-
-// MODE 0: dose grid; MODE 1: per-column boxes.  SMEM_LUT: material table staged in shared memory.
-template <int MODE, bool SMEM_LUT>
-__global__ void __launch_bounds__(256)
-voxel_kernel(const DevParams P, const DevGrid G, const Queue q, const short *__restrict__ hu,
-             const float4 *__restrict__ lut_g, const float rsp_scale, float *__restrict__ edep,
-             const ColumnBoxes cb, const int col0, const unsigned int hps, const uint32_t k0, const uint32_t k1,
-             DevTallies *tal)
-{
-    extern __shared__ float4 lut_s[];
-    if (SMEM_LUT) {
-        for (int i = threadIdx.x; i < G.n_lut; i += blockDim.x) lut_s[i] = lut_g[i];
-        __syncthreads();
-    }
-    const unsigned n_q = min(*q.count, q.capacity);
-    const int lane = threadIdx.x & 31;
-    Tally t;
+    __shared__ WarpTally wt_all[kWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < kWarps * (int)(sizeof(WarpTally) / 4)) reinterpret_cast<unsigned int *>(wt_all)[threadIdx.x] = 0u;
+    __syncthreads();
+    const SmemSink sink{ wt_all + warp };
+    NullTracer tr;
+    LaneCounters lc;
     Hist h;
-    int ix = 0, iy = 0, iz = 0, col = 0;
+    h.region = REG_TO_CT; h.col = 0; h.step = 0u;
     float hdep = 0.0f;
     bool alive = false, exhausted = false;
-    NullTracer tr;
     for (;;) {
-        // S6b: refill dead lanes from the queue (one atomic per warp)
-        const unsigned need = __ballot_sync(0xffffffffu, !alive);
-        if (need && !exhausted) {
+        const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
+        const int n_free = __popc(free_mask);
+        if (!exhausted && (n_free >= kRefillMin || n_free == 32)) {
             unsigned base = 0;
-            const int leader = __ffs(need) - 1;
-            const int cnt = __popc(need);
-            if (lane == leader) base = atomicAdd(q.head, cnt);
+            const int leader = __ffs(free_mask) - 1;
+            if (lane == leader) base = atomicAdd(counter, (unsigned)n_free);
             base = __shfl_sync(0xffffffffu, base, leader);
-            exhausted = base + cnt >= n_q;
+            exhausted = base + (unsigned)n_free >= n_items;
             if (!alive) {
-                const unsigned slot = base + __popc(need & lanemask_lt());
-                if (slot < n_q) {
-                    const float4 a = q.q0[slot], b = q.q1[slot], c = q.q2[slot];
-                    const uint4 e = q.q3[slot];
-                    h.rx = a.x; h.ry = a.y; h.rz = a.z; h.E = a.w;
-                    h.ux = b.x; h.uy = b.y; h.uz = b.z; h.t_rad = b.w; h.A_rad = highland_A(b.w, P.c_log);
-                    h.tau = c.x; h.tau_star = c.y; h.step = __float_as_uint(c.z);
-                    h.R = __longlong_as_double((long long)(((unsigned long long)e.w << 32) | __float_as_uint(c.w)));
-                    h.hid_lo = e.x; h.hid_hi = e.y;
-                    iz = (int)(e.z / (unsigned)(G.nx * G.ny));
-                    const int rem = (int)(e.z - (unsigned)iz * (unsigned)(G.nx * G.ny));
-                    iy = rem / G.nx; ix = rem - iy * G.nx;
-                    if (MODE == 1) col = (int)((((unsigned long long)e.y << 32) | e.x) / hps);
+                const unsigned k = base + __popc(free_mask & lanemask_lt());
+                if (k < n_items) {
+                    const uint4 a = sb.s0[k], b = sb.s1[k], e = sb.s2[k];
+                    h.g0 = a.x; h.g1 = a.y; h.g2 = a.z; h.g3 = a.w;
+                    h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
+                    h.E = __uint_as_float(b.x); h.tau_star = __uint_as_float(b.y);
+                    h.col = (int)(b.z & 0xffffffu); h.region = (int)b.w | (int)((b.z >> 24) << 8);
+                    h.R = __longlong_as_double((long long)(((unsigned long long)e.y << 32) | e.x));
+                    h.hid_lo = e.z; h.hid_hi = e.w;
+                    h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
+                    h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
                     hdep = 0.0f;
                     alive = true;
                 }
             }
         }
-        if (!__any_sync(0xffffffffu, alive)) break;
-        if (alive) {
-            long long v; StepOut o;
-            int cause;
-            const int vx = ix, vy = iy, vz = iz;      // voxel of the deposit = voxel at the start of the step
-            if (SMEM_LUT) cause = ct_step(P, G, hu, LutShared{ lut_s }, rsp_scale, h, ix, iy, iz, v, o, tr, k0, k1);
-            else cause = ct_step(P, G, hu, LutGlobal{ lut_g }, rsp_scale, h, ix, iy, iz, v, o, tr, k0, k1);
-            t.n_steps_ct += (cause != STOPPED);
-            if (o.dep != 0.0f) {
-                if (MODE == 0) {
-                    atomicAdd(edep + v, o.dep);
-                } else {
-                    const int c = col - col0;
-                    const int4 lo = __ldg(cb.lo + c), dm = __ldg(cb.dim + c);
-                    const int bx = vx - lo.x, by = vy - lo.y, bz = vz - lo.z;
-                    if ((unsigned)bx < (unsigned)dm.x && (unsigned)by < (unsigned)dm.y && (unsigned)bz < (unsigned)dm.z) {
-                        atomicAdd(cb.scratch + __ldg(cb.offset + c) + (bx + (unsigned long long)dm.x * (by + (unsigned long long)dm.y * bz)), o.dep);
-                    } else {
-                        const unsigned s = atomicAdd(cb.ovf_count, 1u);
-                        if (s < cb.ovf_capacity) { cb.ovf_col[s] = col; cb.ovf_vox[s] = (int)v; cb.ovf_val[s] = o.dep; }
-                    }
+        if (!__any_sync(0xffffffffu, alive)) {
+            if (exhausted) break;
+            continue;
+        }
+        int code = BEAM_CONT;
+        if (alive) code = beam_step(c, h, hdep, lc, sink, tr);
+        // survivors -> queue (one atomic per warp)
+        const unsigned out_mask = __ballot_sync(0xffffffffu, alive && code == BEAM_EXIT);
+        if (out_mask) {
+            unsigned base = 0;
+            const int leader = __ffs(out_mask) - 1;
+            if (lane == leader) base = atomicAdd(q.count, (unsigned)__popc(out_mask));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (alive && code == BEAM_EXIT) {
+                const unsigned slot = base + __popc(out_mask & lanemask_lt());
+                if (slot < q.capacity) {
+                    q.q0[slot] = make_uint4(h.g0, h.g1, h.g2, h.g3);
+                    q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.E);
+                    q.q2[slot] = make_float4(h.lx, h.ly, h.lz, h.t_rad);
+                    q.q3[slot] = make_uint4(__float_as_uint(h.tau), __float_as_uint(h.tau_star), h.step,
+                                            (unsigned)h.col | ((unsigned)(h.region >> 8) << 24));
+                    const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
+                    q.q4[slot] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
                 }
-                hdep += o.dep;
-            }
-            if (cause != CONT) {
-                t.dep_ct += (double)hdep;
-                t.removed += (double)o.removed;
-                book_end(t, cause, REG_CT, cause == ESCAPED ? h.E : 0.0f);
-                alive = false;
             }
         }
+        if (code != BEAM_CONT) alive = false;
     }
-    flush_tallies(t, tal);
+    flush_warp_tallies(wt_all + warp, lc, tal, lane);
 }
 
-// ------------------------------------------------------------------------------------------- trace
-template <bool DUMMY>
-__global__ void trace_kernel(const DevParams P, const DevGrid G, const unsigned long long *__restrict__ hids,
-                             const int *__restrict__ spot_of, int n, const float4 *__restrict__ spots,
-                             const double *__restrict__ spot_R0, const int *__restrict__ spot_beam, const DevBeam *__restrict__ beams, const float3 shift,
-                             const short *__restrict__ hu, const float4 *__restrict__ lut_g, float rsp_scale,
-                             uint32_t k0, uint32_t k1, StepRec *recs, int max_steps, int *nrec)
+// CT entry of the survivors (C3), one thread per queue entry: q0 becomes (local x, y, z, voxel index) and the direction
+// the CT-frame direction.  A history that misses the CT box is booked as ESCAPED and its record marked.
+__global__ void __launch_bounds__(kBlock)
+entry_kernel(const Ctx c, const Queue q, DevTallies *tal)
+{
+    const unsigned n_q = min(*q.count, q.capacity);
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    double esc = 0.0; unsigned n_esc = 0, n_dev = 0;
+    if (i < n_q) {
+        Hist h;
+        const uint4 p0 = q.q0[i];
+        const float4 a = q.q1[i], b = q.q2[i];
+        const uint4 e = q.q3[i];
+        h.g0 = p0.x; h.g1 = p0.y; h.g2 = p0.z; h.g3 = p0.w;
+        h.ux = a.x; h.uy = a.y; h.uz = a.z; h.E = a.w;
+        h.lx = b.x; h.ly = b.y; h.lz = b.z;
+        h.step = e.z; h.hid_lo = 0u; h.hid_hi = 0u;
+        const DevBeam *bp = c.beams + (e.w >> 24);
+        const float w_now = bp->has_ap ? bp->w_ap_out : (bp->has_rs ? bp->w_rs_out : bp->w_start);
+        NullTracer tr;
+        const int ec = enter_ct(c, *bp, w_now, h, tr);
+        n_dev = h.step;
+        if (ec != CONT) { esc = (double)h.E; n_esc = 1u; h.g3 = 0xffffffffu; }
+        q.q0[i] = make_uint4(__float_as_uint(h.rx), __float_as_uint(h.ry), __float_as_uint(h.rz), h.g3);
+        q.q1[i] = make_float4(h.ux, h.uy, h.uz, a.w);
+        q.q2[i] = make_float4(h.lx, h.ly, h.lz, b.w);
+        q.q3[i] = make_uint4(e.x, e.y, h.step, e.w);
+    }
+    esc = warp_sum(esc);
+    n_esc = __reduce_add_sync(0xffffffffu, n_esc); n_dev = __reduce_add_sync(0xffffffffu, n_dev);
+    if ((threadIdx.x & 31) == 0) {
+        if (esc != 0.0) atomicAdd(&tal->escaped, esc);
+        if (n_esc) atomicAdd(&tal->n_escaped, (unsigned long long)n_esc);
+        if (n_dev) atomicAdd(&tal->n_steps_dev, (unsigned long long)n_dev);
+    }
+}
+
+// S4-S7: persistent warps; free lanes load survivors from the queue (one atomic per warp and refill) and step through
+// the voxels with ct_step().  MODE 0 scores the dose grid(s), MODE 1 per-column boxes, MODE 2 only column bounding
+// boxes.  SMEM_LUT: material table staged in shared memory.
+template <int MODE, bool SMEM_LUT>
+__global__ void __launch_bounds__(kBlock, VPK_MIN_BLOCKS)
+voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const ScoreArgs sa, DevTallies *tal)
+{
+    extern __shared__ float4 smem4[];
+    WarpTally *wt_all = reinterpret_cast<WarpTally *>(smem4);
+    float4 *lut_s = smem4 + (kWarps * sizeof(WarpTally) + 15) / 16;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < kWarps * (int)(sizeof(WarpTally) / 4)) reinterpret_cast<unsigned int *>(wt_all)[threadIdx.x] = 0u;
+    if (SMEM_LUT)
+        for (int i = threadIdx.x; i < c.G.n_lut; i += blockDim.x) lut_s[i] = lut_g[i];
+    __syncthreads();
+    const SmemSink sink{ wt_all + warp };
+    typename ScorerOf<MODE>::type sc = make_scorer<MODE>(sa);
+    NullTracer tr;
+    LaneCounters lc;
+    Hist h;
+    h.region = REG_CT; h.col = 0; h.step = 0u;
+    float hdep = 0.0f;
+    const unsigned n_q = min(*q.count, q.capacity);
+    const unsigned nxy = (unsigned)(c.G.nx * c.G.ny);
+    bool alive = false, exhausted = false;
+    for (;;) {
+        const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
+        const int n_free = __popc(free_mask);
+        if (!exhausted && (n_free >= kRefillMin || n_free == 32)) {
+            unsigned base = 0;
+            const int leader = __ffs(free_mask) - 1;
+            if (lane == leader) base = atomicAdd(q.head, (unsigned)n_free);
+            base = __shfl_sync(0xffffffffu, base, leader);
+            exhausted = base + (unsigned)n_free >= n_q;
+            if (!alive) {
+                const unsigned slot = base + __popc(free_mask & lanemask_lt());
+                if (slot < n_q) {
+                    const uint4 p0 = q.q0[slot];
+                    if (p0.w != 0xffffffffu) {
+                        const float4 a = q.q1[slot], b = q.q2[slot];
+                        const uint4 e = q.q3[slot], f = q.q4[slot];
+                        h.rx = __uint_as_float(p0.x); h.ry = __uint_as_float(p0.y); h.rz = __uint_as_float(p0.z);
+                        h.g3 = p0.w;
+                        h.g2 = p0.w / nxy;
+                        const unsigned rem = p0.w - h.g2 * nxy;
+                        h.g1 = rem / (unsigned)c.G.nx; h.g0 = rem - h.g1 * (unsigned)c.G.nx;
+                        h.ux = a.x; h.uy = a.y; h.uz = a.z; h.E = a.w;
+                        h.lx = b.x; h.ly = b.y; h.lz = b.z; h.t_rad = b.w; h.f_rad = highland_f(b.w, c.P.c_log);
+                        h.tau = __uint_as_float(e.x); h.tau_star = __uint_as_float(e.y); h.step = e.z;
+                        h.col = (int)(e.w & 0xffffffu); h.region = REG_CT | (int)((e.w >> 24) << 8);
+                        h.R = __longlong_as_double((long long)(((unsigned long long)f.y << 32) | f.x));
+                        h.hid_lo = f.z; h.hid_hi = f.w;
+                        hdep = 0.0f;
+                        sc.begin(h);
+                        alive = true;
+                    }
+                }
+            }
+        }
+        if (!__any_sync(0xffffffffu, alive)) {
+            if (exhausted) break;
+            continue;
+        }
+        if (alive) {
+            int cause;
+            if (SMEM_LUT) cause = ct_step(c, LutShared{ lut_s }, h, hdep, lc, sc, sink, tr);
+            else cause = ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, sink, tr);
+            if (cause != CONT) { sc.end(h); alive = false; }
+        }
+    }
+    flush_warp_tallies(wt_all + warp, lc, tal, lane);
+}
+
+// ------------------------------------------------------------------------------------------- trace (test-only)
+__global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__ hids, const int *__restrict__ spot_of, int n,
+                             const float4 *__restrict__ spots, const double *__restrict__ spot_R0,
+                             const int *__restrict__ spot_beam, const float4 *__restrict__ lut_g,
+                             StepRec *recs, int max_steps, int *nrec)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     RecTracer tr{ recs + (size_t)i * max_steps, max_steps, 0 };
     const int g = spot_of[i];
     if (g < 0) { nrec[i] = 0; return; }
-    Hist h; Tally t;
+    Hist h; LaneCounters lc; NullScorer sc; NullSink sink;
+    float hdep = 0.0f;
+    h.col = 0;
     h.hid_lo = (uint32_t)hids[i]; h.hid_hi = (uint32_t)(hids[i] >> 32);
-    const DevBeam b = beams[spot_beam[g]];
-    sample_source(P, spots[g], spot_R0[g], h, k0, k1);
-    int iv[3];
-    const float sh[3] = { shift.x, shift.y, shift.z };
-    float w_now;
-    if (beamline(P, b, h, t, tr, k0, k1, w_now) == CONT && enter_ct(G, b, sh, w_now, h, iv, t, tr) == CONT) {
-        int ix = iv[0], iy = iv[1], iz = iv[2];
-        for (int it = 0; it < 1000000; ++it) {
-            long long v; StepOut o;
-            if (ct_step(P, G, hu, LutGlobal{ lut_g }, rsp_scale, h, ix, iy, iz, v, o, tr, k0, k1) != CONT) break;
-        }
+    const int beam = spot_beam[g];
+    sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.k0, c.k1);
+    int code = BEAM_CONT;
+    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, hdep, lc, sink, tr);
+    if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
+        hdep = 0.0f;
+        for (int it = 0; it < 1000000; ++it)
+            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, sink, tr) != CONT) break;
     }
     nrec[i] = tr.n;
 }
 
 // ------------------------------------------------------------------------------------------- S6 / C6
-// fold one batch into the running sums; f = N / N_b scales the batch to full weight
-__global__ void batch_accumulate_kernel(float *__restrict__ edep_b, float *__restrict__ sum, float *__restrict__ s1,
-                                        float *__restrict__ s2, long long n, float f, int with_unc)
-{
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
-        const float x = edep_b[v];
-        if (x != 0.0f) {
-            edep_b[v] = 0.0f;
-            sum[v] += x;
-            if (with_unc) { const float y = f * x; s1[v] += y; s2[v] = fmaf(y, y, s2[v]); }
-        }
-    }
-}
-
-// dose[v] = scale * E_dep[v] / (max(rho_v, rho_min) V[cm3]) * 1.602176634e-10 Gy
-__global__ void dose_convert_kernel(const float *__restrict__ sum, const short *__restrict__ hu,
-                                    const float4 *__restrict__ lut, DevGrid G, float rho_min, float coef,
-                                    float *__restrict__ dose, long long n, unsigned int *max_bits)
+// One pass over the B batch grids: dose[v] = coef * sum_b E_b[v] / max(rho_v, rho_min); with B >= 2 also the batch
+// sums s1 = sum_b f_b E_b, s2 = sum_b (f_b E_b)^2 (f_b = N / N_b scales a batch to full weight) for C6.
+__global__ void dose_finalize_kernel(const float *__restrict__ edep, int B, const float *__restrict__ fb,
+                                     const short *__restrict__ hu, const float4 *__restrict__ lut, DevGrid G, float rho_min,
+                                     float coef, float *__restrict__ dose, float *__restrict__ s1, float *__restrict__ s2,
+                                     long long n, unsigned int *max_bits)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     float mx = 0.0f;
     for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        float sum = 0.0f, a1 = 0.0f, a2 = 0.0f;
+        for (int b = 0; b < B; ++b) {
+            const float x = edep[(size_t)b * n + v];
+            sum += x;
+            const float y = __ldg(fb + b) * x;
+            a1 += y; a2 = fmaf(y, y, a2);
+        }
         int t = (int)__ldg(hu + v) - G.hu_min;
         t = min(max(t, 0), G.n_lut - 1);
         const float rho = fmaxf(__ldg(lut + t).y, rho_min);
-        const float dv = __fdiv_rn(coef * sum[v], rho);
+        const float dv = __fdiv_rn(coef * sum, rho);
         dose[v] = dv;
+        if (s1) { s1[v] = a1; s2[v] = a2; }
         mx = fmaxf(mx, dv);
     }
 #pragma unroll
@@ -341,6 +457,192 @@ __global__ void uncertainty_kernel(const float *__restrict__ dose, const float *
     }
     s = warp_sum(s); c = warp_sum(c);
     if ((threadIdx.x & 31) == 0 && c > 0.0) { atomicAdd(acc, s); atomicAdd(acc + 1, c); }
+}
+
+// ------------------------------------------------------------------------------------------- S8: CSR writer
+// A "column" is a dense fp32 box (lo, dim) of the CT grid stored contiguously at scratch + offset, element
+// e = bx + dim.x (by + dim.y bz), so ascending e is ascending voxel index v.  Columns are cut into tiles of kTile
+// elements; tile t of the launch belongs to the column found by binary search in tile0[] (prefix of tiles per column).
+// Passes: (1) convert E_dep -> dose value and take the column maximum; (2) count the kept entries per tile
+// (val > 0 and val >= rel_thr * max, product in fp32); (3) per column: exclusive scan of its tile counts;
+// (4) emit (voxel index, value) at base[c] + tile_off + rank.  vpmc_csr_from_dense runs (1) without the conversion on a
+// single column of shape (n, 1, 1), so the writer the tests pin bit-exactly is the writer the influence path uses.
+constexpr int kTile = 2048;
+constexpr int kPerThread = kTile / kBlock;
+
+struct CsrCols {
+    const int4 *lo, *dim;
+    const unsigned long long *offset;   // element offset of each column in `data`
+    const int *tile0;                   // [n_cols + 1] prefix of tiles per column
+    const int *skip;                    // [n_cols] or NULL: non-zero = column not written in this round
+    int n_cols, n_tiles;
+    int nx, ny;                         // of the CT grid (voxel index of box element)
+};
+
+__device__ __forceinline__ int tile_column(const CsrCols &cc, int tile)
+{
+    int lo = 0, hi = cc.n_cols;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(cc.tile0 + mid) <= tile) lo = mid; else hi = mid; }
+    return lo;
+}
+
+// first element of this thread in its tile -> (e, bx, by, bz); returns the number of elements it owns (0..kPerThread)
+__device__ __forceinline__ int tile_thread_range(const CsrCols &cc, int tile, int c, const int4 dm, long long &e, int &bx, int &by, int &bz)
+{
+    const long long vol = (long long)dm.x * dm.y * dm.z;
+    e = (long long)(tile - __ldg(cc.tile0 + c)) * kTile + (long long)threadIdx.x * kPerThread;
+    if (e >= vol) return 0;
+    const long long row = e / dm.x;
+    bx = (int)(e - row * dm.x);
+    bz = (int)(row / dm.y);
+    by = (int)(row - (long long)bz * dm.y);
+    const long long left = vol - e;
+    return left < kPerThread ? (int)left : kPerThread;
+}
+__device__ __forceinline__ void box_next(const int4 dm, int &bx, int &by, int &bz)
+{
+    if (++bx == dm.x) { bx = 0; if (++by == dm.y) { by = 0; ++bz; } }
+}
+
+template <bool CONVERT>
+__global__ void __launch_bounds__(kBlock)
+csr_max_kernel(const CsrCols cc, float *__restrict__ data, const short *__restrict__ hu, const float4 *__restrict__ lut,
+               int hu_min, int n_lut, float rho_min, float coef, unsigned int *__restrict__ colmax_bits)
+{
+    for (int tile = blockIdx.x; tile < cc.n_tiles; tile += gridDim.x) {
+        const int c = tile_column(cc, tile);
+        if (cc.skip && __ldg(cc.skip + c)) continue;
+        const int4 lo = __ldg(cc.lo + c), dm = __ldg(cc.dim + c);
+        long long e; int bx = 0, by = 0, bz = 0;
+        const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
+        float *p = data + __ldg(cc.offset + c) + e;
+        float mx = 0.0f;
+        for (int i = 0; i < cnt; ++i) {
+            float x = p[i];
+            if (CONVERT && x != 0.0f) {
+                const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
+                int t = (int)__ldg(hu + v) - hu_min;
+                t = min(max(t, 0), n_lut - 1);
+                x = __fdiv_rn(coef * x, fmaxf(__ldg(lut + t).y, rho_min));
+                p[i] = x;
+            }
+            mx = fmaxf(mx, x);
+            if (CONVERT) box_next(dm, bx, by, bz);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if ((threadIdx.x & 31) == 0 && mx > 0.0f) atomicMax(colmax_bits + c, __float_as_uint(mx));
+    }
+}
+
+__device__ __forceinline__ bool csr_keep(float x, float thr) { return x > 0.0f && x >= thr; }
+
+__global__ void __launch_bounds__(kBlock)
+csr_count_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned int *__restrict__ colmax_bits, float rel_thr,
+                 unsigned int *__restrict__ tile_count)
+{
+    __shared__ unsigned int wsum[kWarps];
+    for (int tile = blockIdx.x; tile < cc.n_tiles; tile += gridDim.x) {
+        const int c = tile_column(cc, tile);
+        unsigned int k = 0;
+        if (!(cc.skip && __ldg(cc.skip + c))) {
+            const int4 dm = __ldg(cc.dim + c);
+            long long e; int bx, by, bz;
+            const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
+            const float *p = data + __ldg(cc.offset + c) + e;
+            const float thr = rel_thr * __uint_as_float(__ldg(colmax_bits + c));
+            for (int i = 0; i < cnt; ++i) k += csr_keep(p[i], thr) ? 1u : 0u;
+        }
+        k = __reduce_add_sync(0xffffffffu, k);
+        if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = k;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned int s = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) s += wsum[w];
+            tile_count[tile] = s;
+        }
+        __syncthreads();
+    }
+}
+
+// one block per column: exclusive scan of the column's tile counts (in place) and the column total
+__global__ void __launch_bounds__(kBlock)
+csr_tile_scan_kernel(const CsrCols cc, unsigned int *__restrict__ tile_count, long long *__restrict__ col_nnz)
+{
+    __shared__ unsigned int wsum[kWarps];
+    __shared__ unsigned int carry_s;
+    const int c = blockIdx.x;
+    const int t0 = __ldg(cc.tile0 + c), t1 = __ldg(cc.tile0 + c + 1);
+    if (threadIdx.x == 0) carry_s = 0u;
+    __syncthreads();
+    for (int base = t0; base < t1; base += kBlock) {
+        const int t = base + threadIdx.x;
+        const unsigned int x = (t < t1) ? tile_count[t] : 0u;
+        unsigned int inc = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(0xffffffffu, inc, o); if ((threadIdx.x & 31) >= o) inc += y; }
+        if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = inc;
+        __syncthreads();
+        unsigned int woff = 0;
+        for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += wsum[w];
+        const unsigned int carry = carry_s;
+        if (t < t1) tile_count[t] = carry + woff + inc - x;
+        __syncthreads();
+        if (threadIdx.x == kBlock - 1) carry_s = carry + woff + inc;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) col_nnz[c] = (cc.skip && __ldg(cc.skip + c)) ? 0ll : (long long)carry_s;
+}
+
+__global__ void __launch_bounds__(kBlock)
+csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned int *__restrict__ colmax_bits, float rel_thr,
+                const unsigned int *__restrict__ tile_off, const long long *__restrict__ col_base,
+                int *__restrict__ out_idx, float *__restrict__ out_val)
+{
+    __shared__ unsigned int wsum[kWarps];
+    for (int tile = blockIdx.x; tile < cc.n_tiles; tile += gridDim.x) {
+        const int c = tile_column(cc, tile);
+        if (cc.skip && __ldg(cc.skip + c)) continue;          // block-uniform
+        const int4 lo = __ldg(cc.lo + c), dm = __ldg(cc.dim + c);
+        long long e; int bx = 0, by = 0, bz = 0;
+        const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
+        const float *p = data + __ldg(cc.offset + c) + e;
+        const float thr = rel_thr * __uint_as_float(__ldg(colmax_bits + c));
+        float x[kPerThread];
+        unsigned int k = 0;
+#pragma unroll
+        for (int i = 0; i < kPerThread; ++i) { x[i] = (i < cnt) ? p[i] : 0.0f; k += csr_keep(x[i], thr) ? 1u : 0u; }
+        unsigned int inc = k;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(0xffffffffu, inc, o); if ((threadIdx.x & 31) >= o) inc += y; }
+        if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = inc;
+        __syncthreads();
+        unsigned int woff = 0;
+        for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += wsum[w];
+        long long pos = __ldg(col_base + c) + (long long)__ldg(tile_off + tile) + woff + inc - k;
+#pragma unroll
+        for (int i = 0; i < kPerThread; ++i) {
+            if (csr_keep(x[i], thr)) {
+                out_idx[pos] = (int)((lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz)));
+                out_val[pos] = x[i];
+                ++pos;
+            }
+            box_next(dm, bx, by, bz);
+        }
+        __syncthreads();
+    }
+}
+
+// final assembly: row r of the staging area -> its place in the scenario's CSR arrays
+__global__ void csr_gather_rows_kernel(int n_rows, const long long *__restrict__ src_off, const long long *__restrict__ row_ptr,
+                                       const int *__restrict__ s_idx, const float *__restrict__ s_val,
+                                       int *__restrict__ idx, float *__restrict__ val)
+{
+    for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+        const long long a = __ldg(row_ptr + r), n = __ldg(row_ptr + r + 1) - a, s = __ldg(src_off + r);
+        for (long long i = threadIdx.x; i < n; i += blockDim.x) { idx[a + i] = s_idx[s + i]; val[a + i] = s_val[s + i]; }
+    }
 }
 
 }  // namespace vpk

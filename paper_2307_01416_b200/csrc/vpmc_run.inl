@@ -59,31 +59,23 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
         if (h->n_spots == 0) FAIL(h, VPMC_ERR_STATE, "no spots");
         if (h->d_spots) cudaFree(h->d_spots);
         if (h->d_spot_R0) cudaFree(h->d_spot_R0);
-        h->d_spot_R0 = nullptr;
         if (h->d_spot_beam) cudaFree(h->d_spot_beam);
         if (h->d_beams) cudaFree(h->d_beams);
-        h->d_spots = nullptr; h->d_spot_beam = nullptr; h->d_beams = nullptr;
+        h->d_spots = nullptr; h->d_spot_R0 = nullptr; h->d_spot_beam = nullptr; h->d_beams = nullptr;
         CU(h, cudaMalloc(&h->d_spots, sp.size() * sizeof(float4)));
+        CU(h, cudaMalloc(&h->d_spot_R0, r0.size() * sizeof(double)));
         CU(h, cudaMalloc(&h->d_spot_beam, sp.size() * sizeof(int)));
         CU(h, cudaMalloc(&h->d_beams, h->beams.size() * sizeof(DevBeam)));
         CU(h, cudaMemcpy(h->d_spots, sp.data(), sp.size() * sizeof(float4), cudaMemcpyHostToDevice));
-        CU(h, cudaMalloc(&h->d_spot_R0, r0.size() * sizeof(double)));
         CU(h, cudaMemcpy(h->d_spot_R0, r0.data(), r0.size() * sizeof(double), cudaMemcpyHostToDevice));
         CU(h, cudaMemcpy(h->d_spot_beam, h->spot_beam_h.data(), sp.size() * sizeof(int), cudaMemcpyHostToDevice));
-        if (h->map_capacity < h->n_spots + 1) {
-            if (h->d_cum) cudaFree(h->d_cum);
-            if (h->d_first) cudaFree(h->d_first);
-            h->d_cum = nullptr; h->d_first = nullptr;
-            CU(h, cudaMalloc(&h->d_cum, ((size_t)h->n_spots + 1) * sizeof(unsigned long long)));
-            CU(h, cudaMalloc(&h->d_first, ((size_t)h->n_spots + 1) * sizeof(unsigned long long)));
-            h->map_capacity = h->n_spots + 1;
-        }
         h->spots_dirty = false;
     }
     std::vector<DevBeam> db(h->beams.size());
     for (size_t i = 0; i < h->beams.size(); ++i) {
         const BeamHost &b = h->beams[i];
         DevBeam &d = db[i];
+        memset(&d, 0, sizeof(d));
         memcpy(d.iso, b.frame.iso, sizeof(d.iso));
         memcpy(d.rot, b.frame.rot, sizeof(d.rot));
         d.has_rs = b.rs_wet > 0.0f;
@@ -93,7 +85,9 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
         d.w_ap_out = -b.ap_face;
         d.w_ap_in = d.w_ap_out - b.ap_T;
         d.ap_bits = b.d_bits; d.ap_nx = b.ap_nx; d.ap_ny = b.ap_ny; d.ap_row_words = b.ap_row_words;
-        d.ap_u0 = b.ap_u0; d.ap_v0 = b.ap_v0; d.ap_du = b.ap_du; d.ap_dv = b.ap_dv;
+        d.ap_u0 = b.ap_u0; d.ap_v0 = b.ap_v0; d.ap_inv_du = (float)(1.0 / (double)b.ap_du); d.ap_inv_dv = (float)(1.0 / (double)b.ap_dv);
+        d.ap_dist = b.d_dist; d.ap_ntx = b.ap_ntx;
+        d.ap_tile_u = (float)(1 << kApTileShift) * b.ap_du; d.ap_tile_v = (float)(1 << kApTileShift) * b.ap_dv;
         const double wct = ct_min_w(h, b, sc.shift);
         if (d.has_rs && d.has_ap && d.w_rs_out > d.w_ap_in) FAIL(h, VPMC_ERR_GEOMETRY, "beam %zu: range shifter is not upstream of the aperture", i);
         const double w_last = d.has_ap ? d.w_ap_out : (d.has_rs ? d.w_rs_out : -std::numeric_limits<double>::infinity());
@@ -106,32 +100,57 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
     return VPMC_OK;
 }
 
-// one chunk: beam line for `n` items starting at item0, then the persistent voxel kernel on the survivors
-template <int MODE>
-static int launch_chunk(vpmc_t *h, const WorkMap &wm0, unsigned long long item0, unsigned int n, const vpmc_scenario &sc,
-                        uint64_t seed, float *edep, const ColumnBoxes &cb, int col0, cudaStream_t st)
+static Ctx make_ctx(const vpmc_t *h, const vpmc_scenario &sc, uint64_t seed)
 {
-    WorkMap wm = wm0;
-    wm.item0 = item0; wm.n_items = n;
-    CU(h, cudaMemsetAsync(h->d_qctr, 0, 2 * sizeof(unsigned int), st));
-    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-    const float3 shift = make_float3(sc.shift[0], sc.shift[1], sc.shift[2]);
-    {
-        TimedScope ts(h, st, 0);
-        beamline_kernel<<<(n + 255) / 256, 256, 0, st>>>(h->P, h->G, wm, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, shift, k0, k1, h->q, h->d_tal);
+    Ctx c;
+    c.P = h->P; c.G = h->G; c.beams = h->d_beams; c.hu = h->d_hu;
+    c.rsp_scale = sc.rsp_scale; c.inv_rsp_scale = (float)(1.0 / (double)sc.rsp_scale);
+    c.shift[0] = sc.shift[0]; c.shift[1] = sc.shift[1]; c.shift[2] = sc.shift[2];
+    c.k0 = (uint32_t)seed; c.k1 = (uint32_t)(seed >> 32);
+    return c;
+}
+
+// the hot path over wm.n_items work items, in chunks of kChunk: source (S1) -> beam line (S2-S3) -> CT entry -> voxel
+// stepping + scoring (S4-S7)
+template <int MODE>
+static int launch_transport(vpmc_t *h, const Ctx &c, const WorkMap &wm0, const ScoreArgs &sa, DevTallies *tal, cudaStream_t st)
+{
+    if (wm0.n_items == 0) return VPMC_OK;
+    const unsigned long long cap = std::min<unsigned long long>(wm0.n_items, kChunk);
+    int rc;
+    if ((rc = ensure(h, h->s0, cap * sizeof(uint4))) || (rc = ensure(h, h->s1, cap * sizeof(uint4))) || (rc = ensure(h, h->s2, cap * sizeof(uint4))) ||
+        (rc = ensure(h, h->q0, cap * sizeof(uint4))) || (rc = ensure(h, h->q1, cap * sizeof(float4))) || (rc = ensure(h, h->q2, cap * sizeof(float4))) ||
+        (rc = ensure(h, h->q3, cap * sizeof(uint4))) || (rc = ensure(h, h->q4, cap * sizeof(uint4)))) return rc;
+    SourceBuf sb;
+    sb.s0 = h->s0.as<uint4>(); sb.s1 = h->s1.as<uint4>(); sb.s2 = h->s2.as<uint4>();
+    Queue q;
+    q.q0 = h->q0.as<uint4>(); q.q1 = h->q1.as<float4>(); q.q2 = h->q2.as<float4>(); q.q3 = h->q3.as<uint4>(); q.q4 = h->q4.as<uint4>();
+    q.count = h->d_qctr; q.head = h->d_qctr + 1; q.capacity = (unsigned int)cap;
+    for (unsigned long long i0 = 0; i0 < wm0.n_items; i0 += kChunk) {
+        WorkMap wm = wm0;
+        wm.n_items = std::min<unsigned long long>(kChunk, wm0.n_items - i0);
+        const unsigned int n = (unsigned int)wm.n_items;
+        const int blocks = (int)((n + kBlock - 1) / kBlock);
+        CU(h, cudaMemsetAsync(h->d_qctr, 0, 4 * sizeof(unsigned int), st));
+        {
+            TimedScope ts(h, st, 0);
+            source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, i0, h->d_spots, h->d_spot_R0, h->d_spot_beam, sb, tal);
+            beam_kernel<<<std::min(h->grid_beam, blocks), kBlock, 0, st>>>(c, n, sb, q, h->d_qctr + 2, tal);
+        }
+        CU(h, cudaGetLastError());
+        TimedScope ts(h, st, 1);
+        entry_kernel<<<blocks, kBlock, 0, st>>>(c, q, tal);
+        if (h->smem_lut)
+            voxel_kernel<MODE, true><<<std::min(h->grid[MODE][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, q, h->d_lut, sa, tal);
+        else
+            voxel_kernel<MODE, false><<<std::min(h->grid[MODE][0], blocks), kBlock, h->tally_smem, st>>>(c, q, h->d_lut, sa, tal);
+        CU(h, cudaGetLastError());
+        h->launches += 4;
     }
-    CU(h, cudaGetLastError());
-    TimedScope ts(h, st, 1);
-    if (h->smem_lut)
-        voxel_kernel<MODE, true><<<h->voxel_grid[MODE][1], 256, h->lut_bytes, st>>>(h->P, h->G, h->q, h->d_hu, h->d_lut, sc.rsp_scale, edep, cb, col0, wm.hps, k0, k1, h->d_tal);
-    else
-        voxel_kernel<MODE, false><<<h->voxel_grid[MODE][0], 256, 0, st>>>(h->P, h->G, h->q, h->d_hu, h->d_lut, sc.rsp_scale, edep, cb, col0, wm.hps, k0, k1, h->d_tal);
-    CU(h, cudaGetLastError());
-    h->launches += 2;
     return VPMC_OK;
 }
 
-static int grid_for(long long n, int n_sm) { return (int)std::min<long long>((n + 255) / 256, (long long)n_sm * 16); }
+static int grid_for(long long n, int n_sm) { return (int)std::max<long long>(1, std::min<long long>((n + 255) / 256, (long long)n_sm * 16)); }
 
 extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t n_histories, uint64_t seed,
                                   float *dose_out_dev, void *cuda_stream)
@@ -150,62 +169,55 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
         CU(h, cudaMalloc(&h->d_s1, h->nvox * sizeof(float)));
         CU(h, cudaMalloc(&h->d_s2, h->nvox * sizeof(float)));
     }
-    // C2: history ids are contiguous per spot in spot order
+    rc = ensure(h, h->edep, (size_t)B * h->nvox * sizeof(float)); if (rc) return rc;
+    const size_t n_ent = (size_t)B * h->n_spots;
+    rc = ensure(h, h->cum, (n_ent + 1) * sizeof(unsigned long long)); if (rc) return rc;
+    rc = ensure(h, h->first, (n_ent + 1) * sizeof(unsigned long long)); if (rc) return rc;
+    // C2: history ids are contiguous per spot in spot order; batch b takes sub-range b of every spot (R7)
     std::vector<unsigned long long> cnt, start(h->n_spots + 1, 0ull);
     apportion(n_histories, h->spot_w, cnt);
     for (int g = 0; g < h->n_spots; ++g) start[g + 1] = start[g] + cnt[g];
     const unsigned long long wlo = h->win_lo, whi = h->win_hi ? std::min<unsigned long long>(h->win_hi, n_histories) : n_histories;
-
-    CU(h, cudaMemsetAsync(h->d_edep, 0, h->nvox * sizeof(float), st));
-    CU(h, cudaMemsetAsync(h->d_sum, 0, h->nvox * sizeof(float), st));
-    if (with_unc) {
-        CU(h, cudaMemsetAsync(h->d_s1, 0, h->nvox * sizeof(float), st));
-        CU(h, cudaMemsetAsync(h->d_s2, 0, h->nvox * sizeof(float), st));
-    }
-    CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
-    CU(h, cudaMemsetAsync(h->d_max_bits, 0, sizeof(unsigned int), st));
-    CU(h, cudaMemsetAsync(h->d_unc, 0, 2 * sizeof(double), st));
-
-    // total items in the window (for the batch scale factor)
-    std::vector<std::vector<unsigned long long>> cum(B), first(B);
-    unsigned long long n_total = 0;
-    for (int b = 0; b < B; ++b) {
-        cum[b].assign(h->n_spots + 1, 0ull); first[b].assign(h->n_spots + 1, 0ull);
+    std::vector<unsigned long long> cum(n_ent + 1, 0ull), first(n_ent + 1, 0ull);
+    std::vector<float> fb(B, 0.0f);
+    std::vector<unsigned long long> nb(B, 0ull);
+    for (int b = 0; b < B; ++b)
         for (int g = 0; g < h->n_spots; ++g) {
             const unsigned __int128 n = cnt[g];
             unsigned long long lo = start[g] + (unsigned long long)((n * (unsigned)b) / (unsigned)B);
             unsigned long long hi = start[g] + (unsigned long long)((n * (unsigned)(b + 1)) / (unsigned)B);
             lo = std::max(lo, wlo); hi = std::min(hi, whi);
-            first[b][g] = lo;
-            cum[b][g + 1] = cum[b][g] + (hi > lo ? hi - lo : 0ull);
+            const size_t e = (size_t)b * h->n_spots + g;
+            first[e] = lo;
+            const unsigned long long k = hi > lo ? hi - lo : 0ull;
+            cum[e + 1] = cum[e] + k;
+            nb[b] += k;
         }
-        n_total += cum[b][h->n_spots];
-    }
-    ColumnBoxes cb{};
-    for (int b = 0; b < B; ++b) {
-        const unsigned long long nb = cum[b][h->n_spots];
-        if (nb == 0) continue;
-        CU(h, cudaMemcpyAsync(h->d_cum, cum[b].data(), ((size_t)h->n_spots + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
-        CU(h, cudaMemcpyAsync(h->d_first, first[b].data(), ((size_t)h->n_spots + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
-        WorkMap wm{};
-        wm.mode = 0; wm.cum = h->d_cum; wm.first = h->d_first; wm.n_spots = h->n_spots;
-        for (unsigned long long i0 = 0; i0 < nb; i0 += kChunk) {
-            const unsigned int n = (unsigned int)std::min<unsigned long long>(kChunk, nb - i0);
-            rc = launch_chunk<0>(h, wm, i0, n, sc, seed, h->d_edep, cb, 0, st); if (rc) return rc;
-        }
-        const float f = (float)((double)n_total / (double)nb);
-        TimedScope ts(h, st, 2);
-        batch_accumulate_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->d_edep, h->d_sum, h->d_s1, h->d_s2, h->nvox, f, with_unc ? 1 : 0);
-        CU(h, cudaGetLastError());
-        h->launches += 1;
-    }
+    const unsigned long long n_total = cum[n_ent];
+    for (int b = 0; b < B; ++b) fb[b] = nb[b] ? (float)((double)n_total / (double)nb[b]) : 0.0f;
+
+    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)B * h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
+    CU(h, cudaMemsetAsync(h->d_max_bits, 0, sizeof(unsigned int), st));
+    CU(h, cudaMemsetAsync(h->d_unc, 0, 2 * sizeof(double), st));
+    CU(h, cudaMemcpyAsync(h->cum.p, cum.data(), (n_ent + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(h->first.p, first.data(), (n_ent + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(h->d_fb, fb.data(), B * sizeof(float), cudaMemcpyHostToDevice, st));
+
+    WorkMap wm{};
+    wm.mode = 0; wm.n_items = n_total; wm.cum = h->cum.as<unsigned long long>(); wm.first = h->first.as<unsigned long long>();
+    wm.n_entries = (int)n_ent; wm.n_spots = h->n_spots;
+    ScoreArgs sa{};
+    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->nvox;
+    rc = launch_transport<0>(h, make_ctx(h, sc, seed), wm, sa, h->d_tal, st); if (rc) return rc;
     // C6
     double W = 0.0;
     for (double x : h->spot_w) W += x;
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef = (float)((n_histories ? W / (double)n_histories : 0.0) / V * 1.602176634e-10);
     TimedScope ts(h, st, 2);
-    dose_convert_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->d_sum, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef, dose_out_dev, h->nvox, h->d_max_bits);
+    dose_finalize_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->edep.as<float>(), B, h->d_fb, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef,
+                                                                   dose_out_dev, with_unc ? h->d_s1 : nullptr, with_unc ? h->d_s2 : nullptr, h->nvox, h->d_max_bits);
     CU(h, cudaGetLastError());
     h->launches += 1;
     if (with_unc) {
@@ -296,9 +308,7 @@ extern "C" int vpmc_trace(vpmc_t *h, const vpmc_scenario *scp, int32_t mode, uin
     CT_(cudaMemcpy(d_h, hids, n * sizeof(unsigned long long), cudaMemcpyHostToDevice));
     CT_(cudaMemcpy(d_s, spot_of.data(), n * sizeof(int), cudaMemcpyHostToDevice));
     CT_(cudaMemset(d_r, 0, (size_t)n * max_steps * sizeof(StepRec)));
-    trace_kernel<true><<<(n + 63) / 64, 64>>>(h->P, h->G, d_h, d_s, n, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams,
-                                             make_float3(sc.shift[0], sc.shift[1], sc.shift[2]), h->d_hu, h->d_lut, sc.rsp_scale,
-                                             (uint32_t)seed, (uint32_t)(seed >> 32), d_r, max_steps, d_n);
+    trace_kernel<<<(n + 63) / 64, 64>>>(make_ctx(h, sc, seed), d_h, d_s, n, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_lut, d_r, max_steps, d_n);
     CT_(cudaGetLastError());
     h->launches += 1;
     CT_(cudaDeviceSynchronize());

@@ -1,6 +1,11 @@
-// vpmc_transport.cuh -- source sampler (S1), range-shifter / aperture module (S2, S3), CT entry and one
-// CT voxel step (S4, S5) as device functions.  The production kernels and the trace kernel call exactly
-// these functions, so a trace is a faithful record of what the production path does.
+// vpmc_transport.cuh -- the two step functions of the hot path: beam_step() = one iteration of a history in the beam
+// line (S1 source, S2 range shifter, S3 aperture module) and ct_step() = one voxel step (S4, S5, scoring hook S6/S7),
+// plus the CT entry.  The production kernels and the trace kernel call exactly these functions, so a trace is a
+// faithful record of what the production path does.
+//
+// Control structure ("identical control logic"): a warp only ever holds histories of ONE stage -- beam line or
+// CT -- so its lanes run the same code.  Inside the beam line the range shifter and the brass are the same slab step
+// with different constants; only the drift through the aperture opening differs, and it is cheap.
 #pragma once
 #include "vpmc_device.cuh"
 
@@ -11,12 +16,20 @@ struct DevTallies {
     unsigned long long n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;
     unsigned long long n_steps_ct, n_steps_dev;
 };
+enum : int { TD_INCIDENT = 0, TD_DEP_CT, TD_DEP_RS, TD_DEP_BRASS, TD_ESCAPED, TD_REMOVED, TD_N };
+enum : int { TC_STOP_CT = 0, TC_STOP_RS, TC_STOP_BRASS, TC_NUCLEAR, TC_ESCAPED, TC_STEPS_CT, TC_STEPS_DEV, TC_N };
 
-// per-thread partial tallies
-struct Tally {
-    double incident = 0, dep_ct = 0, dep_rs = 0, dep_brass = 0, escaped = 0, removed = 0;
-    unsigned int n_stopped_ct = 0, n_stopped_rs = 0, n_stopped_brass = 0, n_nuclear = 0, n_escaped = 0;
-    unsigned int n_steps_ct = 0, n_steps_dev = 0;
+// per-warp partial tallies in shared memory (fp64 sums; flushed to DevTallies once per warp at kernel end)
+struct WarpTally { double d[TD_N]; unsigned int c[TC_N]; unsigned int pad; };
+
+struct SmemSink {
+    WarpTally *w;
+    __device__ __forceinline__ void add_d(int k, float v) const { if (v != 0.0f) atomicAdd(&w->d[k], (double)v); }
+    __device__ __forceinline__ void add_c(int k, unsigned n) const { if (n) atomicAdd(&w->c[k], n); }
+};
+struct NullSink {
+    __device__ __forceinline__ void add_d(int, float) const {}
+    __device__ __forceinline__ void add_c(int, unsigned) const {}
 };
 
 struct StepRec {   // == vpmc_step_rec
@@ -27,14 +40,15 @@ struct StepRec {   // == vpmc_step_rec
     float E_before, E_after, s;
 };
 
-// Tracers record a step with the position converted back to frame coordinates: r = off + (rx, ry, rz).
 struct NullTracer {
+    static constexpr bool on = false;
     __device__ __forceinline__ void put(const Hist &, float, float, float, uint32_t, int, const int *, float, float, float, int) {}
 };
 
 struct RecTracer {
+    static constexpr bool on = true;
     StepRec *recs; int max, n;
-    __device__ void put(const Hist &h, float ox, float oy, float oz, uint32_t step, int region, const int *iv,
+    __device__ void put(const Hist &h, float x, float y, float z, uint32_t step, int region, const int *iv,
                         float Eb, float Ea, float s, int cause)
     {
         if (n < max) {
@@ -42,47 +56,50 @@ struct RecTracer {
             q.hid = ((unsigned long long)h.hid_hi << 32) | h.hid_lo;
             q.step = (int)step; q.region = region; q.cause = cause;
             q.ivox[0] = iv ? iv[0] : -1; q.ivox[1] = iv ? iv[1] : -1; q.ivox[2] = iv ? iv[2] : -1;
-            q.r[0] = ox + h.rx; q.r[1] = oy + h.ry; q.r[2] = oz + h.rz; q.u[0] = h.ux; q.u[1] = h.uy; q.u[2] = h.uz;
+            q.r[0] = x; q.r[1] = y; q.r[2] = z;
+            q.u[0] = h.ux + h.lx; q.u[1] = h.uy + h.ly; q.u[2] = h.uz + h.lz;
             q.E_before = Eb; q.E_after = Ea; q.s = s;
         }
         ++n;
     }
 };
 
-__device__ __forceinline__ void book_end(Tally &t, int cause, int region, float E_left)
-{
-    if (cause == ESCAPED) { t.escaped += (double)E_left; t.n_escaped++; }
-    else if (cause == NUCLEAR) t.n_nuclear++;
-    else if (cause == STOPPED) {
-        if (region == REG_CT) t.n_stopped_ct++;
-        else if (region == REG_RS) t.n_stopped_rs++;
-        else t.n_stopped_brass++;
-    }
-}
+// everything a step needs besides the history itself (kernel arguments -> constant bank)
+struct Ctx {
+    DevParams P;
+    DevGrid G;
+    const DevBeam *beams;
+    const short *hu;
+    float rsp_scale, inv_rsp_scale;
+    float shift[3];
+    uint32_t k0, k1;
+};
 
 // S1 (C2): sample position, energy and nuclear threshold of history h (hid already set) from spot sp.
 // R0 = alpha E_spot^p in fp64 from the host; recomputed on the device only when the source has an energy spread.
-__device__ __forceinline__ void sample_source(const DevParams &P, const float4 sp /*x,y,E,sigma*/, double R0,
-                                              Hist &h, uint32_t k0, uint32_t k1)
+__device__ __forceinline__ void sample_source(const DevParams &P, const DevBeam &b, int beam, const float4 sp /*x,y,E,sigma*/,
+                                              double R0, Hist &h, uint32_t k0, uint32_t k1)
 {
     const float4 a = draw4(h, 0u, 1u, k0, k1);
     const float rho = sqrtf(-2.0f * logf(a.x));
     float sn, cs;
     sincospif(2.0f * a.y, &sn, &cs);
-    h.rx = fmaf(sp.w, rho * cs, sp.x);
-    h.ry = fmaf(sp.w, rho * sn, sp.y);
-    h.rz = 0.0f;
+    set_beam_x(h, fma((double)sp.w, (double)(rho * cs), (double)sp.x));
+    set_beam_y(h, fma((double)sp.w, (double)(rho * sn), (double)sp.y));
+    h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
     float E0 = sp.z;
     if (P.delta_E != 0.0f) {
         const float zE = sqrtf(-2.0f * logf(a.z)) * cospif(2.0f * a.w);
-        E0 = sp.z * fmaf(P.delta_E, zE, 1.0f);
-        R0 = (double)P.alpha * pow((double)E0, (double)P.p);
+        const float dl = P.delta_E * zE;
+        E0 = sp.z * (1.0f + dl);
+        R0 = fma(R0, (double)expm1f(P.p * log1pf(dl)), R0);      // alpha (E (1 + dl))^p = R0 (1 + dl)^p
     }
     h.E = E0; h.R = R0;
-    const float4 b = draw4(h, 0u, 2u, k0, k1);
-    h.tau_star = -logf(b.x);
-    h.tau = 0.0f; h.t_rad = 0.0f; h.A_rad = 0.0f; h.step = 0u;
-    h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f;
+    const float4 c = draw4(h, 0u, 2u, k0, k1);
+    h.tau_star = -logf(c.x);
+    h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
+    h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
+    h.region = (b.has_rs ? REG_TO_RS : (b.has_ap ? REG_TO_AP : REG_TO_CT)) | (beam << 8);
 }
 
 // vacuum drift over a gap of `gap` mm along w (one step, no RNG); w_to = plane reached (for the record)
@@ -90,172 +107,321 @@ template <class Tracer>
 __device__ __forceinline__ int drift_gap(Hist &h, float gap, float w_to, Tracer &tr)
 {
     if (!(h.uz > 0.0f)) return ESCAPED;
-    const float s = fmaxf(__fdiv_rn(gap, h.uz), 0.0f);
-    h.rx = fmaf(s, h.ux, h.rx); h.ry = fmaf(s, h.uy, h.ry); h.rz = 0.0f;
-    tr.put(h, 0.0f, 0.0f, w_to, h.step, REG_VAC, nullptr, h.E, h.E, s, CONT);
+    const double uz = (double)h.uz + (double)h.lz;
+    const double s = fmax((double)gap / uz, 0.0);
+    const double x = fma(s, (double)h.ux + (double)h.lx, beam_x(h)), y = fma(s, (double)h.uy + (double)h.ly, beam_y(h));
+    set_beam_x(h, x); set_beam_y(h, y);
+    h.rz = 0.0f;
+    if (Tracer::on) tr.put(h, (float)x, (float)y, w_to, h.step, REG_VAC, nullptr, h.E, h.E, (float)s, CONT);
     h.step += 1u;
     return CONT;
 }
 
-__device__ __forceinline__ bool aperture_open(const DevBeam &b, float x, float y)
+// the medium under the current (u, v): bit of the opening bitmap; outside the bitmap = brass.  The pixel index
+// is taken in fp32 from the high part of the position: an error of ~4e-6 mm only matters within that distance of the
+// opening's edge.  (ix, iy) are returned for the safe-distance lookup.
+__device__ __forceinline__ bool aperture_open(const DevBeam *b, float x, float y, int &ix, int &iy)
 {
-    const float fx = floorf(__fdiv_rn(x - b.ap_u0, b.ap_du)), fy = floorf(__fdiv_rn(y - b.ap_v0, b.ap_dv));
-    if (!(fx >= 0.0f && fx < (float)b.ap_nx && fy >= 0.0f && fy < (float)b.ap_ny)) return false;
-    const int ix = (int)fx, iy = (int)fy;
-    const uint32_t wv = __ldg(b.ap_bits + (size_t)iy * b.ap_row_words + (ix >> 5));
+    const float fx = floorf((x - __ldg(&b->ap_u0)) * __ldg(&b->ap_inv_du)), fy = floorf((y - __ldg(&b->ap_v0)) * __ldg(&b->ap_inv_dv));
+    const int nx = __ldg(&b->ap_nx), ny = __ldg(&b->ap_ny);
+    if (!(fx >= 0.0f && fx < (float)nx && fy >= 0.0f && fy < (float)ny)) { ix = iy = -1; return false; }
+    ix = (int)fx; iy = (int)fy;
+    const uint32_t wv = __ldg(b->ap_bits + (size_t)iy * __ldg(&b->ap_row_words) + (ix >> 5));
     return (wv >> (ix & 31)) & 1u;
 }
 
-// S2 + S3 (C3): start plane -> range shifter -> aperture, in the beam frame with rz = local depth in the device.
-// Returns CONT when the history left the last device alive (or there is none), else the terminating cause;
-// w_now = beam-frame w of the plane the history stands on.
+// Beam frame -> CT frame (setup shift moves the patient), ray-box entry, entry voxel (C3).  Done in fp64: it runs
+// once per history and fixes the entry point that every later face crossing inherits.  On return the geometry
+// slots hold ix, iy, iz, v and rx, ry, rz are LOCAL offsets inside that voxel.
 template <class Tracer>
-__device__ int beamline(const DevParams &P, const DevBeam &b, Hist &h, Tally &t, Tracer &tr, uint32_t k0, uint32_t k1,
-                        float &w_now)
+__device__ __forceinline__ int enter_ct(const Ctx &c, const DevBeam &b, float w_now, Hist &h, Tracer &tr)
 {
-    StepOut o;
-    w_now = b.w_start;
-    if (b.has_rs) {
-        if (drift_gap(h, b.w_rs_in - w_now, b.w_rs_in, tr) != CONT) goto escaped;
-        const Medium m = { P.rs_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
-        const float T = b.w_rs_out - b.w_rs_in;
-        w_now = b.w_rs_in;
-        for (;;) {
-            if (!(h.uz > 0.0f)) goto escaped;
-            float d = P.s_rs; const float dist = __fdiv_rn(T - h.rz, h.uz); int ex = 0;
-            if (dist <= d) { d = dist; ex = 1; }
-            d = fmaxf(d, 0.0f);
-            const float Eb = h.E; const uint32_t st = h.step;
-            const int cause = material_step(P, h, m, d, k0, k1, o);
-            t.dep_rs += (double)o.dep; t.removed += (double)o.removed;
-            const bool out = (cause == CONT) && o.on_d && ex;
-            if (out) h.rz = T;
-            tr.put(h, 0.0f, 0.0f, b.w_rs_in, st, REG_RS, nullptr, Eb, h.E, o.s, cause);
-            if (cause != CONT) { book_end(t, cause, REG_RS, 0.0f); return cause; }
-            if (out) break;
-        }
-        w_now = b.w_rs_out;
-    }
-    if (b.has_ap) {
-        if (drift_gap(h, b.w_ap_in - w_now, b.w_ap_in, tr) != CONT) goto escaped;
-        const Medium m = { P.brass_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
-        const float T = b.w_ap_out - b.w_ap_in;
-        w_now = b.w_ap_in;
-        for (;;) {
-            if (!(h.uz > 0.0f)) goto escaped;
-            float d = P.s_ap; const float dist = __fdiv_rn(T - h.rz, h.uz); int ex = 0;
-            if (dist <= d) { d = dist; ex = 1; }
-            d = fmaxf(d, 0.0f);
-            if (aperture_open(b, h.rx, h.ry)) {     // transported with the previous velocity and direction
-                h.rx = fmaf(d, h.ux, h.rx); h.ry = fmaf(d, h.uy, h.ry); h.rz = ex ? T : fmaf(d, h.uz, h.rz);
-                tr.put(h, 0.0f, 0.0f, b.w_ap_in, h.step, REG_AP_OPEN, nullptr, h.E, h.E, d, CONT);
-                h.step += 1u;
-                if (ex) break;
-                continue;
-            }
-            const float Eb = h.E; const uint32_t st = h.step;
-            const int cause = material_step(P, h, m, d, k0, k1, o);
-            t.dep_brass += (double)o.dep; t.removed += (double)o.removed;
-            const bool out = (cause == CONT) && o.on_d && ex;
-            if (out) h.rz = T;
-            tr.put(h, 0.0f, 0.0f, b.w_ap_in, st, REG_AP_BRASS, nullptr, Eb, h.E, o.s, cause);
-            if (cause != CONT) { book_end(t, cause, REG_AP_BRASS, 0.0f); return cause; }
-            if (out) break;
-        }
-        w_now = b.w_ap_out;
-    }
-    h.rz = 0.0f;
-    return CONT;
-escaped:
-    tr.put(h, 0.0f, 0.0f, w_now, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
-    book_end(t, ESCAPED, REG_VAC, h.E);
-    return ESCAPED;
-}
-
-// Beam frame -> CT frame (setup shift moves the patient), ray-box entry, entry voxel (C3).  On return the
-// position variables are LOCAL offsets inside voxel iv.
-template <class Tracer>
-__device__ int enter_ct(const DevGrid &G, const DevBeam &b, const float shift[3], float w_now, Hist &h, int iv[3],
-                        Tally &t, Tracer &tr)
-{
-    float r[3], u[3];
+    const DevGrid &G = c.G;
+    double r[3], u[3];
     {
-        const float x = h.rx, y = h.ry, z = w_now, a = h.ux, c = h.uy, e = h.uz;
-        r[0] = (b.iso[0] - shift[0]) + (b.rot[0] * x + b.rot[1] * y + b.rot[2] * z);
-        r[1] = (b.iso[1] - shift[1]) + (b.rot[3] * x + b.rot[4] * y + b.rot[5] * z);
-        r[2] = (b.iso[2] - shift[2]) + (b.rot[6] * x + b.rot[7] * y + b.rot[8] * z);
-        u[0] = b.rot[0] * a + b.rot[1] * c + b.rot[2] * e;
-        u[1] = b.rot[3] * a + b.rot[4] * c + b.rot[5] * e;
-        u[2] = b.rot[6] * a + b.rot[7] * c + b.rot[8] * e;
-        h.ux = u[0]; h.uy = u[1]; h.uz = u[2];
+        const double x = beam_x(h), y = beam_y(h), z = (double)w_now;
+        const double a = (double)h.ux + (double)h.lx, q = (double)h.uy + (double)h.ly, e = (double)h.uz + (double)h.lz;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            r[k] = ((double)b.iso[k] - (double)c.shift[k]) + (double)b.rot[3 * k] * x + (double)b.rot[3 * k + 1] * y + (double)b.rot[3 * k + 2] * z;
+            u[k] = (double)b.rot[3 * k] * a + (double)b.rot[3 * k + 1] * q + (double)b.rot[3 * k + 2] * e;
+        }
     }
-    const float lo[3] = { G.ox, G.oy, G.oz };
-    const float hh[3] = { G.hx, G.hy, G.hz };
+    h.ux = (float)u[0]; h.uy = (float)u[1]; h.uz = (float)u[2];
+    h.lx = (float)(u[0] - (double)h.ux); h.ly = (float)(u[1] - (double)h.uy); h.lz = (float)(u[2] - (double)h.uz);
+    const double lo[3] = { (double)G.ox, (double)G.oy, (double)G.oz };
+    const double hh[3] = { (double)G.hx, (double)G.hy, (double)G.hz };
     const int n[3] = { G.nx, G.ny, G.nz };
-    float t_in = 0.0f, t_out = __int_as_float(0x7f800000); int ax = -1; bool miss = false;
+    double t_in = 0.0, t_out = __longlong_as_double(0x7ff0000000000000LL); int ax = -1; bool miss = false;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const float hi = lo[a] + (float)n[a] * hh[a];
-        if (u[a] == 0.0f) { if (r[a] < lo[a] || r[a] >= hi) miss = true; continue; }
-        const float t1 = __fdiv_rn(lo[a] - r[a], u[a]), t2 = __fdiv_rn(hi - r[a], u[a]);
-        const float tn = fminf(t1, t2), tf = fmaxf(t1, t2);
+        const double hi = lo[a] + (double)n[a] * hh[a];
+        if (u[a] == 0.0) { if (r[a] < lo[a] || r[a] >= hi) miss = true; continue; }
+        const double t1 = (lo[a] - r[a]) / u[a], t2 = (hi - r[a]) / u[a];
+        const double tn = fmin(t1, t2), tf = fmax(t1, t2);
         if (tn > t_in) { t_in = tn; ax = a; }
-        t_out = fminf(t_out, tf);
+        t_out = fmin(t_out, tf);
     }
     if (miss || !(t_in < t_out)) {
-        h.rx = r[0]; h.ry = r[1]; h.rz = r[2];
-        tr.put(h, 0.0f, 0.0f, 0.0f, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
-        book_end(t, ESCAPED, REG_VAC, h.E);
+        if (Tracer::on) tr.put(h, (float)r[0], (float)r[1], (float)r[2], h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
         return ESCAPED;
     }
-    float l[3];
+    int iv[3]; float l[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const float q = fmaf(t_in, u[a], r[a]);
+        const double q = fma(t_in, u[a], r[a]);
         if (a == ax) {
-            if (u[a] > 0.0f) { iv[a] = 0; l[a] = 0.0f; } else { iv[a] = n[a] - 1; l[a] = hh[a]; }
+            if (u[a] > 0.0) { iv[a] = 0; l[a] = 0.0f; } else { iv[a] = n[a] - 1; l[a] = (float)hh[a]; }
         } else {
-            float f = floorf(__fdiv_rn(q - lo[a], hh[a]));
-            f = fminf(fmaxf(f, 0.0f), (float)(n[a] - 1));
+            double f = floor((q - lo[a]) / hh[a]);
+            f = fmin(fmax(f, 0.0), (double)(n[a] - 1));
             iv[a] = (int)f;
-            l[a] = fminf(fmaxf(q - fmaf(f, hh[a], lo[a]), 0.0f), hh[a]);
+            l[a] = (float)fmin(fmax(q - fma(f, hh[a], lo[a]), 0.0), hh[a]);
         }
     }
     h.rx = l[0]; h.ry = l[1]; h.rz = l[2];
-    tr.put(h, fmaf((float)iv[0], G.hx, G.ox), fmaf((float)iv[1], G.hy, G.oy), fmaf((float)iv[2], G.hz, G.oz),
-           h.step, REG_VAC, nullptr, h.E, h.E, t_in, CONT);
+    h.g0 = (uint32_t)iv[0]; h.g1 = (uint32_t)iv[1]; h.g2 = (uint32_t)iv[2];
+    h.g3 = (uint32_t)(iv[0] + G.nx * (iv[1] + G.ny * iv[2]));
+    if (Tracer::on) tr.put(h, fmaf((float)iv[0], G.hx, G.ox) + l[0], fmaf((float)iv[1], G.hy, G.oy) + l[1], fmaf((float)iv[2], G.hz, G.oz) + l[2],
+                           h.step, REG_VAC, nullptr, h.E, h.E, (float)t_in, CONT);
     h.step += 1u;
     return CONT;
 }
 
-// S4: distance to the nearest face of the current voxel from the local offset, ties to the lowest axis
-__device__ __forceinline__ float face_distance(const DevGrid &G, const Hist &h, int &ax)
+// S4: distance to the nearest face of the current voxel from the local offset.  The nearest axis is found by
+// cross-multiplication (dist_a |u_b| < dist_b |u_a|), so only ONE reciprocal goes through the MUFU pipe; ties go to the
+// lowest axis.  `up` = the history moves towards +axis on that axis during the step.
+__device__ __forceinline__ float face_distance(const DevGrid &G, const Hist &h, int &ax, bool &up)
 {
-    const float inf = __int_as_float(0x7f800000);
-    float dx = inf, dy = inf, dz = inf;
-    if (h.ux > 0.0f) dx = __fdividef(G.hx - h.rx, h.ux); else if (h.ux < 0.0f) dx = __fdividef(-h.rx, h.ux);
-    if (h.uy > 0.0f) dy = __fdividef(G.hy - h.ry, h.uy); else if (h.uy < 0.0f) dy = __fdividef(-h.ry, h.uy);
-    if (h.uz > 0.0f) dz = __fdividef(G.hz - h.rz, h.uz); else if (h.uz < 0.0f) dz = __fdividef(-h.rz, h.uz);
-    float d = dx; ax = 0;
-    if (dy < d) { d = dy; ax = 1; }
-    if (dz < d) { d = dz; ax = 2; }
-    return fmaxf(d, 0.0f);
+    float nx = (h.ux > 0.0f) ? G.hx - h.rx : h.rx, ax_ = fabsf(h.ux);
+    float ny = (h.uy > 0.0f) ? G.hy - h.ry : h.ry, ay_ = fabsf(h.uy);
+    float nz = (h.uz > 0.0f) ? G.hz - h.rz : h.rz, az_ = fabsf(h.uz);
+    if (ax_ == 0.0f) { nx = 1e30f; ax_ = 1.0f; }
+    if (ay_ == 0.0f) { ny = 1e30f; ay_ = 1.0f; }
+    if (az_ == 0.0f) { nz = 1e30f; az_ = 1.0f; }
+    float n = nx, a = ax_; ax = 0; up = h.ux > 0.0f;
+    if (ny * a < n * ay_) { n = ny; a = ay_; ax = 1; up = h.uy > 0.0f; }
+    if (nz * a < n * az_) { n = nz; a = az_; ax = 2; up = h.uz > 0.0f; }
+    return fmaxf(__fdividef(n, a), 0.0f);
 }
 
 // C4-9: the step ended on a voxel face: advance that index, snap that local coordinate.  `up` = direction sign
 // on that axis BEFORE the scattering of this step.  Returns true if the history left the grid.
-__device__ __forceinline__ bool cross_face(const DevGrid &G, Hist &h, int &ix, int &iy, int &iz, int ax, bool up)
+__device__ __forceinline__ bool cross_face(const DevGrid &G, Hist &h, int ax, bool up)
 {
     if (ax == 0) {
-        if (up) { ix += 1; h.rx = 0.0f; } else { ix -= 1; h.rx = G.hx; }
-        return ix < 0 || ix >= G.nx;
+        if (up) { h.g0 += 1u; h.g3 += 1u; h.rx = 0.0f; } else { h.g0 -= 1u; h.g3 -= 1u; h.rx = G.hx; }
+        return h.g0 >= (uint32_t)G.nx;
     } else if (ax == 1) {
-        if (up) { iy += 1; h.ry = 0.0f; } else { iy -= 1; h.ry = G.hy; }
-        return iy < 0 || iy >= G.ny;
+        if (up) { h.g1 += 1u; h.g3 += (uint32_t)G.nx; h.ry = 0.0f; } else { h.g1 -= 1u; h.g3 -= (uint32_t)G.nx; h.ry = G.hy; }
+        return h.g1 >= (uint32_t)G.ny;
     } else {
-        if (up) { iz += 1; h.rz = 0.0f; } else { iz -= 1; h.rz = G.hz; }
-        return iz < 0 || iz >= G.nz;
+        const uint32_t nxy = (uint32_t)(G.nx * G.ny);
+        if (up) { h.g2 += 1u; h.g3 += nxy; h.rz = 0.0f; } else { h.g2 -= 1u; h.g3 -= nxy; h.rz = G.hz; }
+        return h.g2 >= (uint32_t)G.nz;
     }
+}
+
+// per-thread counters that live for the whole kernel (flushed once at its end)
+struct LaneCounters { unsigned int n_ct = 0, n_dev = 0; double incident = 0.0; };
+
+struct NullScorer {
+    __device__ __forceinline__ void begin(const Hist &) {}
+    __device__ __forceinline__ void deposit(const Hist &, float) {}
+    __device__ __forceinline__ void end(const Hist &) {}
+};
+
+struct LutShared { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return p[i]; } };
+struct LutGlobal { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return __ldg(p + i); } };
+
+enum : int { BEAM_CONT = 0, BEAM_ENDED = 1, BEAM_EXIT = 2 };
+
+// One iteration of history h in the beam line: pending vacuum drifts, the drifts through the opening (safe-distance
+// skipping makes a clean transit two passes of the loop), then at most ONE slab step (range shifter or brass).  Returns BEAM_CONT, BEAM_ENDED (all tallies booked) or BEAM_EXIT
+// (the history stands on the exit plane of the last device, region = REG_TO_CT).
+// hdep = energy deposited so far in the current device.
+template <class Sink, class Tracer>
+__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &hdep, LaneCounters &lc, const Sink &sink, Tracer &tr)
+{
+    // Single-exit structured control flow on purpose: every lane passes through `if (do_step)`, so lanes that stand in
+    // different regions re-converge BEFORE the expensive slab step.  (With early returns the re-convergence point of the
+    // region branches moves to the end of the function and range-shifter and brass lanes execute the step in turns:
+    // measured 17 of 32 lanes active, profiles/r1c.)
+    const DevParams &P = c.P;
+    int reg = h.region & 0xff;
+    const int beam_bits = h.region & ~0xff;
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    Medium m = { 1.0f, 1.0f, 1.0f, 0.0f, 0.0f };
+    float d = 0.0f, T = 0.0f, w_in = 0.0f;
+    bool ex = false, do_step = false, esc = false;
+    int status = BEAM_CONT;
+
+    if (reg == REG_TO_CT) status = BEAM_EXIT;              // no device at all
+    if (reg == REG_TO_RS) {
+        const float w1 = __ldg(&bp->w_rs_in);
+        w_in = __ldg(&bp->w_start);
+        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else reg = REG_RS;
+    }
+    if (reg == REG_TO_AP) {
+        const float w1 = __ldg(&bp->w_ap_in);
+        w_in = __ldg(&bp->has_rs) ? __ldg(&bp->w_rs_out) : __ldg(&bp->w_start);
+        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else reg = REG_AP;
+    }
+    if (reg == REG_AP && !esc) {
+        w_in = __ldg(&bp->w_ap_in);
+        T = __ldg(&bp->w_ap_out) - w_in;
+        for (;;) {
+            if (!(h.uz > 0.0f)) { esc = true; break; }
+            d = P.s_ap; ex = false;
+            const float rem = T - h.rz, duz = d * h.uz;
+            if (rem <= duz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
+            int ix, iy;
+            if (!aperture_open(bp, beam_xh(h), beam_yh(h), ix, iy)) {
+                m = Medium{ P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
+                do_step = true;
+                break;
+            }
+            // in the opening the proton is transported with its previous velocity and direction.
+            // Safe-distance skipping: every tile within Chebyshev distance k - 1 of this one is fully open, so the next n
+            // per-step tests are known to answer "open" as long as the lateral travel stays below (k - 1) tiles; take those
+            // n full steps at once (the last full step and the exit step always go through the per-step code).
+            int n = 1;
+            if (!ex) {
+                const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
+                if (k >= 2) {
+                    const float safe = 0.99f * (float)(k - 1);
+                    const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(d * h.ux), 1e-12f));
+                    const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(d * h.uy), 1e-12f));
+                    const float nfull = __fdividef(rem, duz) - 2.0f;          // full steps certainly before the exit step
+                    const float nn = floorf(fminf(fminf(nu, nv), nfull));
+                    if (nn >= 2.0f) n = (int)fminf(nn, 65536.0f);
+                }
+            }
+            if (Tracer::on && n > 1) {     // the same arithmetic, one record per step
+                const uint32_t g0 = h.g0, g1 = h.g1, g2 = h.g2, g3 = h.g3; const float rz0 = h.rz;
+                for (int j = 1; j < n; ++j) {
+                    const float sj = (float)j * d;
+                    h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3;
+                    pair_axpy(h.g0, h.g1, sj, h.ux, h.lx); pair_axpy(h.g2, h.g3, sj, h.uy, h.ly);
+                    h.rz = fmaf(sj, h.uz, rz0);
+                    tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_AP_OPEN, nullptr, h.E, h.E, d, CONT);
+                    h.step += 1u;
+                }
+                h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3; h.rz = rz0; h.step -= (uint32_t)(n - 1);
+            }
+            const float sn = (float)n * d;
+            pair_axpy(h.g0, h.g1, sn, h.ux, h.lx); pair_axpy(h.g2, h.g3, sn, h.uy, h.ly);
+            h.rz = ex ? T : fmaf(sn, h.uz, h.rz);
+            h.step += (uint32_t)n;
+            if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step - 1u, REG_AP_OPEN, nullptr, h.E, h.E, d, CONT);
+            if (ex) {
+                sink.add_d(TD_DEP_BRASS, hdep); hdep = 0.0f;
+                reg = REG_TO_CT; status = BEAM_EXIT;
+                break;
+            }
+        }
+    }
+    if (reg == REG_RS && !esc) {
+        if (!(h.uz > 0.0f)) esc = true;
+        else {
+            w_in = __ldg(&bp->w_rs_in);
+            T = __ldg(&bp->w_rs_out) - w_in;
+            d = P.s_rs; ex = false;
+            const float rem = T - h.rz;
+            if (rem <= d * h.uz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
+            m = Medium{ P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
+            do_step = true;
+        }
+    }
+    if (do_step) {
+        StepOut o;
+        const float Eb = h.E; const uint32_t st = h.step;
+        const int cause = step_physics(P, h, m, d, c.k0, c.k1, o);
+        if (cause == CONT) {
+            // C4-8: move along the OLD direction, then rotate
+            pair_axpy(h.g0, h.g1, o.s, h.ux, h.lx);
+            pair_axpy(h.g2, h.g3, o.s, h.uy, h.ly);
+            h.rz = fmaf(o.s, h.uz, h.rz);
+            if (P.flags & 1) rotate(h, o.theta, o.uphi);
+        }
+        hdep += o.dep;
+        sink.add_d(TD_REMOVED, o.removed);
+        const bool out = (cause == CONT) && o.on_d && ex;
+        if (out) h.rz = T;
+        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause);
+        if (out || cause != CONT) { sink.add_d(reg == REG_RS ? TD_DEP_RS : TD_DEP_BRASS, hdep); hdep = 0.0f; }
+        if (cause != CONT) {
+            lc.n_dev += h.step;
+            sink.add_c(cause == NUCLEAR ? TC_NUCLEAR : (reg == REG_RS ? TC_STOP_RS : TC_STOP_BRASS), 1u);
+            status = BEAM_ENDED;
+        } else if (out) {
+            reg = (reg == REG_RS && __ldg(&bp->has_ap)) ? REG_TO_AP : REG_TO_CT;
+            if (reg == REG_TO_CT) status = BEAM_EXIT;
+        }
+    }
+    if (esc) {   // u_w <= 0 inside the beam line (C4, last paragraph)
+        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
+        if (hdep != 0.0f) { sink.add_d((reg == REG_RS || reg == REG_TO_AP) ? TD_DEP_RS : TD_DEP_BRASS, hdep); hdep = 0.0f; }
+        sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u);
+        lc.n_dev += h.step;
+        status = BEAM_ENDED;
+    }
+    h.region = reg | beam_bits;
+    return status;
+}
+
+// CT entry of a history that left the beam line (region REG_TO_CT): books the beam-line step count and, on a miss,
+// the escape.  Returns CONT or ESCAPED.
+template <class Sink, class Tracer>
+__device__ __forceinline__ int ct_entry(const Ctx &c, Hist &h, LaneCounters &lc, const Sink &sink, Tracer &tr)
+{
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    const float w_now = __ldg(&bp->has_ap) ? __ldg(&bp->w_ap_out) : (__ldg(&bp->has_rs) ? __ldg(&bp->w_rs_out) : __ldg(&bp->w_start));
+    const int ec = enter_ct(c, *bp, w_now, h, tr);
+    lc.n_dev += h.step;
+    h.region = REG_CT | (h.region & ~0xff);
+    if (ec != CONT) { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
+    return ec;
+}
+
+// One voxel step of history h (S4, S5, S6/S7).  Returns CONT or the cause that ended the history (tallies booked).
+// hdep = energy deposited in the CT so far by this history.
+template <class Lut, class Scorer, class Sink, class Tracer>
+__device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, float &hdep, LaneCounters &lc,
+                                       Scorer &sc, const Sink &sink, Tracer &tr)
+{
+    const DevParams &P = c.P;
+    const DevGrid &G = c.G;
+    int ax; bool up;
+    const float d = face_distance(G, h, ax, up);
+    int t = (int)__ldg(c.hu + h.g3) - G.hu_min;
+    t = min(max(t, 0), G.n_lut - 1);
+    const float4 mv = lut[t];                 // rsp, rho, xsp / X0_w, 1 / rsp
+    const Medium m = { mv.x * c.rsp_scale, mv.w * c.inv_rsp_scale, mv.y, mv.z, P.za_w * mv.y };
+    StepOut o;
+    const float Eb = h.E; const uint32_t st = h.step;
+    int cause = step_physics(P, h, m, d, c.k0, c.k1, o);
+    if (cause == CONT) {
+        // C4-8: move along the OLD direction, then rotate
+        h.rx = fmaf(o.s, h.lx, fmaf(o.s, h.ux, h.rx));
+        h.ry = fmaf(o.s, h.ly, fmaf(o.s, h.uy, h.ry));
+        h.rz = fmaf(o.s, h.lz, fmaf(o.s, h.uz, h.rz));
+        if (P.flags & 1) rotate(h, o.theta, o.uphi);
+    }
+    hdep += o.dep;
+    sink.add_d(TD_REMOVED, o.removed);
+    if (o.dep != 0.0f) sc.deposit(h, o.dep);      // S6 / S7: the voxel at the START of the step
+    const int iv0[3] = { (int)h.g0, (int)h.g1, (int)h.g2 };
+    if (cause == CONT && o.on_d && cross_face(G, h, ax, up)) cause = ESCAPED;
+    lc.n_ct += (cause != STOPPED);
+    if (Tracer::on) tr.put(h, fmaf((float)(int)h.g0, G.hx, G.ox) + h.rx, fmaf((float)(int)h.g1, G.hy, G.oy) + h.ry,
+                           fmaf((float)(int)h.g2, G.hz, G.oz) + h.rz, st, REG_CT, iv0, Eb, h.E, o.s, cause);
+    if (cause != CONT) {
+        sink.add_d(TD_DEP_CT, hdep); hdep = 0.0f;
+        if (cause == ESCAPED) { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
+        else sink.add_c(cause == NUCLEAR ? TC_NUCLEAR : TC_STOP_CT, 1u);
+    }
+    return cause;
 }
 
 }  // namespace vpk
