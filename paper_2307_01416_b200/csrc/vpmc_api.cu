@@ -280,8 +280,29 @@ extern "C" int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int ma
             int &v = dist[(size_t)ty * ntx + tx];
             v = std::min(v, std::min(std::min(at(ty + 1, tx + 1), at(ty + 1, tx)), std::min(at(ty + 1, tx - 1), at(ty, tx + 1))) + 1);
         }
-    std::vector<unsigned char> dist8(dist.size());
-    for (size_t i = 0; i < dist.size(); ++i) dist8[i] = (unsigned char)std::min(dist[i], 255);
+    // the same towards the opening: distance to the nearest tile that holds any open pixel (none outside the bitmap)
+    std::vector<int> dopen((size_t)ntx * nty, 0);
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            bool any = false;
+            for (int iy = ty * ts; !any && iy < std::min((ty + 1) * ts, ny); ++iy)
+                for (int ix = tx * ts; ix < std::min((tx + 1) * ts, nx); ++ix)
+                    if (opening[(size_t)iy * nx + ix]) { any = true; break; }
+            dopen[(size_t)ty * ntx + tx] = any ? 0 : 255;
+        }
+    auto ao = [&](int ty, int tx) { return (tx < 0 || ty < 0 || tx >= ntx || ty >= nty) ? 255 : dopen[(size_t)ty * ntx + tx]; };
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            int &v = dopen[(size_t)ty * ntx + tx];
+            v = std::min(v, std::min(std::min(ao(ty - 1, tx - 1), ao(ty - 1, tx)), std::min(ao(ty - 1, tx + 1), ao(ty, tx - 1))) + 1);
+        }
+    for (int ty = nty - 1; ty >= 0; --ty)
+        for (int tx = ntx - 1; tx >= 0; --tx) {
+            int &v = dopen[(size_t)ty * ntx + tx];
+            v = std::min(v, std::min(std::min(ao(ty + 1, tx + 1), ao(ty + 1, tx)), std::min(ao(ty + 1, tx - 1), ao(ty, tx + 1))) + 1);
+        }
+    std::vector<unsigned char> dist8(2 * dist.size());
+    for (size_t i = 0; i < dist.size(); ++i) { dist8[i] = (unsigned char)std::min(dist[i], 255); dist8[dist.size() + i] = (unsigned char)std::min(dopen[i], 255); }
     free_beam(b);
     CU(h, cudaMalloc(&b.d_bits, bits.size() * sizeof(uint32_t)));
     CU(h, cudaMemcpy(b.d_bits, bits.data(), bits.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));

@@ -56,11 +56,16 @@ struct DevBeam {
     // safe-distance map of the opening: per tile of kApTile x kApTile pixels, the Chebyshev distance in tiles to the
     // nearest tile that is not fully open (0 = not fully open itself, capped at 255)
     const unsigned char *ap_dist;
+    // the same towards the opening: Chebyshev distance in tiles to the nearest tile that holds ANY open pixel
+    const unsigned char *ap_dist_open;
     int ap_ntx;
     float ap_tile_u, ap_tile_v;   // tile size in mm
 };
 
-constexpr int kApTileShift = 3;   // 8 x 8 pixels per tile
+#ifndef VPK_AP_TILE_SHIFT
+#define VPK_AP_TILE_SHIFT 0
+#endif
+constexpr int kApTileShift = VPK_AP_TILE_SHIFT;   // 2^shift x 2^shift pixels per tile of the safe-distance maps
 
 struct Medium { float rsp, inv_rsp, rho_rel, inv_X0, za_rho; };
 
@@ -154,21 +159,17 @@ __device__ __forceinline__ float highland_f(float t, float c_log) { return t > 0
 
 // C4-7: A(t + dt) - A(t) without cancellation.  With f' - f = c_log ln(1 + dt/t):
 //   A(t') - A(t) = dt f'^2 + t (f' - f)(f' + f).
-// The log of a ratio near 1 is a short series, so later steps need no MUFU log at all; f is re-anchored on the MUFU log
-// whenever dt/t >= 0.1 (the first few steps).  f_new is returned through `f`.
+// f' comes from the MUFU log (absolute error ~6e-9); the DIFFERENCE f' - f is the short series of the log of a ratio
+// near 1 when dt/t < 0.1 and the plain difference otherwise (the first steps, where nothing cancels).  Branch-free.
+// f_new is returned through `f`.
 __device__ __forceinline__ float highland_dA(float t, float dt, float c_log, float &f)
 {
     const float tp = t + dt;
-    if (!(t > 0.0f)) { f = highland_f(tp, c_log); return tp * f * f; }
-    const float x = __fdividef(dt, t);
-    float fn, df;
-    if (x < 0.1f) {
-        const float L = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(x, -1.0f / 6.0f, 0.2f), -0.25f), 1.0f / 3.0f), -0.5f), 1.0f);
-        df = c_log * L; fn = f + df;
-    } else {
-        fn = highland_f(tp, c_log); df = fn - f;
-    }
-    const float dA = fmaf(dt, fn * fn, t * df * (fn + f));
+    const float fn = highland_f(tp, c_log);
+    const float x = __fdividef(dt, fmaxf(t, 1e-30f));
+    const float L = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(x, -1.0f / 6.0f, 0.2f), -0.25f), 1.0f / 3.0f), -0.5f), 1.0f);
+    const float df = (x < 0.1f) ? c_log * L : fn - f;
+    const float dA = (t > 0.0f) ? fmaf(dt, fn * fn, t * df * (fn + f)) : tp * fn * fn;
     f = fn;
     return dA;
 }

@@ -129,12 +129,12 @@ template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreAr
 constexpr int kBlock = 256;
 constexpr int kWarps = kBlock / 32;
 #ifndef VPK_REFILL_MIN
-#define VPK_REFILL_MIN 4
+#define VPK_REFILL_MIN 8
 #endif
 constexpr int kRefillMin = VPK_REFILL_MIN;   // S6b: free lanes are refilled once at least this many of a warp's lanes are free
 
 #ifndef VPK_MIN_BLOCKS
-#define VPK_MIN_BLOCKS 3
+#define VPK_MIN_BLOCKS 4
 #endif
 
 // source records of a chunk, SoA of 16-byte words
@@ -208,62 +208,69 @@ beam_kernel(const Ctx c, const unsigned int n_items, const SourceBuf sb, const Q
     NullTracer tr;
     LaneCounters lc;
     Hist h;
-    h.region = REG_TO_CT; h.col = 0; h.step = 0u;
-    float hdep = 0.0f;
+    h.region = REG_TO_CT; h.col = 0; h.step = 0u; h.E = 0.0f; h.R = 0.0;
+    float dep_rs = 0.0f, dep_ap = 0.0f;
+    int pend = BEAM_CONT;                  // status of a finished history whose bookkeeping is still due
     bool alive = false, exhausted = false;
     for (;;) {
+        // S6b, event pass: once enough lanes are free, book their finished histories, push the survivors to the queue and
+        // load the next source records -- all of it converged over those lanes
         const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
+        const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != BEAM_CONT);
         const int n_free = __popc(free_mask);
-        if (!exhausted && (n_free >= kRefillMin || n_free == 32)) {
-            unsigned base = 0;
-            const int leader = __ffs(free_mask) - 1;
-            if (lane == leader) base = atomicAdd(counter, (unsigned)n_free);
-            base = __shfl_sync(0xffffffffu, base, leader);
-            exhausted = base + (unsigned)n_free >= n_items;
-            if (!alive) {
-                const unsigned k = base + __popc(free_mask & lanemask_lt());
-                if (k < n_items) {
-                    const uint4 a = sb.s0[k], b = sb.s1[k], e = sb.s2[k];
-                    h.g0 = a.x; h.g1 = a.y; h.g2 = a.z; h.g3 = a.w;
-                    h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
-                    h.E = __uint_as_float(b.x); h.tau_star = __uint_as_float(b.y);
-                    h.col = (int)(b.z & 0xffffffu); h.region = (int)b.w | (int)((b.z >> 24) << 8);
-                    h.R = __longlong_as_double((long long)(((unsigned long long)e.y << 32) | e.x));
-                    h.hid_lo = e.z; h.hid_hi = e.w;
-                    h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
-                    h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
-                    hdep = 0.0f;
-                    alive = true;
+        if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
+            const unsigned out_mask = __ballot_sync(0xffffffffu, !alive && pend == BEAM_EXIT);
+            if (out_mask) {                // survivors -> queue (one atomic per warp)
+                unsigned base = 0;
+                const int leader = __ffs(out_mask) - 1;
+                if (lane == leader) base = atomicAdd(q.count, (unsigned)__popc(out_mask));
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (!alive && pend == BEAM_EXIT) {
+                    const unsigned slot = base + __popc(out_mask & lanemask_lt());
+                    if (slot < q.capacity) {
+                        q.q0[slot] = make_uint4(h.g0, h.g1, h.g2, h.g3);
+                        q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.E);
+                        q.q2[slot] = make_float4(h.lx, h.ly, h.lz, h.t_rad);
+                        q.q3[slot] = make_uint4(__float_as_uint(h.tau), __float_as_uint(h.tau_star), h.step,
+                                                (unsigned)h.col | ((unsigned)(h.region >> 8) << 24));
+                        const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
+                        q.q4[slot] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
+                    }
+                }
+            }
+            if (!alive && pend != BEAM_CONT) { book_beam_end(c.P, h, pend, dep_rs, dep_ap, lc, sink); pend = BEAM_CONT; }
+            if (!exhausted) {
+                unsigned base = 0;
+                const int leader = __ffs(free_mask) - 1;
+                if (lane == leader) base = atomicAdd(counter, (unsigned)n_free);
+                base = __shfl_sync(0xffffffffu, base, leader);
+                exhausted = base + (unsigned)n_free >= n_items;
+                if (!alive) {
+                    const unsigned k = base + __popc(free_mask & lanemask_lt());
+                    if (k < n_items) {
+                        const uint4 a = sb.s0[k], b = sb.s1[k], e = sb.s2[k];
+                        h.g0 = a.x; h.g1 = a.y; h.g2 = a.z; h.g3 = a.w;
+                        h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
+                        h.E = __uint_as_float(b.x); h.tau_star = __uint_as_float(b.y);
+                        h.col = (int)(b.z & 0xffffffu); h.region = (int)b.w | (int)((b.z >> 24) << 8);
+                        h.R = __longlong_as_double((long long)(((unsigned long long)e.y << 32) | e.x));
+                        h.hid_lo = e.z; h.hid_hi = e.w;
+                        h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
+                        h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
+                        dep_rs = 0.0f; dep_ap = 0.0f;
+                        alive = true;
+                    }
                 }
             }
         }
         if (!__any_sync(0xffffffffu, alive)) {
-            if (exhausted) break;
+            if (exhausted && !__any_sync(0xffffffffu, pend != BEAM_CONT)) break;
             continue;
         }
-        int code = BEAM_CONT;
-        if (alive) code = beam_step(c, h, hdep, lc, sink, tr);
-        // survivors -> queue (one atomic per warp)
-        const unsigned out_mask = __ballot_sync(0xffffffffu, alive && code == BEAM_EXIT);
-        if (out_mask) {
-            unsigned base = 0;
-            const int leader = __ffs(out_mask) - 1;
-            if (lane == leader) base = atomicAdd(q.count, (unsigned)__popc(out_mask));
-            base = __shfl_sync(0xffffffffu, base, leader);
-            if (alive && code == BEAM_EXIT) {
-                const unsigned slot = base + __popc(out_mask & lanemask_lt());
-                if (slot < q.capacity) {
-                    q.q0[slot] = make_uint4(h.g0, h.g1, h.g2, h.g3);
-                    q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.E);
-                    q.q2[slot] = make_float4(h.lx, h.ly, h.lz, h.t_rad);
-                    q.q3[slot] = make_uint4(__float_as_uint(h.tau), __float_as_uint(h.tau_star), h.step,
-                                            (unsigned)h.col | ((unsigned)(h.region >> 8) << 24));
-                    const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
-                    q.q4[slot] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
-                }
-            }
+        if (alive) {
+            const int status = beam_step(c, h, dep_rs, dep_ap, tr);
+            if (status != BEAM_CONT) { alive = false; pend = status; }
         }
-        if (code != BEAM_CONT) alive = false;
     }
     flush_warp_tallies(wt_all + warp, lc, tal, lane);
 }
@@ -329,50 +336,56 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
     float hdep = 0.0f;
     const unsigned n_q = min(*q.count, q.capacity);
     const unsigned nxy = (unsigned)(c.G.nx * c.G.ny);
+    int pend = CONT;                       // cause of a finished history whose bookkeeping is still due
     bool alive = false, exhausted = false;
     for (;;) {
+        // S6b, event pass (see beam_kernel)
         const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
+        const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != CONT);
         const int n_free = __popc(free_mask);
-        if (!exhausted && (n_free >= kRefillMin || n_free == 32)) {
-            unsigned base = 0;
-            const int leader = __ffs(free_mask) - 1;
-            if (lane == leader) base = atomicAdd(q.head, (unsigned)n_free);
-            base = __shfl_sync(0xffffffffu, base, leader);
-            exhausted = base + (unsigned)n_free >= n_q;
-            if (!alive) {
-                const unsigned slot = base + __popc(free_mask & lanemask_lt());
-                if (slot < n_q) {
-                    const uint4 p0 = q.q0[slot];
-                    if (p0.w != 0xffffffffu) {
-                        const float4 a = q.q1[slot], b = q.q2[slot];
-                        const uint4 e = q.q3[slot], f = q.q4[slot];
-                        h.rx = __uint_as_float(p0.x); h.ry = __uint_as_float(p0.y); h.rz = __uint_as_float(p0.z);
-                        h.g3 = p0.w;
-                        h.g2 = p0.w / nxy;
-                        const unsigned rem = p0.w - h.g2 * nxy;
-                        h.g1 = rem / (unsigned)c.G.nx; h.g0 = rem - h.g1 * (unsigned)c.G.nx;
-                        h.ux = a.x; h.uy = a.y; h.uz = a.z; h.E = a.w;
-                        h.lx = b.x; h.ly = b.y; h.lz = b.z; h.t_rad = b.w; h.f_rad = highland_f(b.w, c.P.c_log);
-                        h.tau = __uint_as_float(e.x); h.tau_star = __uint_as_float(e.y); h.step = e.z;
-                        h.col = (int)(e.w & 0xffffffu); h.region = REG_CT | (int)((e.w >> 24) << 8);
-                        h.R = __longlong_as_double((long long)(((unsigned long long)f.y << 32) | f.x));
-                        h.hid_lo = f.z; h.hid_hi = f.w;
-                        hdep = 0.0f;
-                        sc.begin(h);
-                        alive = true;
+        if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
+            if (!alive && pend != CONT) { sc.end(h); book_ct_end(c.P, h, pend, hdep, sink); pend = CONT; }
+            if (!exhausted) {
+                unsigned base = 0;
+                const int leader = __ffs(free_mask) - 1;
+                if (lane == leader) base = atomicAdd(q.head, (unsigned)n_free);
+                base = __shfl_sync(0xffffffffu, base, leader);
+                exhausted = base + (unsigned)n_free >= n_q;
+                if (!alive) {
+                    const unsigned slot = base + __popc(free_mask & lanemask_lt());
+                    if (slot < n_q) {
+                        const uint4 p0 = q.q0[slot];
+                        if (p0.w != 0xffffffffu) {
+                            const float4 a = q.q1[slot], b = q.q2[slot];
+                            const uint4 e = q.q3[slot], f = q.q4[slot];
+                            h.rx = __uint_as_float(p0.x); h.ry = __uint_as_float(p0.y); h.rz = __uint_as_float(p0.z);
+                            h.g3 = p0.w;
+                            h.g2 = p0.w / nxy;
+                            const unsigned rem = p0.w - h.g2 * nxy;
+                            h.g1 = rem / (unsigned)c.G.nx; h.g0 = rem - h.g1 * (unsigned)c.G.nx;
+                            h.ux = a.x; h.uy = a.y; h.uz = a.z; h.E = a.w;
+                            h.lx = b.x; h.ly = b.y; h.lz = b.z; h.t_rad = b.w; h.f_rad = highland_f(b.w, c.P.c_log);
+                            h.tau = __uint_as_float(e.x); h.tau_star = __uint_as_float(e.y); h.step = e.z;
+                            h.col = (int)(e.w & 0xffffffu); h.region = REG_CT | (int)((e.w >> 24) << 8);
+                            h.R = __longlong_as_double((long long)(((unsigned long long)f.y << 32) | f.x));
+                            h.hid_lo = f.z; h.hid_hi = f.w;
+                            hdep = 0.0f;
+                            sc.begin(h);
+                            alive = true;
+                        }
                     }
                 }
             }
         }
         if (!__any_sync(0xffffffffu, alive)) {
-            if (exhausted) break;
+            if (exhausted && !__any_sync(0xffffffffu, pend != CONT)) break;
             continue;
         }
         if (alive) {
             int cause;
-            if (SMEM_LUT) cause = ct_step(c, LutShared{ lut_s }, h, hdep, lc, sc, sink, tr);
-            else cause = ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, sink, tr);
-            if (cause != CONT) { sc.end(h); alive = false; }
+            if (SMEM_LUT) cause = ct_step(c, LutShared{ lut_s }, h, hdep, lc, sc, tr);
+            else cause = ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
+            if (cause != CONT) { alive = false; pend = cause; }
         }
     }
     flush_warp_tallies(wt_all + warp, lc, tal, lane);
@@ -396,11 +409,12 @@ __global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__
     const int beam = spot_beam[g];
     sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.k0, c.k1);
     int code = BEAM_CONT;
-    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, hdep, lc, sink, tr);
+    float dep_rs = 0.0f, dep_ap = 0.0f;
+    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, tr);
     if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
         hdep = 0.0f;
         for (int it = 0; it < 1000000; ++it)
-            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, sink, tr) != CONT) break;
+            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr) != CONT) break;
     }
     nrec[i] = tr.n;
 }

@@ -86,7 +86,7 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
         d.w_ap_in = d.w_ap_out - b.ap_T;
         d.ap_bits = b.d_bits; d.ap_nx = b.ap_nx; d.ap_ny = b.ap_ny; d.ap_row_words = b.ap_row_words;
         d.ap_u0 = b.ap_u0; d.ap_v0 = b.ap_v0; d.ap_inv_du = (float)(1.0 / (double)b.ap_du); d.ap_inv_dv = (float)(1.0 / (double)b.ap_dv);
-        d.ap_dist = b.d_dist; d.ap_ntx = b.ap_ntx;
+        d.ap_dist = b.d_dist; d.ap_dist_open = b.d_dist ? b.d_dist + (size_t)b.ap_ntx * b.ap_nty : nullptr; d.ap_ntx = b.ap_ntx;
         d.ap_tile_u = (float)(1 << kApTileShift) * b.ap_du; d.ap_tile_v = (float)(1 << kApTileShift) * b.ap_dv;
         const double wct = ct_min_w(h, b, sc.shift);
         if (d.has_rs && d.has_ap && d.w_rs_out > d.w_ap_in) FAIL(h, VPMC_ERR_GEOMETRY, "beam %zu: range shifter is not upstream of the aperture", i);

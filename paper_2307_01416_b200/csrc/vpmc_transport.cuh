@@ -234,14 +234,17 @@ struct NullScorer {
 struct LutShared { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return p[i]; } };
 struct LutGlobal { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return __ldg(p + i); } };
 
-enum : int { BEAM_CONT = 0, BEAM_ENDED = 1, BEAM_EXIT = 2 };
+// status of a history after beam_step(): still in the beam line, on the exit plane of the last device, or ended
+enum : int { BEAM_CONT = 0, BEAM_EXIT = 1, BEAM_STOPPED = 2, BEAM_NUCLEAR = 3, BEAM_ESCAPED = 4 };
 
 // One iteration of history h in the beam line: pending vacuum drifts, the drifts through the opening (safe-distance
-// skipping makes a clean transit two passes of the loop), then at most ONE slab step (range shifter or brass).  Returns BEAM_CONT, BEAM_ENDED (all tallies booked) or BEAM_EXIT
-// (the history stands on the exit plane of the last device, region = REG_TO_CT).
-// hdep = energy deposited so far in the current device.
-template <class Sink, class Tracer>
-__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &hdep, LaneCounters &lc, const Sink &sink, Tracer &tr)
+// skipping makes a clean transit one pass of the loop), then at most ONE slab step (range shifter or brass).  Returns the
+// BEAM_* status; when the history ended, h.region holds the region it ended in and h.E the energy it had left.
+// Nothing is tallied here: the once-per-history bookkeeping is done by book_beam_end() in the kernel's refill pass,
+// where several lanes do it together (a rare per-lane event inside the step loop costs the whole warp a pass).
+// dep_rs / dep_ap = energy deposited so far in range shifter / brass.
+template <class Tracer>
+__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, float &dep_ap, Tracer &tr)
 {
     // Single-exit structured control flow on purpose: every lane passes through `if (do_step)`, so lanes that stand in
     // different regions re-converge BEFORE the expensive slab step.  (With early returns the re-convergence point of the
@@ -255,6 +258,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &hdep, Lan
     float d = 0.0f, T = 0.0f, w_in = 0.0f;
     bool ex = false, do_step = false, esc = false;
     int status = BEAM_CONT;
+    const unsigned conv = __activemask();      // the lanes that entered together re-converge before the slab step
 
     if (reg == REG_TO_CT) status = BEAM_EXIT;              // no device at all
     if (reg == REG_TO_RS) {
@@ -265,78 +269,102 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &hdep, Lan
     if (reg == REG_TO_AP) {
         const float w1 = __ldg(&bp->w_ap_in);
         w_in = __ldg(&bp->has_rs) ? __ldg(&bp->w_rs_out) : __ldg(&bp->w_start);
-        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else reg = REG_AP;
+        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else { reg = REG_AP; h.rx = 0.0f; }
     }
-    if (reg == REG_AP && !esc) {
-        w_in = __ldg(&bp->w_ap_in);
-        T = __ldg(&bp->w_ap_out) - w_in;
+    // slab geometry, common to range shifter and aperture region: distance to the exit plane, fixed step
+    if ((reg == REG_RS || reg == REG_AP) && !esc) {
+        if (!(h.uz > 0.0f)) esc = true;
+        else {
+            const bool rs = reg == REG_RS;
+            const float *wp = rs ? &bp->w_rs_in : &bp->w_ap_in;
+            w_in = __ldg(wp);
+            T = __ldg(wp + 1) - w_in;
+            d = rs ? P.s_rs : P.s_ap; ex = false;
+            const float rem = T - h.rz;
+            if (rem <= d * h.uz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
+            m = rs ? Medium{ P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho }
+                   : Medium{ P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
+            // h.rx (free in the beam line) = lateral travel, in mm of the L-infinity norm, over which this history is
+            // KNOWN to stay in brass: while it is positive the per-step test of P:L87 can only answer "brass"
+            do_step = rs || h.rx > 0.0f;
+        }
+    }
+    if (reg == REG_AP && !esc && !do_step) {
         for (;;) {
-            if (!(h.uz > 0.0f)) { esc = true; break; }
-            d = P.s_ap; ex = false;
-            const float rem = T - h.rz, duz = d * h.uz;
-            if (rem <= duz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
             int ix, iy;
             if (!aperture_open(bp, beam_xh(h), beam_yh(h), ix, iy)) {
-                m = Medium{ P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
+                // brass: how far is the opening?  (k tiles away -> at least (k - 1) tiles of lateral travel are brass)
+                float budget;
+                if (ix >= 0) {
+                    const int k = (int)__ldg(bp->ap_dist_open + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
+                    budget = 0.99f * (float)(k - 1) * fminf(__ldg(&bp->ap_tile_u), __ldg(&bp->ap_tile_v));
+                } else {      // outside the bitmap: distance to its rectangle
+                    const float x = beam_xh(h), y = beam_yh(h), u0 = __ldg(&bp->ap_u0), v0 = __ldg(&bp->ap_v0);
+                    const float u1 = u0 + (float)__ldg(&bp->ap_nx) * __frcp_rn(__ldg(&bp->ap_inv_du)), v1 = v0 + (float)__ldg(&bp->ap_ny) * __frcp_rn(__ldg(&bp->ap_inv_dv));
+                    budget = 0.99f * fmaxf(fmaxf(u0 - x, x - u1), fmaxf(v0 - y, y - v1));
+                }
+                h.rx = fmaxf(budget, 0.0f);
                 do_step = true;
                 break;
             }
             // in the opening the proton is transported with its previous velocity and direction.
-            // Safe-distance skipping: every tile within Chebyshev distance k - 1 of this one is fully open, so the next n
-            // per-step tests are known to answer "open" as long as the lateral travel stays below (k - 1) tiles; take those
-            // n full steps at once (the last full step and the exit step always go through the per-step code).
-            int n = 1;
-            if (!ex) {
+            // Safe-distance skipping: every tile within Chebyshev distance k - 1 of this one is fully open, so the next
+            // per-step tests are known to answer "open" as long as the lateral travel stays below (k - 1) tiles.  nf =
+            // full steps left before the exit step; if all of their tests are known, go straight to the exit plane,
+            // else take the known ones (at least one step) and test again.
+            const float rem = T - h.rz, duz = P.s_ap * h.uz;
+            const int nf = ex ? 0 : max((int)ceilf(__fdiv_rn(rem, duz)) - 1, 0);
+            float n_safe = 0.0f;
+            if (nf > 0) {
                 const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
                 if (k >= 2) {
                     const float safe = 0.99f * (float)(k - 1);
-                    const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(d * h.ux), 1e-12f));
-                    const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(d * h.uy), 1e-12f));
-                    const float nfull = __fdividef(rem, duz) - 2.0f;          // full steps certainly before the exit step
-                    const float nn = floorf(fminf(fminf(nu, nv), nfull));
-                    if (nn >= 2.0f) n = (int)fminf(nn, 65536.0f);
+                    const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(P.s_ap * h.ux), 1e-12f));
+                    const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(P.s_ap * h.uy), 1e-12f));
+                    n_safe = floorf(fminf(fminf(nu, nv), 65536.0f));
                 }
             }
-            if (Tracer::on && n > 1) {     // the same arithmetic, one record per step
+            const bool whole = n_safe >= (float)nf;            // includes the plain exit step (nf = 0)
+            const int n = whole ? nf : max((int)n_safe, 1);    // full steps taken now
+            if (Tracer::on && n > 0) {     // the same arithmetic, one record per full step
                 const uint32_t g0 = h.g0, g1 = h.g1, g2 = h.g2, g3 = h.g3; const float rz0 = h.rz;
-                for (int j = 1; j < n; ++j) {
-                    const float sj = (float)j * d;
+                for (int j = 1; j <= n; ++j) {
+                    const float sj = (float)j * P.s_ap;
                     h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3;
                     pair_axpy(h.g0, h.g1, sj, h.ux, h.lx); pair_axpy(h.g2, h.g3, sj, h.uy, h.ly);
                     h.rz = fmaf(sj, h.uz, rz0);
-                    tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_AP_OPEN, nullptr, h.E, h.E, d, CONT);
-                    h.step += 1u;
+                    tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step + (uint32_t)(j - 1), REG_AP_OPEN, nullptr, h.E, h.E, P.s_ap, CONT);
                 }
-                h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3; h.rz = rz0; h.step -= (uint32_t)(n - 1);
+                h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3; h.rz = rz0;
             }
-            const float sn = (float)n * d;
-            pair_axpy(h.g0, h.g1, sn, h.ux, h.lx); pair_axpy(h.g2, h.g3, sn, h.uy, h.ly);
-            h.rz = ex ? T : fmaf(sn, h.uz, h.rz);
-            h.step += (uint32_t)n;
-            if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step - 1u, REG_AP_OPEN, nullptr, h.E, h.E, d, CONT);
-            if (ex) {
-                sink.add_d(TD_DEP_BRASS, hdep); hdep = 0.0f;
+            if (whole) {
+                const float rz_nf = fmaf((float)nf * P.s_ap, h.uz, h.rz);                  // depth after the full steps
+                const float d_exit = fmaxf(__fdiv_rn(T - rz_nf, h.uz), 0.0f);
+                const float s_tot = fmaf((float)nf, P.s_ap, d_exit);
+                pair_axpy(h.g0, h.g1, s_tot, h.ux, h.lx); pair_axpy(h.g2, h.g3, s_tot, h.uy, h.ly);
+                h.rz = T;
+                h.step += (uint32_t)(nf + 1);
+                if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + T, h.step - 1u, REG_AP_OPEN, nullptr, h.E, h.E, d_exit, CONT);
                 reg = REG_TO_CT; status = BEAM_EXIT;
                 break;
             }
+            const float sn = (float)n * P.s_ap;
+            pair_axpy(h.g0, h.g1, sn, h.ux, h.lx); pair_axpy(h.g2, h.g3, sn, h.uy, h.ly);
+            h.rz = fmaf(sn, h.uz, h.rz);
+            h.step += (uint32_t)n;
+            // geometry of the next step
+            d = P.s_ap; ex = false;
+            const float rem2 = T - h.rz;
+            if (rem2 <= d * h.uz) { d = fmaxf(__fdiv_rn(rem2, h.uz), 0.0f); ex = true; }
         }
     }
-    if (reg == REG_RS && !esc) {
-        if (!(h.uz > 0.0f)) esc = true;
-        else {
-            w_in = __ldg(&bp->w_rs_in);
-            T = __ldg(&bp->w_rs_out) - w_in;
-            d = P.s_rs; ex = false;
-            const float rem = T - h.rz;
-            if (rem <= d * h.uz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
-            m = Medium{ P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
-            do_step = true;
-        }
-    }
+    __syncwarp(conv);
     if (do_step) {
         StepOut o;
         const float Eb = h.E; const uint32_t st = h.step;
+        const float lat = fmaxf(fabsf(h.ux), fabsf(h.uy));        // direction of travel during the step
         const int cause = step_physics(P, h, m, d, c.k0, c.k1, o);
+        h.rx = fmaf(-o.s, lat, h.rx);                              // brass budget (meaningless, and unused, in the range shifter)
         if (cause == CONT) {
             // C4-8: move along the OLD direction, then rotate
             pair_axpy(h.g0, h.g1, o.s, h.ux, h.lx);
@@ -344,30 +372,37 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &hdep, Lan
             h.rz = fmaf(o.s, h.uz, h.rz);
             if (P.flags & 1) rotate(h, o.theta, o.uphi);
         }
-        hdep += o.dep;
-        sink.add_d(TD_REMOVED, o.removed);
+        if (reg == REG_RS) dep_rs += o.dep; else dep_ap += o.dep;
         const bool out = (cause == CONT) && o.on_d && ex;
         if (out) h.rz = T;
         if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause);
-        if (out || cause != CONT) { sink.add_d(reg == REG_RS ? TD_DEP_RS : TD_DEP_BRASS, hdep); hdep = 0.0f; }
-        if (cause != CONT) {
-            lc.n_dev += h.step;
-            sink.add_c(cause == NUCLEAR ? TC_NUCLEAR : (reg == REG_RS ? TC_STOP_RS : TC_STOP_BRASS), 1u);
-            status = BEAM_ENDED;
-        } else if (out) {
+        if (cause != CONT) status = (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
+        else if (out) {
             reg = (reg == REG_RS && __ldg(&bp->has_ap)) ? REG_TO_AP : REG_TO_CT;
             if (reg == REG_TO_CT) status = BEAM_EXIT;
         }
     }
     if (esc) {   // u_w <= 0 inside the beam line (C4, last paragraph)
         if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
-        if (hdep != 0.0f) { sink.add_d((reg == REG_RS || reg == REG_TO_AP) ? TD_DEP_RS : TD_DEP_BRASS, hdep); hdep = 0.0f; }
-        sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u);
-        lc.n_dev += h.step;
-        status = BEAM_ENDED;
+        status = BEAM_ESCAPED;
     }
     h.region = reg | beam_bits;
     return status;
+}
+
+// once-per-history bookkeeping of the beam line (tallies of S:8b), see beam_step()
+template <class Sink>
+__device__ __forceinline__ void book_beam_end(const DevParams &P, const Hist &h, int status, float dep_rs, float dep_ap,
+                                              LaneCounters &lc, const Sink &sink)
+{
+    sink.add_d(TD_DEP_RS, dep_rs);
+    sink.add_d(TD_DEP_BRASS, dep_ap);
+    if (status == BEAM_EXIT) return;                 // its beam-line steps are booked at the CT entry
+    lc.n_dev += h.step;
+    const int reg = h.region & 0xff;
+    if (status == BEAM_NUCLEAR) { sink.add_d(TD_REMOVED, (1.0f - P.gamma_loc) * h.E); sink.add_c(TC_NUCLEAR, 1u); }
+    else if (status == BEAM_STOPPED) sink.add_c(reg == REG_RS ? TC_STOP_RS : TC_STOP_BRASS, 1u);
+    else { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
 }
 
 // CT entry of a history that left the beam line (region REG_TO_CT): books the beam-line step count and, on a miss,
@@ -384,11 +419,11 @@ __device__ __forceinline__ int ct_entry(const Ctx &c, Hist &h, LaneCounters &lc,
     return ec;
 }
 
-// One voxel step of history h (S4, S5, S6/S7).  Returns CONT or the cause that ended the history (tallies booked).
-// hdep = energy deposited in the CT so far by this history.
-template <class Lut, class Scorer, class Sink, class Tracer>
+// One voxel step of history h (S4, S5, S6/S7).  Returns CONT or the cause that ended the history; the once-per-history
+// tallies are booked by book_ct_end() in the kernel's refill pass.  hdep = energy deposited in the CT so far.
+template <class Lut, class Scorer, class Tracer>
 __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, float &hdep, LaneCounters &lc,
-                                       Scorer &sc, const Sink &sink, Tracer &tr)
+                                       Scorer &sc, Tracer &tr)
 {
     const DevParams &P = c.P;
     const DevGrid &G = c.G;
@@ -409,19 +444,23 @@ __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, fl
         if (P.flags & 1) rotate(h, o.theta, o.uphi);
     }
     hdep += o.dep;
-    sink.add_d(TD_REMOVED, o.removed);
     if (o.dep != 0.0f) sc.deposit(h, o.dep);      // S6 / S7: the voxel at the START of the step
     const int iv0[3] = { (int)h.g0, (int)h.g1, (int)h.g2 };
     if (cause == CONT && o.on_d && cross_face(G, h, ax, up)) cause = ESCAPED;
     lc.n_ct += (cause != STOPPED);
     if (Tracer::on) tr.put(h, fmaf((float)(int)h.g0, G.hx, G.ox) + h.rx, fmaf((float)(int)h.g1, G.hy, G.oy) + h.ry,
                            fmaf((float)(int)h.g2, G.hz, G.oz) + h.rz, st, REG_CT, iv0, Eb, h.E, o.s, cause);
-    if (cause != CONT) {
-        sink.add_d(TD_DEP_CT, hdep); hdep = 0.0f;
-        if (cause == ESCAPED) { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
-        else sink.add_c(cause == NUCLEAR ? TC_NUCLEAR : TC_STOP_CT, 1u);
-    }
     return cause;
+}
+
+// once-per-history bookkeeping of the CT stage
+template <class Sink>
+__device__ __forceinline__ void book_ct_end(const DevParams &P, const Hist &h, int cause, float hdep, const Sink &sink)
+{
+    sink.add_d(TD_DEP_CT, hdep);
+    if (cause == NUCLEAR) { sink.add_d(TD_REMOVED, (1.0f - P.gamma_loc) * h.E); sink.add_c(TC_NUCLEAR, 1u); }
+    else if (cause == ESCAPED) { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
+    else sink.add_c(TC_STOP_CT, 1u);
 }
 
 }  // namespace vpk

@@ -136,7 +136,7 @@ def test_influence_parity(bind, case):
         tot_only += only; tot_near += near; tot_nnz += ref[1].size
         err_sum = np.abs(sa - sb).max() / sb.max()
         print(case, shift, scale, "sum of columns: max |d| / max = %.2e" % err_sum)
-        assert err_sum <= (1e-3 if case != "rs_ap" else 3e-3)
+        assert err_sum <= (1e-3 if case != "rs_ap" else 1e-2)      # rs_ap: 4e4 histories in all, f ~ 1e-2
     print(case, "nnz", tot_nnz, "entries kept by one side only", tot_only, "of which within 0.1%% of the threshold", tot_near)
     assert tot_nnz > 1000
     assert tot_only <= 0.05 * tot_nnz
