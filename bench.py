@@ -27,10 +27,16 @@ if ROOT not in sys.path:
 
 METRIC = "proton histories/s"
 SEED = 2
-# dominant kernel = voxel_kernel; ALU-bound.  Thread-instructions per CT step, from the committed
-# ncu capture (profiles/): smsp__thread_inst_executed.sum / CT steps of the launch.
-INST_PER_CT_STEP = 530.0
-ALG_BYTES_PER_CT_STEP = 10.0           # 2 B HU read + 4 B read + 4 B write of the dose add
+# The path is bound by plain ALU / MUFU instruction issue.  Unit of work = one material step of one history;
+# per-unit figure = USEFUL lane-instructions of that step (step physics + Philox + rotation + move + the stage's geometry),
+# from the committed ncu source-level counts (profiles/r1_*): overhead passes (refill, bookkeeping, idle lanes) are
+# deliberately not counted, so `frac` is the fraction of the issue peak spent on the method's arithmetic.
+INST_PER_SLAB_STEP = 450.0            # beam_kernel: range-shifter / brass step
+INST_PER_CT_STEP = 510.0              # voxel_kernel: voxel step incl. face distance, material fetch, scoring
+ALG_BYTES_PER_CT_STEP = 10.0          # 2 B HU read + 4 B read + 4 B write of the dose add
+ALG_BYTES_PER_HISTORY_BEAM = 48.0     # source record read; + 80 B queue record written per survivor
+# DRAM traffic per history of the two kernels, from the ncu --set full capture (profiles/r1_ncu_full.md)
+DRAM_BYTES_PER_HISTORY = {"beam_kernel": 63.0, "voxel_kernel": 22.0}
 
 
 def load_peaks():
@@ -221,29 +227,41 @@ def run_b200(args):
     hist_per_step = N * len(plans) * world
     value = hist_per_step * args.steps / (t_ms * 1e-3)
 
-    # ---- roofline of the dominant kernel (voxel_kernel), live CUDA-event durations from the library
+    # ---- roofline of the dominant kernel, live CUDA-event durations from the library (events on the launching stream)
     tm = {"beamline": [0.0, 0], "voxel": [0.0, 0], "scoring": [0.0, 0], "writer": [0.0, 0]}
-    steps_ct = 0
+    steps_ct = steps_slab = n_surv = 0
     for e in engines:
         for k, (ms, n) in e.timing().items():
             tm[k][0] += ms; tm[k][1] += n
         e.set_timing(False)
-        tl = e.tallies()
-        steps_ct += tl.n_steps_ct + tl.n_steps_dev       # of the last dose() call = one timed step's share
-    vox_ms, vox_n = tm["beamline"][0] + tm["voxel"][0], tm["voxel"][1]
-    ct_steps_per_launch = steps_ct * args.steps / max(vox_n, 1)
-    avg_launch_s = vox_ms * 1e-3 / max(vox_n, 1)
+        tl = e.tallies()                                 # of the last dose() call = one timed step's share
+        steps_ct += tl.n_steps_ct; steps_slab += tl.n_steps_slab
+        n_surv += tl.n_stopped_ct + tl.n_nuclear + tl.n_escaped     # upper bound of the histories that reached the CT
     peak_ginst = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e9        # lane-instructions/s at the max SM clock
-    achieved_ginst = INST_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9
-    roofline = {"bound": "alu", "kernel": "beam_kernel + voxel_kernel<0>", "achieved": achieved_ginst, "peak": peak_ginst,
-                "unit": "Glane-inst/s", "frac": achieved_ginst / peak_ginst, "traffic": None,
-                "peak_source": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (%s sm_max_mhz)" % (sm_max_mhz, peak_kind),
-                "inst_per_ct_step": INST_PER_CT_STEP, "ct_steps_per_launch": ct_steps_per_launch,
-                "avg_launch_ms": avg_launch_s * 1e3, "launches": vox_n,
-                "share_of_step": {k: v[0] / max(t_ms, 1e-9) for k, v in tm.items()},
-                "hbm": {"achieved": ALG_BYTES_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9, "peak": hbm_gbs,
-                        "unit": "GB/s", "frac": ALG_BYTES_PER_CT_STEP * ct_steps_per_launch / avg_launch_s / 1e9 / hbm_gbs,
+
+    def kernel_roofline(name, cls, inst_per_unit, units_per_step, alg_bytes_per_step):
+        ms, n = tm[cls]
+        launches = max(n, 1)
+        avg_s = ms * 1e-3 / launches
+        units = units_per_step * args.steps / launches
+        ach = inst_per_unit * units / avg_s / 1e9 if avg_s > 0 else 0.0
+        hist_per_launch = N * len(plans) * args.steps / launches
+        return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak_ginst, "unit": "Glane-inst/s", "frac": ach / peak_ginst,
+                "traffic": DRAM_BYTES_PER_HISTORY[name] * hist_per_launch, "inst_per_unit": inst_per_unit, "units_per_launch": units,
+                "avg_launch_ms": avg_s * 1e3, "launches": n, "share_of_step": ms / max(t_ms, 1e-9),
+                "hbm": {"achieved": alg_bytes_per_step * args.steps / launches / avg_s / 1e9 if avg_s > 0 else 0.0, "peak": hbm_gbs, "unit": "GB/s",
+                        "frac": (alg_bytes_per_step * args.steps / launches / avg_s / 1e9 / hbm_gbs) if avg_s > 0 else 0.0,
                         "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"}}
+
+    kr = [kernel_roofline("beam_kernel", "beamline", INST_PER_SLAB_STEP, steps_slab, ALG_BYTES_PER_HISTORY_BEAM * N * len(plans) + 80.0 * n_surv),
+          kernel_roofline("voxel_kernel", "voxel", INST_PER_CT_STEP, steps_ct, ALG_BYTES_PER_CT_STEP * steps_ct + 80.0 * n_surv)]
+    dom = max(kr, key=lambda r: r["share_of_step"])
+    roofline = dict(dom)
+    roofline["peak_source"] = "148 SM x 4 SMSP x 32 lanes x %.0f MHz (%s sm_max_mhz); DESIGN.md 7" % (sm_max_mhz, peak_kind)
+    roofline["note"] = ("timed classes: beamline = source_kernel + beam_kernel, voxel = entry_kernel + voxel_kernel; the one-thread-per-item "
+                        "source / entry kernels are < 5 % of their class (profiles/r1_launches.md)")
+    roofline["other_kernels"] = [r for r in kr if r is not dom]
+    roofline["share_of_step"] = {k: v[0] / max(t_ms, 1e-9) for k, v in tm.items()}
 
     # ---- e2e: host buffers in, host dose out, through the C-ABI, H2D/D2H inside the timed region
     pinned_problems = [pin_problem(p) for p in problems]

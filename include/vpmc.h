@@ -117,6 +117,7 @@ typedef struct {
     double incident, dep_ct, dep_rs, dep_brass, escaped, removed;                   /* MeV */
     uint64_t n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;     /* histories by fate */
     uint64_t n_steps_ct, n_steps_dev;   /* steps taken in the CT / in the beam line (drifts included) */
+    uint64_t n_steps_slab;              /* material steps among n_steps_dev (range shifter + brass) */
 } vpmc_tallies;
 
 /* One step of one history (vpmc_trace).  r, u after the step: beam frame in the beam line, CT frame from the

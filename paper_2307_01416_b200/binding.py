@@ -62,7 +62,7 @@ class _Csr(C.Structure):
 class Tallies(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("incident", "dep_ct", "dep_rs", "dep_brass", "escaped", "removed")] + \
                [(n, C.c_uint64) for n in ("n_stopped_ct", "n_stopped_rs", "n_stopped_brass", "n_nuclear", "n_escaped",
-                                          "n_steps_ct", "n_steps_dev")]
+                                          "n_steps_ct", "n_steps_dev", "n_steps_slab")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -29,7 +29,7 @@ static thread_local std::string g_create_err;
     } while (0)
 
 static constexpr size_t kMaxSmemLut = 96 * 1024;      // larger material tables are read through L1 instead
-static constexpr unsigned long long kChunk = 1ull << 23;   // work items per pass of the pipeline = queue capacity
+static unsigned long long kChunk = 1ull << 23;             // work items per pass of the pipeline = queue capacity (VPMC_CHUNK overrides)
 
 // grow-only device buffer
 static int ensure(vpmc_t *h, DevBuf &b, size_t bytes);
@@ -173,6 +173,7 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     {
         h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
         if (const char *e = getenv("VPMC_LUT")) { if (!strcmp(e, "global")) h->smem_lut = false; }
+        if (const char *e = getenv("VPMC_CHUNK")) { const long long v = atoll(e); if (v >= 1024 && v <= (1ll << 30)) kChunk = (unsigned long long)v; }
         int occ = 0;
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel, kBlock, 0));
         h->grid_beam = std::max(occ, 1) * h->n_sm;

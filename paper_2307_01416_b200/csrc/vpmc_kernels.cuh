@@ -163,8 +163,9 @@ __device__ __forceinline__ void flush_warp_tallies(WarpTally *w, const LaneCount
 {
     const double inc = warp_sum(lc.incident);
     const unsigned nct = __reduce_add_sync(0xffffffffu, lc.n_ct), ndev = __reduce_add_sync(0xffffffffu, lc.n_dev);
+    const unsigned nslab = __reduce_add_sync(0xffffffffu, lc.n_slab);
     __syncwarp();
-    if (lane == 0) { w->d[TD_INCIDENT] += inc; w->c[TC_STEPS_CT] += nct; w->c[TC_STEPS_DEV] += ndev; }
+    if (lane == 0) { w->d[TD_INCIDENT] += inc; w->c[TC_STEPS_CT] += nct; w->c[TC_STEPS_DEV] += ndev; w->c[TC_STEPS_SLAB] += nslab; }
     __syncwarp();
     if (lane < TD_N && w->d[lane] != 0.0) atomicAdd(&tal->incident + lane, w->d[lane]);
     if (lane < TC_N && w->c[lane]) atomicAdd(&tal->n_stopped_ct + lane, (unsigned long long)w->c[lane]);
@@ -268,7 +269,7 @@ beam_kernel(const Ctx c, const unsigned int n_items, const SourceBuf sb, const Q
             continue;
         }
         if (alive) {
-            const int status = beam_step(c, h, dep_rs, dep_ap, tr);
+            const int status = beam_step(c, h, dep_rs, dep_ap, lc, tr);
             if (status != BEAM_CONT) { alive = false; pend = status; }
         }
     }
@@ -410,7 +411,7 @@ __global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__
     sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.k0, c.k1);
     int code = BEAM_CONT;
     float dep_rs = 0.0f, dep_ap = 0.0f;
-    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, tr);
+    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, lc, tr);
     if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
         hdep = 0.0f;
         for (int it = 0; it < 1000000; ++it)

@@ -14,13 +14,13 @@ namespace vpk {
 struct DevTallies {
     double incident, dep_ct, dep_rs, dep_brass, escaped, removed;
     unsigned long long n_stopped_ct, n_stopped_rs, n_stopped_brass, n_nuclear, n_escaped;
-    unsigned long long n_steps_ct, n_steps_dev;
+    unsigned long long n_steps_ct, n_steps_dev, n_steps_slab;
 };
 enum : int { TD_INCIDENT = 0, TD_DEP_CT, TD_DEP_RS, TD_DEP_BRASS, TD_ESCAPED, TD_REMOVED, TD_N };
-enum : int { TC_STOP_CT = 0, TC_STOP_RS, TC_STOP_BRASS, TC_NUCLEAR, TC_ESCAPED, TC_STEPS_CT, TC_STEPS_DEV, TC_N };
+enum : int { TC_STOP_CT = 0, TC_STOP_RS, TC_STOP_BRASS, TC_NUCLEAR, TC_ESCAPED, TC_STEPS_CT, TC_STEPS_DEV, TC_STEPS_SLAB, TC_N };
 
 // per-warp partial tallies in shared memory (fp64 sums; flushed to DevTallies once per warp at kernel end)
-struct WarpTally { double d[TD_N]; unsigned int c[TC_N]; unsigned int pad; };
+struct WarpTally { double d[TD_N]; unsigned int c[TC_N]; };
 
 struct SmemSink {
     WarpTally *w;
@@ -223,7 +223,7 @@ __device__ __forceinline__ bool cross_face(const DevGrid &G, Hist &h, int ax, bo
 }
 
 // per-thread counters that live for the whole kernel (flushed once at its end)
-struct LaneCounters { unsigned int n_ct = 0, n_dev = 0; double incident = 0.0; };
+struct LaneCounters { unsigned int n_ct = 0, n_dev = 0, n_slab = 0; double incident = 0.0; };
 
 struct NullScorer {
     __device__ __forceinline__ void begin(const Hist &) {}
@@ -244,7 +244,7 @@ enum : int { BEAM_CONT = 0, BEAM_EXIT = 1, BEAM_STOPPED = 2, BEAM_NUCLEAR = 3, B
 // where several lanes do it together (a rare per-lane event inside the step loop costs the whole warp a pass).
 // dep_rs / dep_ap = energy deposited so far in range shifter / brass.
 template <class Tracer>
-__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, float &dep_ap, Tracer &tr)
+__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, float &dep_ap, LaneCounters &lc, Tracer &tr)
 {
     // Single-exit structured control flow on purpose: every lane passes through `if (do_step)`, so lanes that stand in
     // different regions re-converge BEFORE the expensive slab step.  (With early returns the re-convergence point of the
@@ -373,6 +373,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
             if (P.flags & 1) rotate(h, o.theta, o.uphi);
         }
         if (reg == REG_RS) dep_rs += o.dep; else dep_ap += o.dep;
+        lc.n_slab += (cause != STOPPED);
         const bool out = (cause == CONT) && o.on_d && ex;
         if (out) h.rz = T;
         if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause);

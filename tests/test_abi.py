@@ -31,7 +31,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 def test_struct_mirrors_match_the_header_sizes():
     from paper_2307_01416_b200 import binding
     assert ctypes.sizeof(binding.Params) == 25 * 4
-    assert ctypes.sizeof(binding.Tallies) == 6 * 8 + 7 * 8
+    assert ctypes.sizeof(binding.Tallies) == 6 * 8 + 8 * 8
     assert binding.STEP_DTYPE.itemsize == 72
     assert ctypes.sizeof(binding.Scenario) == 16
 
