@@ -197,10 +197,17 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     const double Rp = fma(-(double)s, (double)m.rsp, h.R);
     // E is re-derived from the fp64 range every step, so a 3e-7 relative MUFU error does not accumulate
     const float Ebar = exp2f(P.inv_p * __log2f((float)Rp * P.inv_alpha));
+    // mean energy lost in the step.  E - Ebar cancels when the step is thin in water-equivalent terms (1 mm of air
+    // loses 5e-4 MeV of 150: fp32 resolves 1.5e-5, the MUFU pow 4e-5), so for s rsp / R < 0.03 it is taken from
+    // Ebar ((R / R')^(1/p) - 1) = Ebar expm1(-log1p(-x) / p) with two short series (relative error < 1e-7).
+    const float x = __fdividef(s * m.rsp, R);
+    const float Lm = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 0.2f, 0.25f), 1.0f / 3.0f), 0.5f), 1.0f);
+    const float y = P.inv_p * Lm;
+    const float dEm = (x < 0.03f) ? Ebar * (y * fmaf(y, fmaf(y, fmaf(y, 1.0f / 24.0f, 1.0f / 6.0f), 0.5f), 1.0f)) : E - Ebar;
     // 3
     const float4 u = draw4(h, h.step, 0u, k0, k1);
     // 4
-    float Ep = Ebar;
+    float Ep = Ebar, dep = dEm;
     double Rn = Rp;
     if (P.flags & 2) {
         const float Emid = 0.5f * (E + Ebar);
@@ -208,9 +215,10 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
         const float var = P.k_bohr * m.za_rho * s * 0.5f * fmaf(g, g, 1.0f);   // gamma^2 (1 - beta^2/2) = (gamma^2+1)/2
         const float dE = -sqrt_fast(var * bm_radius2_fast(u.z)) * cos_2pi_fast(u.w);
         Ep = Ebar + dE;
-        if (Ep <= 0.0f) { Ep = 0.0f; Rn = 0.0; }
-        else if (Ep >= E) { Ep = E; Rn = h.R; }
+        if (Ep <= 0.0f) { Ep = 0.0f; Rn = 0.0; dep = E; }
+        else if (Ep >= E) { Ep = E; Rn = h.R; dep = 0.0f; }
         else {
+            dep = dEm - dE;
             const float dl = __fdividef(dE, Ebar);
             float g1;                                   // (1 + dl)^p - 1
             if (fabsf(dl) < 0.05f) g1 = dl * fmaf(dl, fmaf(dl, fmaf(dl, fmaf(dl, P.pc5, P.pc4), P.pc3), P.pc2), P.p);
@@ -219,7 +227,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
         }
     }
     // 5
-    o.dep = E - Ep;
+    o.dep = dep;
     o.s = s;
     // 6
     if (P.flags & 4) {

@@ -123,3 +123,174 @@ def small_water(n=(8, 8, 40), h=(2.0, 2.0, 2.0), energy=70.0, sigma=1.5, with_ap
     sp = [((j - 0.5 * (n_spots - 1)) * 2.0, 0.0, energy, 1.0 + j, sigma) for j in range(n_spots)]
     return {"name": "small_water", "ct": ct, "calib": calibration(),
             "beams": [beam(sp, iso=(0, 0, z_iso), rs_wet=rs_wet, rs_face=rs_face, aperture=ap)]}
+
+
+# ------------------------------------------------------------------------------------------ configs 3-5
+# Plan design below (which energies reach the target, whether a range shifter is needed) uses the water-equivalent
+# depth along the beam axis.  It is an INPUT choice made by the harness, like a planning system's; no transport code.
+
+ALPHA, P_EXP = 0.022, 1.77
+
+
+def _rsp_of_hu(hu):
+    return np.interp(hu, CALIB_NODES[:, 0], CALIB_NODES[:, 1])
+
+
+def _range_w(E):
+    return ALPHA * np.asarray(E, dtype=np.float64) ** P_EXP
+
+
+def _energy_of_range(R):
+    return (np.asarray(R, dtype=np.float64) / ALPHA) ** (1.0 / P_EXP)
+
+
+def _beam_rot(direction):
+    """rot (3x3, columns = beam axes in the CT frame) with the third column = direction of travel."""
+    w = np.asarray(direction, dtype=np.float64)
+    w = w / np.linalg.norm(w)
+    a = np.array([0.0, 0.0, 1.0]) if abs(w[2]) < 0.9 else np.array([1.0, 0.0, 0.0])
+    u = np.cross(a, w); u /= np.linalg.norm(u)
+    v = np.cross(w, u)
+    return np.stack([u, v, w], axis=1).astype(F)
+
+
+def _wet_profile(ct, iso, direction, s_lo, s_hi, ds=0.5):
+    """water-equivalent path length along iso + s*direction for s in [s_lo, s_hi], starting at 0 at s_lo."""
+    n, h, o = np.array(ct["n"]), np.array(ct["h"], dtype=np.float64), np.array(ct["origin"], dtype=np.float64)
+    s = np.arange(s_lo, s_hi, ds) + 0.5 * ds
+    p = np.asarray(iso, dtype=np.float64)[None, :] + s[:, None] * np.asarray(direction, dtype=np.float64)[None, :]
+    idx = np.floor((p - o) / h).astype(np.int64)
+    inside = ((idx >= 0) & (idx < n)).all(axis=1)
+    idx = np.clip(idx, 0, n - 1)
+    hu = ct["hu"][idx[:, 2], idx[:, 1], idx[:, 0]].astype(np.float64)
+    rsp = np.where(inside, _rsp_of_hu(hu), 0.0)
+    return s + 0.5 * ds, np.cumsum(rsp * ds)
+
+
+def _ct_min_w(ct, iso, rot):
+    n, h, o = np.array(ct["n"]), np.array(ct["h"], dtype=np.float64), np.array(ct["origin"], dtype=np.float64)
+    lo, hi = o, o + n * h
+    w = np.asarray(rot, dtype=np.float64)[:, 2]
+    return min(float(np.dot(np.where([(k >> a) & 1 for a in range(3)], hi, lo) - np.asarray(iso, dtype=np.float64), w)) for k in range(8))
+
+
+def head_ct(seed: int = 3):
+    """Synthetic head: 256x256x160 voxels of 1x1x1.5 mm, ellipsoid skull shell +1000 HU,
+    brain N(40, 20^2) HU, three air cavities, outside air."""
+    rng = np.random.default_rng(seed)
+    n, h = (256, 256, 160), (1.0, 1.0, 1.5)
+    origin = (-128.0, -128.0, -120.0)
+    x = origin[0] + (np.arange(n[0]) + 0.5) * h[0]
+    y = origin[1] + (np.arange(n[1]) + 0.5) * h[1]
+    z = origin[2] + (np.arange(n[2]) + 0.5) * h[2]
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    ax_o = np.array([80.0, 100.0, 105.0]); ax_i = ax_o - 7.0
+    e_o = (X / ax_o[0]) ** 2 + (Y / ax_o[1]) ** 2 + (Z / ax_o[2]) ** 2
+    e_i = (X / ax_i[0]) ** 2 + (Y / ax_i[1]) ** 2 + (Z / ax_i[2]) ** 2
+    hu = np.full(X.shape, -1000.0)
+    hu[e_o <= 1.0] = 1000.0
+    brain = e_i <= 1.0
+    hu[brain] = np.rint(rng.normal(40.0, 20.0, size=int(brain.sum())))
+    for _ in range(3):                                    # air cavities, lower-anterior interior
+        r = rng.uniform(8.0, 15.0)
+        c = np.array([rng.uniform(-25, 25), rng.uniform(35, 60), rng.uniform(-70, -35)])
+        hu[((X - c[0]) ** 2 + (Y - c[1]) ** 2 + (Z - c[2]) ** 2 <= r * r) & brain] = -1000.0
+    return {"n": n, "h": tuple(F(v) for v in h), "origin": tuple(F(v) for v in origin), "hu": hu.astype(np.int16)}
+
+
+def _plan_beam(ct, target_c, r_t, direction, pitch, layer_step=2.5, margin_spots=5.0, margin_ap=3.0, bitmap_pitch=0.1):
+    """One beam on a spherical target: isocentre = target centre; aperture opening = BEV projection + margin_ap;
+    spot lattice within r_t + margin_spots; layers every layer_step MeV over the target's WET extent +- one layer;
+    range shifter iff the proximal edge is shallower than R_w(71.3 MeV) + 5 mm (Table 1 of the paper: "Range Shifter
+    Yes/No")."""
+    rot = _beam_rot(direction)
+    d = rot[:, 2].astype(np.float64)
+    wmin = _ct_min_w(ct, target_c, rot)
+    s, wet = _wet_profile(ct, target_c, d, wmin, r_t + 1.0)
+    wet_prox = float(np.interp(-r_t, s, wet)); wet_dist = float(np.interp(r_t, s, wet))
+    use_rs = wet_prox < float(_range_w(71.3)) + 5.0
+    extra = 45.0 if use_rs else 0.0
+    e_lo = float(_energy_of_range(wet_prox + extra)) - layer_step
+    e_hi = float(_energy_of_range(wet_dist + extra)) + layer_step
+    energies = np.arange(np.ceil(max(e_lo, 70.0) / layer_step) * layer_step, min(e_hi, 230.0) + 1e-9, layer_step)
+    k = int(np.floor((r_t + margin_spots) / pitch + 1e-9))
+    g = np.arange(-k, k + 1) * pitch
+    lat = [(x, y) for y in g for x in g if x * x + y * y <= (r_t + margin_spots) ** 2 + 1e-9]
+    spots = [(x, y, E, 1.0, float(spot_sigma(E))) for E in energies for (x, y) in lat]
+    n_pix = int(2 ** np.ceil(np.log2(2.0 * (r_t + margin_ap + 2.0) / bitmap_pitch)))
+    op, u0, v0, du, dv = disc_bitmap(n_pix, bitmap_pitch, r_t + margin_ap)
+    # devices ride 150 / 190 mm upstream of the isocentre unless the CT box (with its air) reaches further
+    face = max(150.0, np.ceil(-wmin) + 5.0)
+    return beam(spots, iso=target_c, rot=rot, rs_wet=45.0 if use_rs else 0.0, rs_face=face + 40.0,
+                aperture=aperture(op, u0, v0, du, dv, 30.0, face))
+
+
+def config3(seed: int = 3, n_histories: int = 10_000_000, pitch: float = 2.5):
+    """BASELINE.json configs[2]: head CT, spherical target of volume log-uniform in 0.4-43 cc, 2 beams (the second
+    rotated 60 degrees about z), apertures = target projection + 3 mm, 2.5 mm spot pitch."""
+    ct = head_ct(seed)
+    rng = np.random.default_rng(seed + 1000)
+    vol = np.exp(rng.uniform(np.log(0.4), np.log(43.0)))              # cc
+    r_t = float((3.0 * vol * 1000.0 / (4.0 * np.pi)) ** (1.0 / 3.0))  # mm
+    phi = rng.uniform(-0.35, 0.35) + (np.pi if rng.random() < 0.5 else 0.0)      # lateral, tilted <= 20 degrees
+    d_t = np.array([np.cos(phi), np.sin(phi), rng.uniform(-0.2, 0.2)]); d_t /= np.linalg.norm(d_t)
+    ax_i = np.array([73.0, 93.0, 98.0])
+    t_surf = 1.0 / np.sqrt(((d_t / ax_i) ** 2).sum())                 # inner skull surface along d_t
+    depth = rng.uniform(15.0, 40.0) + r_t
+    c = np.round(d_t * max(t_surf - depth, 0.0), 1).astype(np.float64)
+    dir1 = -d_t                                                       # shallowest approach
+    ca, sa = np.cos(np.pi / 3), np.sin(np.pi / 3)
+    dir2 = np.array([ca * dir1[0] - sa * dir1[1], sa * dir1[0] + ca * dir1[1], dir1[2]])
+    beams = [_plan_beam(ct, c, r_t, dir1, pitch), _plan_beam(ct, c, r_t, dir2, pitch)]
+    return {"name": "config3_seed%d" % seed, "ct": ct, "calib": calibration(), "beams": beams, "n_histories": n_histories,
+            "seed": seed, "target": {"centre": c, "radius": r_t, "volume_cc": float(vol)}}
+
+
+SCENARIOS13 = ([((0.0, 0.0, 0.0), 1.0)] +
+               [(tuple(float(s) * 3.0 if a == k else 0.0 for a in range(3)), 1.0) for k in range(3) for s in (+1, -1)] +
+               [((0.0, 0.0, 0.0), 1.035), ((0.0, 0.0, 0.0), 0.965)] +
+               [((0.0, 0.0, float(sz) * 3.0), sc) for sc in (1.035, 0.965) for sz in (+1, -1)])
+
+
+def config4(hist_per_spot: int = 10_000, lo: int = 1800, hi: int = 2200, max_seed: int = 64):
+    """BASELINE.json configs[3]: influence-matrix build on a config-3 head with about 2000 spots (the first seed whose
+    plan has lo..hi spots over its 2 beams), 13 scenarios (SCENARIOS13: 3 mm, 3.5 %), threshold 1e-4."""
+    for seed in range(3, 3 + max_seed):
+        rng = np.random.default_rng(seed + 1000)
+        vol = np.exp(rng.uniform(np.log(0.4), np.log(43.0)))
+        if not (3.0 < vol < 14.0):                         # cheap pre-filter: spot count grows with the target volume
+            continue
+        w = config3(seed)
+        n = sum(b["spots"].shape[0] for b in w["beams"])
+        if lo <= n <= hi:
+            w["name"] = "config4_seed%d" % seed
+            w["hist_per_spot"] = hist_per_spot
+            w["scenarios"] = SCENARIOS13
+            w["rel_threshold"] = 1e-4
+            return w
+    raise RuntimeError("no seed gives %d..%d spots" % (lo, hi))
+
+
+def config5(seed: int = 5, n_histories: int = 100_000_000):
+    """BASELINE.json configs[4]: 512x512x200 voxels of 1 mm, random z-slabs (-1000..+1500 HU), 45 mm WET range shifter,
+    30 mm brass with a star-shaped opening (bitmap 1024^2 @ 0.1 mm), 65 layers 70..230 MeV, 5 mm lattice."""
+    rng = np.random.default_rng(seed)
+    n, h = (512, 512, 200), (1.0, 1.0, 1.0)
+    hu = np.empty((n[2], n[1], n[0]), dtype=np.int16)
+    z = 0
+    while z < n[2]:
+        t = int(rng.integers(4, 33))
+        hu[z:z + t] = np.int16(rng.integers(-1000, 1501))
+        z += t
+    ct = {"n": n, "h": tuple(F(v) for v in h), "origin": (F(-256.0), F(-256.0), F(0.0)), "hu": hu}
+    a = rng.uniform(0.0, 0.12, size=5); ph = rng.uniform(0.0, 2 * np.pi, size=5)
+    phi = np.linspace(0.0, 2 * np.pi, 720, endpoint=False)
+    r = 15.0 * (1.0 + sum(a[i] * np.cos((i + 2) * phi + ph[i]) for i in range(5)))
+    poly = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1)
+    op, u0, v0, du, dv = polygon_bitmap(1024, 0.1, poly)
+    half = np.ceil(np.abs(poly).max() / 5.0) * 5.0 + 5.0
+    g = np.arange(-half, half + 1e-9, 5.0)
+    energies = 70.0 + 2.5 * np.arange(65)
+    spots = [(x, y, E, 1.0, float(spot_sigma(E))) for E in energies for y in g for x in g]
+    b = beam(spots, iso=(0.0, 0.0, 100.0), rs_wet=45.0, rs_face=190.0, aperture=aperture(op, u0, v0, du, dv, 30.0, 150.0))
+    return {"name": "config5", "ct": ct, "calib": calibration(), "beams": [b], "n_histories": n_histories, "seed": seed}
