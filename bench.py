@@ -114,6 +114,24 @@ def pin_problem(w):
     return w
 
 
+def workload_plans(args):
+    """(label, workloads function name, kwargs) of the plans one step runs, and the default histories per plan."""
+    from paper_2307_01416_b200 import workloads as wl
+    if args.workload == "config2":
+        plans = wl.config2_plans()
+        if args.plans:
+            plans = [(int(x.split(":")[0]), bool(int(x.split(":")[1]))) for x in args.plans.split(",")]
+        return [("d%d_%s" % (d, "rs" if rs else "nors"), "config2", {"opening_mm": d, "range_shifter": rs}) for (d, rs) in plans], 10_000_000, \
+            "BASELINE.json configs[1]: water 100x100x150 @ 2 mm, 8 plans (opening 1/2/3/4 cm x RS off/on), 825-3993 spots"
+    if args.workload == "config3":
+        return [("seed%d" % s, "config3", {"seed": s}) for s in (3, 4, 5, 6)], 10_000_000, \
+            "BASELINE.json configs[2]: synthetic head CT 256x256x160 @ 1x1x1.5 mm, 2 beams, apertures = target + 3 mm, 4 patients (seeds 3-6)"
+    if args.workload == "config5":
+        return [("stress", "config5", {})], 100_000_000, \
+            "BASELINE.json configs[4]: 512x512x200 @ 1 mm random-slab phantom, RS 45 mm + star-shaped aperture, 70-230 MeV"
+    raise SystemExit("unknown --workload %s" % args.workload)
+
+
 def run_reference(args):
     """The CPU oracle on the same workload/metric; each step = a bounded sample of the plans."""
     from oracle import cpu_bench
@@ -121,15 +139,17 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    plans = wl.config2_plans()
+    plans, n_default, label = workload_plans(args)
+    if args.histories <= 0:
+        args.histories = n_default
     per_plan = args.ref_sample // len(plans)
     rates, cores = [], cpu_bench.n_cores()
     t_all = []
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         done, busy = 0, 0.0
-        for (d, rs) in plans:
-            r, cores, _ = cpu_bench.time_oracle("config2", {"opening_mm": d, "range_shifter": rs}, args.histories, SEED, per_plan)
+        for (_, fn, kw) in plans:
+            r, cores, _ = cpu_bench.time_oracle(fn, kw, args.histories, SEED, per_plan)
             busy += per_plan / r
             done += per_plan
         if it >= args.warmup:
@@ -141,7 +161,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": v, "unit": "histories/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * sum(t_all) / len(t_all), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "BASELINE.json configs[1]: 8 water-phantom plans, bounded sample", "histories_per_plan": args.histories},
+        "config": {"workload": label + " (bounded sample)", "histories_per_plan": args.histories},
         "cpu_baseline": {"value": v, "unit": "histories/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": "histories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -153,7 +173,9 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200")
-    ap.add_argument("--histories", type=int, default=10_000_000, help="histories per plan (BASELINE.json: 1e7)")
+    ap.add_argument("--workload", default="config2", help="config2 (default, the bench workload) | config3 | config5 | config4 (influence build)")
+    ap.add_argument("--histories", type=int, default=0, help="histories per plan (0 = the config's own: 1e7, 1e8 for config5)")
+    ap.add_argument("--hist-per-spot", type=int, default=10_000, help="config4: histories per spot and scenario")
     ap.add_argument("--ref-sample", type=int, default=800_000, help="oracle histories per reference step")
     ap.add_argument("--cpu-sample", type=int, default=1_600_000, help="oracle histories of the cpu_baseline leg")
     ap.add_argument("--plans", default="", help="subset of the 8 plans as opening_mm:rs pairs, e.g. 20:0,20:1 (profiling)")
@@ -163,6 +185,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "config4":
+        return run_influence(args)
     run_b200(args)
 
 
@@ -179,12 +203,10 @@ def run_b200(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     hbm_gbs, sm_max_mhz, peak_kind = load_peaks()
-    N = int(args.histories)
+    plans, n_default, label = workload_plans(args)
+    N = int(args.histories) if args.histories > 0 else n_default
     seed = dist.rank_seed(SEED, rank)
-    plans = wl.config2_plans()
-    if args.plans:
-        plans = [(int(x.split(":")[0]), bool(int(x.split(":")[1]))) for x in args.plans.split(",")]
-    problems = [wl.config2(d, rs, N, SEED) for (d, rs) in plans]
+    problems = [getattr(wl, fn)(**kw) for (_, fn, kw) in plans]
     params = binding.default_params(n_batches=args.n_batches)
 
     # ---- set-up (S0), not part of histories/s
@@ -292,20 +314,19 @@ def run_b200(args):
     out = {"metric": METRIC, "value": value, "unit": "histories/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
-           "config": {"workload": "BASELINE.json configs[1]: water 100x100x150 @ 2 mm, 8 plans (opening 1/2/3/4 cm x RS off/on), "
-                                  "825-3993 spots", "histories_per_plan": N, "plans_per_step": len(plans),
+           "config": {"workload": label, "histories_per_plan": N, "plans_per_step": len(plans),
                       "n_batches": args.n_batches, "l2_flush_between_steps": True, "parallelism": "replicas x%d + dose all-reduce" % world,
                       "setup_s": setup_s},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
 
-    if rank == 0 and world == 1 and not args.no_dose_at_unc:
+    if rank == 0 and world == 1 and not args.no_dose_at_unc and args.workload == "config2":
         out["dose_at_0p5pct"] = dose_at_uncertainty(binding, wl)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import cpu_bench
         per_plan = args.cpu_sample // len(plans)
         busy, done, cores = 0.0, 0, 1
-        for (d, rs) in plans:
-            r, cores, _ = cpu_bench.time_oracle("config2", {"opening_mm": d, "range_shifter": rs}, N, SEED, per_plan)
+        for (_, fn, kw) in plans:
+            r, cores, _ = cpu_bench.time_oracle(fn, kw, N, SEED, per_plan)
             busy += per_plan / r; done += per_plan
         out["cpu_baseline"] = {"value": done / busy, "unit": "histories/s", "cores": cores, "kind": "oracle",
                                "sample": "%d histories per plan over the %d plans, ids spread over the %d-history run, "
@@ -333,6 +354,53 @@ def dose_at_uncertainty(binding, wl, target=0.005):
     e.close()
     return {"workload": "config2 opening 2 cm, no range shifter", "seconds": sec, "histories": n + n0, "uncertainty": u,
             "pilot_uncertainty": u0, "target": target}
+
+
+
+
+def run_influence(args):
+    """--workload config4: the 13-scenario influence-matrix build (S7 + S8) on the config-3 head with ~2000 spots."""
+    import torch
+    from paper_2307_01416_b200 import binding, workloads as wl
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(0)
+    w = wl.config4(hist_per_spot=args.hist_per_spot)
+    eng = binding.Engine(w)
+    sc = [binding.scenario(s, k) for s, k in w["scenarios"]]
+    hps = int(args.hist_per_spot)
+
+    def step():
+        res = eng.influence(sc, hps, w["rel_threshold"], SEED)
+        nnz = sum(int(c.numel()) for (_, c, _) in res)
+        del res
+        return nnz
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    torch.cuda.synchronize()
+    eng.set_timing(True); eng.timing()
+    l0 = eng.launch_count()
+    sampler = ClockSampler(torch.cuda.current_device()); sampler.start()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(args.steps):
+        nnz = step()
+    b.record(); torch.cuda.synchronize()
+    clocks = sampler.stop()
+    t_ms = a.elapsed_time(b)
+    tm = eng.timing()
+    n_hist = len(sc) * eng.n_spots * hps
+    out = {"metric": METRIC, "value": n_hist * args.steps / (t_ms * 1e-3), "unit": "histories/s", "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": "BASELINE.json configs[3]: 13-scenario influence matrices on the config-3 head (%s), %d spots, "
+                                  "%d histories per spot, threshold 1e-4" % (w["name"], eng.n_spots, hps),
+                      "seconds_per_13_matrices": t_ms * 1e-3 / args.steps, "nnz_total": nnz, "csr_bytes": nnz * 8 + 13 * (eng.n_spots + 1) * 8,
+                      "l2_flush_between_steps": False, "inputs_larger_than_l2": True},
+           "clocks": clocks, "gpu_launches": eng.launch_count() - l0,
+           "share_of_step": {k: v[0] / t_ms for k, v in tm.items()}}
+    eng.close()
+    print(json.dumps(out))
 
 
 if __name__ == "__main__":

@@ -246,6 +246,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     staged += add;
                 }
             }
+            if (getenv("VPMC_DEBUG")) fprintf(stderr, "[vpmc] influence scenario %d round %d: %zu columns, %zu to replay\n", s, round, todo.size(), next.size());
             todo.swap(next);
             replay = true;
         }
