@@ -8,6 +8,8 @@
 #include <limits>
 #include <numeric>
 
+#include <cub/cub.cuh>
+
 #include "vpmc_host.h"
 
 using namespace vpk;
@@ -105,7 +107,8 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     for (void *p : ptrs) if (p) cudaFree(p);
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
-                       &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc };
+                       &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
+                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n };
     for (DevBuf *b : bufs) if (b->p) cudaFree(b->p);
     delete h;
     return VPMC_OK;

@@ -2,17 +2,20 @@
 //
 // Per scenario:
 //   1. pilot: the first n_pilot histories of every spot run in MODE 2 and leave the bounding box of their deposits;
-//   2. boxes: the pilot box of each column, grown by kGrow of its extent + kPad voxels per side, clipped to the grid;
+//   2. boxes: the pilot box of each column, grown by kGrow of its extent + kPad voxels per side, clipped to the grid
+//      (tight on purpose: the overflow list of step 4 takes the halo, and every box element is zeroed and scanned);
 //   3. columns are packed into groups whose boxes fit the workspace; per group: zero the boxes, transport all
 //      hist_per_spot histories of the group's spots in MODE 1, then max / count / scan / emit into a staging area;
-//   4. a column that deposited outside its box is NOT written; its box is replaced by the union with the bounding box
-//      of the outside deposits and the column is replayed in a later group -- streams are keyed by history id, so the
-//      replay reproduces the same histories and now fits by construction;
+//   4. deposits outside a column's box go to an overflow list of (column, voxel, MeV) entries, which is sorted, summed
+//      per voxel, thresholded with the column and merged into the row at the end.  Only when that list is full is a
+//      column NOT written: its box is replaced by the union with the bounding box of the lost deposits and the column is
+//      replayed in a later group -- streams are keyed by history id, so the replay reproduces the same histories and
+//      now fits by construction;
 //   5. row_ptr = exclusive scan of the row counts; the caller's allocator provides row_ptr / col / val and the rows are
 //      gathered from the staging area.
 
-static constexpr float kGrow = 0.30f;
-static constexpr int kPad = 2;
+static constexpr float kGrow = 0.05f;
+static constexpr int kPad = 1;
 // test knobs: VPMC_BOX_GROW / VPMC_BOX_PAD override the two constants (e.g. 0 / 0 forces the replay path)
 static float box_grow() { const char *e = getenv("VPMC_BOX_GROW"); return e ? (float)atof(e) : kGrow; }
 static int box_pad() { const char *e = getenv("VPMC_BOX_PAD"); return e ? atoi(e) : kPad; }
@@ -41,22 +44,33 @@ static int grow_keep(vpmc_t *h, DevBuf &b, size_t bytes, size_t keep, cudaStream
     return VPMC_OK;
 }
 
-// the four writer passes over a set of columns; leaves per-column counts in inf_colnnz (device)
-static int csr_count_passes(vpmc_t *h, const CsrCols &cc, float *data, bool convert, float coef, float rel_thr, cudaStream_t st)
+// writer pass 1 over a set of columns: (E_dep -> dose value,) column maxima
+static int csr_max_pass(vpmc_t *h, const CsrCols &cc, float *data, bool convert, float coef, cudaStream_t st)
 {
-    int rc = ensure(h, h->inf_tilecnt, (size_t)std::max(cc.n_tiles, 1) * sizeof(unsigned int)); if (rc) return rc;
-    rc = ensure(h, h->inf_colmax, (size_t)cc.n_cols * sizeof(unsigned int)); if (rc) return rc;
-    rc = ensure(h, h->inf_colnnz, (size_t)cc.n_cols * sizeof(long long)); if (rc) return rc;
+    int rc = ensure(h, h->inf_colmax, (size_t)cc.n_cols * sizeof(unsigned int)); if (rc) return rc;
     CU(h, cudaMemsetAsync(h->inf_colmax.p, 0, (size_t)cc.n_cols * sizeof(unsigned int), st));
-    const int grid = std::max(1, std::min(cc.n_tiles, h->n_sm * 8));
-    TimedScope ts(h, st, 3);
     if (cc.n_tiles > 0) {
+        const int grid = std::max(1, std::min(cc.n_tiles, h->n_sm * 8));
+        TimedScope ts(h, st, 3);
         if (convert)
             csr_max_kernel<true><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
         else
             csr_max_kernel<false><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
-        csr_count_kernel<<<grid, kBlock, 0, st>>>(cc, data, h->inf_colmax.as<unsigned int>(), rel_thr, h->inf_tilecnt.as<unsigned int>());
-        h->launches += 2;
+        CU(h, cudaGetLastError());
+        h->launches += 1;
+    }
+    return VPMC_OK;
+}
+
+// writer passes 2 + 3: kept entries per tile, exclusive scan per column; leaves per-column counts in inf_colnnz (device)
+static int csr_count_pass(vpmc_t *h, const CsrCols &cc, const float *data, float rel_thr, cudaStream_t st)
+{
+    int rc = ensure(h, h->inf_tilecnt, (size_t)std::max(cc.n_tiles, 1) * sizeof(unsigned int)); if (rc) return rc;
+    rc = ensure(h, h->inf_colnnz, (size_t)cc.n_cols * sizeof(long long)); if (rc) return rc;
+    TimedScope ts(h, st, 3);
+    if (cc.n_tiles > 0) {
+        csr_count_kernel<<<std::max(1, std::min(cc.n_tiles, h->n_sm * 8)), kBlock, 0, st>>>(cc, data, h->inf_colmax.as<unsigned int>(), rel_thr, h->inf_tilecnt.as<unsigned int>());
+        h->launches += 1;
     }
     csr_tile_scan_kernel<<<cc.n_cols, kBlock, 0, st>>>(cc, h->inf_tilecnt.as<unsigned int>(), h->inf_colnnz.as<long long>());
     CU(h, cudaGetLastError());
@@ -81,7 +95,8 @@ extern "C" int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, f
     CsrCols cc{};
     cc.lo = h->inf_lo.as<int4>(); cc.dim = h->inf_dim.as<int4>(); cc.offset = h->inf_off.as<unsigned long long>();
     cc.tile0 = h->inf_tile0.as<int>(); cc.skip = nullptr; cc.n_cols = 1; cc.n_tiles = tile0[1]; cc.nx = (int)n; cc.ny = 1;
-    rc = csr_count_passes(h, cc, const_cast<float *>(col_dev), false, 1.0f, rel_threshold, st); if (rc) return rc;
+    rc = csr_max_pass(h, cc, const_cast<float *>(col_dev), false, 1.0f, st); if (rc) return rc;
+    rc = csr_count_pass(h, cc, col_dev, rel_threshold, st); if (rc) return rc;
     long long nnz = 0;
     CU(h, cudaMemcpy(&nnz, h->inf_colnnz.p, sizeof(long long), cudaMemcpyDeviceToHost));
     *nnz_out = nnz;
@@ -138,6 +153,8 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef = (float)(1.0 / (double)hist_per_spot / V * 1.602176634e-10);          // C6: scale 1 / hist_per_spot
     const uint32_t n_pilot = std::min<uint32_t>(hist_per_spot, std::max<uint32_t>(32u, hist_per_spot / 32u));
+    unsigned int ovf_cap = 1u << 25;          // entries of the overflow list (12 B each); VPMC_OVF_CAP overrides (0 forces replays)
+    if (const char *e = getenv("VPMC_OVF_CAP")) ovf_cap = (unsigned int)std::min<long long>(std::max<long long>(atoll(e), 0), 1ll << 28);
 
     for (int s = 0; s < n_sc; ++s) {
         const vpmc_scenario sc = scs[s];
@@ -167,8 +184,9 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
             else box[g] = grown_box(&bb[6 * g], h->G);
         }
         // ---- 3./4. groups, with replay of the columns that outgrew their box
-        std::vector<long long> row_nnz(ns, 0), row_src(ns, 0);
-        long long staged = 0;
+        std::vector<long long> row_nnz(ns, 0), row_src(ns, 0), row_ovf_off(ns, 0);
+        std::vector<int> row_ovf_n(ns, 0);
+        long long staged = 0, ostaged = 0;
         std::vector<int> todo(ns);
         std::iota(todo.begin(), todo.end(), 0);
         bool replay = false;
@@ -201,6 +219,12 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 ColumnBoxes cb{};
                 cb.lo = h->inf_lo.as<int4>(); cb.dim = h->inf_dim.as<int4>(); cb.offset = h->inf_off.as<unsigned long long>();
                 cb.scratch = h->inf_scratch.as<float>(); cb.bbox = h->inf_bbox.as<int>();
+                // overflow list: deposits outside the boxes (ovf_ctr: [0] entries appended, [1] unique entries, [2] kept entries)
+                if ((rc = ensure(h, h->ovf_key, (size_t)ovf_cap * 8 + 8)) || (rc = ensure(h, h->ovf_val, (size_t)ovf_cap * 4 + 4)) ||
+                    (rc = ensure(h, h->ovf_ctr, 4 * sizeof(int)))) return rc;
+                CU(h, cudaMemsetAsync(h->ovf_ctr.p, 0, 4 * sizeof(int), st));
+                cb.ovf_key = h->ovf_key.as<unsigned long long>(); cb.ovf_val = h->ovf_val.as<float>();
+                cb.ovf_count = h->ovf_ctr.as<unsigned int>(); cb.ovf_cap = ovf_cap;
                 {
                     WorkMap wm{};
                     wm.mode = 1; wm.hps = hist_per_spot; wm.n_sub = hist_per_spot; wm.cols = h->inf_cols.as<int>(); wm.g0 = 0;
@@ -210,9 +234,12 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     if (replay) CU(h, cudaMemsetAsync(h->d_tal_scratch, 0, sizeof(DevTallies), st));
                     rc = launch_transport<1>(h, ctx, wm, sa, replay ? h->d_tal_scratch : h->d_tal, st); if (rc) return rc;
                 }
-                // which columns outgrew their box
+                // which columns lost outside deposits (overflow list full): those are replayed with a larger box
+                unsigned int n_ovf = 0;
                 CU(h, cudaMemcpyAsync(obb.data(), h->inf_bbox.p, obb.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
+                CU(h, cudaMemcpyAsync(&n_ovf, h->ovf_ctr.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
                 CU(h, cudaStreamSynchronize(st));
+                n_ovf = std::min(n_ovf, ovf_cap);
                 std::vector<int> skip(nc, 0);
                 for (int c = 0; c < nc; ++c)
                     if (obb[6 * c + 3] >= 0) {
@@ -227,12 +254,60 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 CsrCols cc{};
                 cc.lo = cb.lo; cc.dim = cb.dim; cc.offset = cb.offset; cc.tile0 = h->inf_tile0.as<int>(); cc.skip = h->inf_skip.as<int>();
                 cc.n_cols = nc; cc.n_tiles = tile0.back(); cc.nx = h->G.nx; cc.ny = h->G.ny;
-                rc = csr_count_passes(h, cc, cb.scratch, true, coef, rel_threshold, st); if (rc) return rc;
+                rc = csr_max_pass(h, cc, cb.scratch, true, coef, st); if (rc) return rc;
+                std::vector<unsigned int> ocnt(nc, 0u);
+                int n_sel = 0;
+                if (n_ovf > 0) {
+                    // sort by (column, voxel), sum duplicates, convert, threshold against the column maximum, compact
+                    if ((rc = ensure(h, h->ovf_key2, (size_t)n_ovf * 8)) || (rc = ensure(h, h->ovf_val2, (size_t)n_ovf * 4)) ||
+                        (rc = ensure(h, h->ovf_flag, (size_t)n_ovf)) || (rc = ensure(h, h->ovf_colcnt, (size_t)nc * 4))) return rc;
+                    unsigned long long *k1 = h->ovf_key.as<unsigned long long>(), *k2 = h->ovf_key2.as<unsigned long long>();
+                    float *v1 = h->ovf_val.as<float>(), *v2 = h->ovf_val2.as<float>();
+                    int *ctr = h->ovf_ctr.as<int>();
+                    size_t t1 = 0, t2 = 0, t3 = 0;
+                    cub::DeviceRadixSort::SortPairs(nullptr, t1, k1, k2, v1, v2, (int)n_ovf, 0, 56, st);
+                    cub::DeviceReduce::ReduceByKey(nullptr, t2, k2, k1, v2, v1, ctr + 1, cub::Sum(), (int)n_ovf, st);
+                    cub::DeviceSelect::Flagged(nullptr, t3, k1, h->ovf_flag.as<unsigned char>(), k2, ctr + 2, (int)n_ovf, st);
+                    size_t tb = std::max(t1, std::max(t2, t3));
+                    rc = ensure(h, h->cub_temp, tb); if (rc) return rc;
+                    TimedScope ts(h, st, 3);
+                    CU(h, cub::DeviceRadixSort::SortPairs(h->cub_temp.p, tb, k1, k2, v1, v2, (int)n_ovf, 0, 56, st));
+                    CU(h, cub::DeviceReduce::ReduceByKey(h->cub_temp.p, tb, k2, k1, v2, v1, ctr + 1, cub::Sum(), (int)n_ovf, st));
+                    const int g1 = std::max(1, std::min((int)((n_ovf + 255) / 256), h->n_sm * 8));
+                    ovf_convert_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
+                    CU(h, cudaMemsetAsync(h->ovf_colcnt.p, 0, (size_t)nc * 4, st));
+                    CU(h, cudaMemsetAsync(h->ovf_flag.p, 0, (size_t)n_ovf, st));
+                    ovf_flag_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->inf_colmax.as<unsigned int>(), h->inf_skip.as<int>(), rel_threshold,
+                                                       h->ovf_flag.as<unsigned char>(), h->ovf_colcnt.as<unsigned int>());
+                    CU(h, cub::DeviceSelect::Flagged(h->cub_temp.p, tb, k1, h->ovf_flag.as<unsigned char>(), k2, ctr + 2, (int)n_ovf, st));
+                    CU(h, cub::DeviceSelect::Flagged(h->cub_temp.p, tb, v1, h->ovf_flag.as<unsigned char>(), v2, ctr + 3, (int)n_ovf, st));
+                    CU(h, cudaGetLastError());
+                    h->launches += 8;
+                    CU(h, cudaMemcpyAsync(ocnt.data(), h->ovf_colcnt.p, (size_t)nc * 4, cudaMemcpyDeviceToHost, st));
+                    CU(h, cudaMemcpyAsync(&n_sel, ctr + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
+                }
+                rc = csr_count_pass(h, cc, cb.scratch, rel_threshold, st); if (rc) return rc;
                 std::vector<long long> nnz(nc), base(nc);
                 CU(h, cudaMemcpyAsync(nnz.data(), h->inf_colnnz.p, (size_t)nc * sizeof(long long), cudaMemcpyDeviceToHost, st));
                 CU(h, cudaStreamSynchronize(st));
-                long long add = 0;
-                for (int c = 0; c < nc; ++c) { base[c] = staged + add; if (!skip[c]) { row_nnz[cols[c]] = nnz[c]; row_src[cols[c]] = base[c]; add += nnz[c]; } }
+                long long add = 0, oadd = 0;
+                for (int c = 0; c < nc; ++c) {
+                    base[c] = staged + add;
+                    if (!skip[c]) {
+                        row_nnz[cols[c]] = nnz[c] + ocnt[c]; row_src[cols[c]] = base[c]; add += nnz[c];
+                        row_ovf_off[cols[c]] = ostaged + oadd; row_ovf_n[cols[c]] = (int)ocnt[c]; oadd += ocnt[c];
+                    }
+                }
+                if (oadd != n_sel) FAIL(h, VPMC_ERR_STATE, "influence: overflow bookkeeping mismatch (%lld vs %d)", oadd, n_sel);
+                if (oadd > 0) {       // the kept overflow entries, sorted by (column, voxel), join the persistent overflow staging
+                    if ((rc = grow_keep(h, h->ostage_idx, (size_t)(ostaged + oadd) * sizeof(int), (size_t)ostaged * sizeof(int), st)) ||
+                        (rc = grow_keep(h, h->ostage_val, (size_t)(ostaged + oadd) * sizeof(float), (size_t)ostaged * sizeof(float), st))) return rc;
+                    ovf_split_keys_kernel<<<std::max(1, std::min((int)((oadd + 255) / 256), h->n_sm * 8)), 256, 0, st>>>(h->ovf_key2.as<unsigned long long>(), (int)oadd, h->ostage_idx.as<int>() + ostaged);
+                    CU(h, cudaMemcpyAsync(h->ostage_val.as<float>() + ostaged, h->ovf_val2.p, (size_t)oadd * sizeof(float), cudaMemcpyDeviceToDevice, st));
+                    h->launches += 1;
+                    ostaged += oadd;
+                }
+                if (getenv("VPMC_DEBUG")) fprintf(stderr, "[vpmc]   group of %d columns: %u outside deposits, %lld kept entries of them, %lld box entries\n", nc, n_ovf, oadd, add);
                 if (add > 0) {
                     if ((rc = grow_keep(h, h->inf_stage_idx, (size_t)(staged + add) * sizeof(int), (size_t)staged * sizeof(int), st)) ||
                         (rc = grow_keep(h, h->inf_stage_val, (size_t)(staged + add) * sizeof(float), (size_t)staged * sizeof(float), st)) ||
@@ -261,11 +336,12 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         o.val = (float *)alloc((size_t)std::max<long long>(nnz, 1) * sizeof(float), user);
         if (!o.row_ptr || !o.col || !o.val) FAIL(h, VPMC_ERR_ALLOC, "the caller's allocator returned NULL (scenario %d, nnz %lld)", s, nnz);
         CU(h, cudaMemcpyAsync(o.row_ptr, row_ptr.data(), (size_t)(ns + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
-        rc = upload(h, h->inf_rowsrc, row_src, st); if (rc) return rc;
+        if ((rc = upload(h, h->inf_rowsrc, row_src, st)) || (rc = upload(h, h->row_ovf_off, row_ovf_off, st)) || (rc = upload(h, h->row_ovf_n, row_ovf_n, st))) return rc;
         if (nnz > 0) {
             TimedScope ts(h, st, 3);
-            csr_gather_rows_kernel<<<std::min(ns, h->n_sm * 8), 256, 0, st>>>(ns, h->inf_rowsrc.as<long long>(), (const long long *)o.row_ptr,
-                                                                             h->inf_stage_idx.as<int>(), h->inf_stage_val.as<float>(), o.col, o.val);
+            csr_gather_rows_kernel<<<std::min(ns, h->n_sm * 8), 256, 0, st>>>(ns, h->inf_rowsrc.as<long long>(), h->row_ovf_off.as<long long>(), h->row_ovf_n.as<int>(),
+                                                                             (const long long *)o.row_ptr, h->inf_stage_idx.as<int>(), h->inf_stage_val.as<float>(),
+                                                                             h->ostage_idx.as<int>(), h->ostage_val.as<float>(), o.col, o.val);
             CU(h, cudaGetLastError());
             h->launches += 1;
         }

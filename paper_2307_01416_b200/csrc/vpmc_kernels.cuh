@@ -31,7 +31,13 @@ struct ColumnBoxes {
     const int4 *dim;         // [n_cols] box extent (bx, by, bz, 0)
     const unsigned long long *offset;   // [n_cols] offset of the box in `scratch`
     float *scratch;          // concatenated boxes (MeV)
-    int *bbox;               // [n_cols][6] min x,y,z, max x,y,z of deposits OUTSIDE the box (MODE 1) / of all (MODE 2)
+    int *bbox;               // [n_cols][6] MODE 2: bounding box of all deposits; MODE 1: of the outside deposits that did
+                             // NOT fit the overflow list (such a column is replayed with a larger box)
+    // MODE 1: deposits outside the box go to a list of (column << 32 | voxel, MeV) entries, merged into the rows later
+    unsigned long long *ovf_key;
+    float *ovf_val;
+    unsigned int *ovf_count;
+    unsigned int ovf_cap;
 };
 
 __device__ __forceinline__ unsigned lanemask_lt()
@@ -87,8 +93,11 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
         const int bx = (int)h.g0 - lo.x, by = (int)h.g1 - lo.y, bz = (int)h.g2 - lo.z;
         if ((unsigned)bx < (unsigned)dm.x && (unsigned)by < (unsigned)dm.y && (unsigned)bz < (unsigned)dm.z)
             atomicAdd(cb.scratch + __ldg(cb.offset + c) + (bx + (unsigned long long)dm.x * (by + (unsigned long long)dm.y * bz)), dep);
-        else
-            bbox_merge(cb.bbox + 6 * c, (int)h.g0, (int)h.g1, (int)h.g2, (int)h.g0, (int)h.g1, (int)h.g2);
+        else {
+            const unsigned slot = atomicAdd(cb.ovf_count, 1u);
+            if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | h.g3; cb.ovf_val[slot] = dep; }
+            else bbox_merge(cb.bbox + 6 * c, (int)h.g0, (int)h.g1, (int)h.g2, (int)h.g0, (int)h.g1, (int)h.g2);
+        }
     }
     __device__ __forceinline__ void end(const Hist &) {}
 };
@@ -649,14 +658,71 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
     }
 }
 
-// final assembly: row r of the staging area -> its place in the scenario's CSR arrays
-__global__ void csr_gather_rows_kernel(int n_rows, const long long *__restrict__ src_off, const long long *__restrict__ row_ptr,
+// ---- overflow list (deposits outside a column's box), after sort + reduce-by-key: unique (column << 32 | voxel, MeV)
+// E_dep -> dose value, in place; the column maximum takes these entries into account
+__global__ void ovf_convert_kernel(const unsigned long long *__restrict__ key, float *__restrict__ val, const int *__restrict__ n_ptr,
+                                   const short *__restrict__ hu, const float4 *__restrict__ lut, int hu_min, int n_lut,
+                                   float rho_min, float coef, unsigned int *__restrict__ colmax_bits)
+{
+    const int n = *n_ptr;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const unsigned long long k = key[i];
+        int t = (int)__ldg(hu + (unsigned)k) - hu_min;
+        t = min(max(t, 0), n_lut - 1);
+        const float x = __fdiv_rn(coef * val[i], fmaxf(__ldg(lut + t).y, rho_min));
+        val[i] = x;
+        if (x > 0.0f) atomicMax(colmax_bits + (unsigned)(k >> 32), __float_as_uint(x));
+    }
+}
+
+// keep flags of the unique overflow entries and kept entries per column
+__global__ void ovf_flag_kernel(const unsigned long long *__restrict__ key, const float *__restrict__ val, const int *__restrict__ n_ptr,
+                                const unsigned int *__restrict__ colmax_bits, const int *__restrict__ skip, float rel_thr,
+                                unsigned char *__restrict__ flag, unsigned int *__restrict__ col_cnt)
+{
+    const int n = *n_ptr;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const unsigned c = (unsigned)(key[i] >> 32);
+        const bool keep = !__ldg(skip + c) && csr_keep(val[i], rel_thr * __uint_as_float(__ldg(colmax_bits + c)));
+        flag[i] = keep ? 1 : 0;
+        if (keep) atomicAdd(col_cnt + c, 1u);
+    }
+}
+
+__global__ void ovf_split_keys_kernel(const unsigned long long *__restrict__ key, int n, int *__restrict__ vox)
+{
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) vox[i] = (int)(unsigned)key[i];
+}
+
+// final assembly: row r = merge of its staged box entries (a) and its kept overflow entries (b), both ascending in voxel
+// index and disjoint, into the scenario's CSR arrays.  Position of an element = its rank in its own list + the number of
+// elements of the other list below it (binary search).
+__global__ void csr_gather_rows_kernel(int n_rows, const long long *__restrict__ src_off, const long long *__restrict__ ovf_off,
+                                       const int *__restrict__ ovf_n, const long long *__restrict__ row_ptr,
                                        const int *__restrict__ s_idx, const float *__restrict__ s_val,
+                                       const int *__restrict__ o_idx, const float *__restrict__ o_val,
                                        int *__restrict__ idx, float *__restrict__ val)
 {
     for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
-        const long long a = __ldg(row_ptr + r), n = __ldg(row_ptr + r + 1) - a, s = __ldg(src_off + r);
-        for (long long i = threadIdx.x; i < n; i += blockDim.x) { idx[a + i] = s_idx[s + i]; val[a + i] = s_val[s + i]; }
+        const long long dst = __ldg(row_ptr + r), n = __ldg(row_ptr + r + 1) - dst, sa = __ldg(src_off + r);
+        const int nb = __ldg(ovf_n + r);
+        const long long na = n - nb, sb = __ldg(ovf_off + r);
+        if (nb == 0) {
+            for (long long i = threadIdx.x; i < na; i += blockDim.x) { idx[dst + i] = s_idx[sa + i]; val[dst + i] = s_val[sa + i]; }
+            continue;
+        }
+        for (long long i = threadIdx.x; i < na; i += blockDim.x) {
+            const int v = s_idx[sa + i];
+            int lo = 0, hi = nb;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (o_idx[sb + mid] < v) lo = mid + 1; else hi = mid; }
+            idx[dst + i + lo] = v; val[dst + i + lo] = s_val[sa + i];
+        }
+        for (int j = threadIdx.x; j < nb; j += blockDim.x) {
+            const int v = o_idx[sb + j];
+            long long lo = 0, hi = na;
+            while (lo < hi) { const long long mid = (lo + hi) >> 1; if (s_idx[sa + mid] < v) lo = mid + 1; else hi = mid; }
+            idx[dst + j + lo] = v; val[dst + j + lo] = o_val[sb + j];
+        }
     }
 }
 

@@ -144,7 +144,8 @@ def test_influence_parity(bind, case):
 
 
 def test_influence_groups_and_replay_give_the_same_matrix(bind):
-    """Small workspace -> several groups; zero box margin -> the replay path; both must reproduce the default run."""
+    """Small workspace -> several groups; zero box margin -> the overflow list, or without it the replay path; all must
+    reproduce the default run."""
     w = hetero_case()
     hps, thr, seed = 3000, 1e-4, 3
     sc = [bind.scenario((0, 0, 0), 1.0)]
@@ -157,12 +158,16 @@ def test_influence_groups_and_replay_give_the_same_matrix(bind):
     os.environ["VPMC_BOX_GROW"] = "0"; os.environ["VPMC_BOX_PAD"] = "0"
     try:
         eng.set_workspace_limit(0)
+        overflow = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]      # tight boxes: the overflow list fills the rows
+        n2 = eng.launch_count()
+        os.environ["VPMC_OVF_CAP"] = "0"                                                # no list: the replay path
         replay = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]
     finally:
         del os.environ["VPMC_BOX_GROW"], os.environ["VPMC_BOX_PAD"]
-    n2 = eng.launch_count()
-    assert n1 - n0 > n0 and n2 - n1 > n0 / 2           # more groups / extra rounds really ran
-    for other in (small, replay):
+        os.environ.pop("VPMC_OVF_CAP", None)
+    n3 = eng.launch_count()
+    assert n1 - n0 > n0 and n3 - n2 > n0 + 3           # more groups / an extra round really ran
+    for other in (small, overflow, replay):
         only = compare_rows(other, base, eng.nvox, thr)[0]
         assert only <= 0.02 * base[1].size
         check_csr_structure(*other, eng.n_spots, eng.nvox)
