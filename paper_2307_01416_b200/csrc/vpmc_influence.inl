@@ -39,7 +39,7 @@ static int grow_keep(vpmc_t *h, DevBuf &b, size_t bytes, size_t keep, cudaStream
     if (cudaMalloc(&np, want) != cudaSuccess) { cudaGetLastError(); FAIL(h, VPMC_ERR_ALLOC, "out of device memory (%zu bytes of CSR staging)", want); }
     if (b.p && keep) CU(h, cudaMemcpyAsync(np, b.p, keep, cudaMemcpyDeviceToDevice, st));
     CU(h, cudaStreamSynchronize(st));
-    if (b.p) cudaFree(b.p);
+    if (b.p) pool_give(b.p, b.bytes);       // the stream was synchronised just above
     b.p = np; b.bytes = want;
     return VPMC_OK;
 }

@@ -239,14 +239,15 @@ extern "C" int vpmc_dose_host(vpmc_t *h, uint64_t n_histories, uint64_t seed, fl
 {
     if (!h) return VPMC_ERR_INVALID_ARG;
     if (!dose_out_host) FAIL(h, VPMC_ERR_INVALID_ARG, "NULL argument");
-    float *d = nullptr;
-    CU(h, cudaMalloc(&d, h->nvox * sizeof(float)));
-    int rc = vpmc_dose(h, n_histories, seed, d, nullptr);
+    DevBuf tmp;
+    int rc = ensure(h, tmp, h->nvox * sizeof(float)); if (rc) return rc;
+    float *d = tmp.as<float>();
+    rc = vpmc_dose(h, n_histories, seed, d, nullptr);
     if (rc == VPMC_OK) {
         cudaError_t e = cudaMemcpy(dose_out_host, d, h->nvox * sizeof(float), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { h->err = cudaGetErrorString(e); rc = VPMC_ERR_CUDA; }
     }
-    cudaFree(d);
+    pool_give(tmp.p, tmp.bytes);
     return rc;
 }
 

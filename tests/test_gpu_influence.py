@@ -150,23 +150,26 @@ def test_influence_groups_and_replay_give_the_same_matrix(bind):
     hps, thr, seed = 3000, 1e-4, 3
     sc = [bind.scenario((0, 0, 0), 1.0)]
     eng = bind.Engine(w)
-    base = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]
-    n0 = eng.launch_count()
-    eng.set_workspace_limit(64 * 1024)                 # a few columns' worth at most
-    small = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]
-    n1 = eng.launch_count()
+    eng.set_timing(True)
+
+    def run():
+        eng.timing()
+        m = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]
+        return m, eng.timing()["voxel"][1]              # passes of the pipeline: pilot + groups (+ replays)
+
+    base, p_base = run()
+    eng.set_workspace_limit(4 * 1024)                   # 1024 box elements: one column per group
+    small, p_small = run()
     os.environ["VPMC_BOX_GROW"] = "0"; os.environ["VPMC_BOX_PAD"] = "0"
     try:
         eng.set_workspace_limit(0)
-        overflow = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]      # tight boxes: the overflow list fills the rows
-        n2 = eng.launch_count()
-        os.environ["VPMC_OVF_CAP"] = "0"                                                # no list: the replay path
-        replay = [x.cpu().numpy() for x in eng.influence(sc, hps, thr, seed)[0]]
+        overflow, p_ovf = run()                         # tight boxes: the overflow list fills the rows
+        os.environ["VPMC_OVF_CAP"] = "0"                # no list: the replay path
+        replay, p_replay = run()
     finally:
         del os.environ["VPMC_BOX_GROW"], os.environ["VPMC_BOX_PAD"]
         os.environ.pop("VPMC_OVF_CAP", None)
-    n3 = eng.launch_count()
-    assert n1 - n0 > n0 and n3 - n2 > n0 + 3           # more groups / an extra round really ran
+    assert p_base == 2 and p_small == 1 + eng.n_spots and p_ovf == 2 and p_replay == 3, (p_base, p_small, p_ovf, p_replay)
     for other in (small, overflow, replay):
         only = compare_rows(other, base, eng.nvox, thr)[0]
         assert only <= 0.02 * base[1].size
