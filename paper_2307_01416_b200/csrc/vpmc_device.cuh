@@ -106,16 +106,18 @@ __device__ __forceinline__ void pair_axpy(uint32_t &ghi, uint32_t &glo, float s,
 struct StepOut { float s, dep, removed, theta, uphi; int on_d; };
 
 // ---------------------------------------------------------------------------------------------- C1
-__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               uint32_t k0, uint32_t k1)
+// the ten round keys (k + r * Weyl increment) are the same for every thread: they are computed once on the host and
+// sit in the kernel's constant bank, so a round is two wide multiplies and two three-input XORs
+struct PhiloxKey { uint32_t k0[10], k1[10]; };
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKey &K)
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
         const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        const uint32_t n0 = hi1 ^ c1 ^ K.k0[r], n2 = hi0 ^ c3 ^ K.k1[r];
         c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     return make_uint4(c0, c1, c2, c3);
 }
@@ -127,9 +129,9 @@ __device__ __forceinline__ float u01(uint32_t x)
     return __uint_as_float(0x3f800000u | (x >> 9)) - 0.99999994039535522461f;
 }
 
-__device__ __forceinline__ float4 draw4(const Hist &h, uint32_t step, uint32_t purpose, uint32_t k0, uint32_t k1)
+__device__ __forceinline__ float4 draw4(const Hist &h, uint32_t step, uint32_t purpose, const PhiloxKey &K)
 {
-    const uint4 o = philox4x32_10(h.hid_lo, h.hid_hi, step, purpose, k0, k1);
+    const uint4 o = philox4x32_10(h.hid_lo, h.hid_hi, step, purpose, K);
     return make_float4(u01(o.x), u01(o.y), u01(o.z), u01(o.w));
 }
 
@@ -182,7 +184,7 @@ __device__ __forceinline__ float highland_dA(float t, float dt, float c_log, flo
 // amplifies (dE/dR ~ 10 MeV/mm).  Here R is carried in fp64 and updated by differences:
 // R' = R - s rsp, and, after straggling, R_next = alpha E'^p = R' (E'/Ebar')^p = R' + R' ((1 + delta)^p - 1).
 __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const Medium &m, float d,
-                                            uint32_t k0, uint32_t k1, StepOut &o)
+                                            const PhiloxKey &K, StepOut &o)
 {
     o.removed = 0.0f; o.on_d = 0; o.theta = 0.0f; o.uphi = 0.5f;
     const float E = h.E;
@@ -205,7 +207,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     const float y = P.inv_p * Lm;
     const float dEm = (x < 0.03f) ? Ebar * (y * fmaf(y, fmaf(y, fmaf(y, 1.0f / 24.0f, 1.0f / 6.0f), 0.5f), 1.0f)) : E - Ebar;
     // 3
-    const float4 u = draw4(h, h.step, 0u, k0, k1);
+    const float4 u = draw4(h, h.step, 0u, K);
     // 4
     float Ep = Ebar, dep = dEm;
     double Rn = Rp;

@@ -18,7 +18,7 @@ struct BeamHost {
     int ap_nx = 0, ap_ny = 0, ap_row_words = 0;
     float ap_u0 = 0, ap_v0 = 0, ap_du = 1, ap_dv = 1;
     uint32_t *d_bits = nullptr;       // packed opening bitmap on the device
-    unsigned char *d_dist = nullptr;  // safe-distance maps of the opening (tiles of 8 x 8 pixels): to brass, then to the opening
+    unsigned char *d_dist = nullptr;  // safe-distance maps of the opening, one byte per tile of 2^kApTileShift pixels: to brass, then to the opening
     int ap_ntx = 0, ap_nty = 0;
 };
 

@@ -1,9 +1,10 @@
 // vpmc_kernels.cuh -- the sm_100a kernels of the hot path.  See DESIGN.md 5:
-//   beam_kernel       S1-S3: persistent warps carry histories through source, range shifter and aperture; lanes whose
-//                     history ended or left the beam line are refilled from a global item counter (warp-aggregated);
-//                     survivors are pushed to a queue
-//   voxel_kernel      S4-S7: persistent warps pull survivors from the queue, take the CT entry, step through the voxels
-//                     and score; MODE 0 the dose grid(s), MODE 1 per-column boxes, MODE 2 only column bounding boxes
+//   source_kernel     S1: one thread per work item -> source record
+//   beam_kernel       S2-S3: persistent warps carry histories through range shifter and aperture; free lanes load the
+//                     next source record (warp-aggregated claim); survivors are pushed to a queue
+//   entry_kernel      CT entry (fp64), one thread per survivor
+//   voxel_kernel      S4-S7: persistent warps pull survivors from the queue, step through the voxels and score;
+//                     MODE 0 the dose grid(s), MODE 1 per-column boxes + overflow list, MODE 2 only column bounding boxes
 //   dose_finalize / uncertainty kernels: S6 dose conversion and the C6 batch estimator
 //   csr_* kernels     S8: threshold + count + scan + emit of the per-spot sparse columns
 #pragma once
@@ -83,7 +84,7 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
     atomicMax(bb + 3, x1); atomicMax(bb + 4, y1); atomicMax(bb + 5, z1);
 }
 
-struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it only grows the column's overflow bbox
+struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
     ColumnBoxes cb;
     __device__ __forceinline__ void begin(const Hist &) {}
     __device__ __forceinline__ void deposit(const Hist &h, float dep)
@@ -193,7 +194,7 @@ source_kernel(const Ctx c, const WorkMap wm, const unsigned long long item0, con
         map_item(wm, item0 + k, g, hid, h.col);
         h.hid_lo = (uint32_t)hid; h.hid_hi = (uint32_t)(hid >> 32);
         const int beam = __ldg(spot_beam + g);
-        sample_source(c.P, c.beams[beam], beam, __ldg(spots + g), __ldg(spot_R0 + g), h, c.k0, c.k1);
+        sample_source(c.P, c.beams[beam], beam, __ldg(spots + g), __ldg(spot_R0 + g), h, c.K);
         inc = (double)h.E;
         const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
         sb.s0[k] = make_uint4(h.g0, h.g1, h.g2, h.g3);
@@ -417,7 +418,7 @@ __global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__
     h.col = 0;
     h.hid_lo = (uint32_t)hids[i]; h.hid_hi = (uint32_t)(hids[i] >> 32);
     const int beam = spot_beam[g];
-    sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.k0, c.k1);
+    sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.K);
     int code = BEAM_CONT;
     float dep_rs = 0.0f, dep_ap = 0.0f;
     for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, lc, tr);

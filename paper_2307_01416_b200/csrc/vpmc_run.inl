@@ -106,7 +106,7 @@ static Ctx make_ctx(const vpmc_t *h, const vpmc_scenario &sc, uint64_t seed)
     c.P = h->P; c.G = h->G; c.beams = h->d_beams; c.hu = h->d_hu;
     c.rsp_scale = sc.rsp_scale; c.inv_rsp_scale = (float)(1.0 / (double)sc.rsp_scale);
     c.shift[0] = sc.shift[0]; c.shift[1] = sc.shift[1]; c.shift[2] = sc.shift[2];
-    c.k0 = (uint32_t)seed; c.k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { c.K.k0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; c.K.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u; }
     return c;
 }
 

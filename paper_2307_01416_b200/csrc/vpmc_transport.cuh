@@ -72,15 +72,15 @@ struct Ctx {
     const short *hu;
     float rsp_scale, inv_rsp_scale;
     float shift[3];
-    uint32_t k0, k1;
+    PhiloxKey K;
 };
 
 // S1 (C2): sample position, energy and nuclear threshold of history h (hid already set) from spot sp.
 // R0 = alpha E_spot^p in fp64 from the host; recomputed on the device only when the source has an energy spread.
 __device__ __forceinline__ void sample_source(const DevParams &P, const DevBeam &b, int beam, const float4 sp /*x,y,E,sigma*/,
-                                              double R0, Hist &h, uint32_t k0, uint32_t k1)
+                                              double R0, Hist &h, const PhiloxKey &K)
 {
-    const float4 a = draw4(h, 0u, 1u, k0, k1);
+    const float4 a = draw4(h, 0u, 1u, K);
     const float rho = sqrtf(-2.0f * logf(a.x));
     float sn, cs;
     sincospif(2.0f * a.y, &sn, &cs);
@@ -95,7 +95,7 @@ __device__ __forceinline__ void sample_source(const DevParams &P, const DevBeam 
         R0 = fma(R0, (double)expm1f(P.p * log1pf(dl)), R0);      // alpha (E (1 + dl))^p = R0 (1 + dl)^p
     }
     h.E = E0; h.R = R0;
-    const float4 c = draw4(h, 0u, 2u, k0, k1);
+    const float4 c = draw4(h, 0u, 2u, K);
     h.tau_star = -logf(c.x);
     h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
     h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
@@ -209,17 +209,15 @@ __device__ __forceinline__ float face_distance(const DevGrid &G, const Hist &h, 
 // on that axis BEFORE the scattering of this step.  Returns true if the history left the grid.
 __device__ __forceinline__ bool cross_face(const DevGrid &G, Hist &h, int ax, bool up)
 {
-    if (ax == 0) {
-        if (up) { h.g0 += 1u; h.g3 += 1u; h.rx = 0.0f; } else { h.g0 -= 1u; h.g3 -= 1u; h.rx = G.hx; }
-        return h.g0 >= (uint32_t)G.nx;
-    } else if (ax == 1) {
-        if (up) { h.g1 += 1u; h.g3 += (uint32_t)G.nx; h.ry = 0.0f; } else { h.g1 -= 1u; h.g3 -= (uint32_t)G.nx; h.ry = G.hy; }
-        return h.g1 >= (uint32_t)G.ny;
-    } else {
-        const uint32_t nxy = (uint32_t)(G.nx * G.ny);
-        if (up) { h.g2 += 1u; h.g3 += nxy; h.rz = 0.0f; } else { h.g2 -= 1u; h.g3 -= nxy; h.rz = G.hz; }
-        return h.g2 >= (uint32_t)G.nz;
-    }
+    // selects instead of a three-way branch: the lanes of a warp cross different faces
+    const uint32_t stride = ax == 0 ? 1u : (ax == 1 ? (uint32_t)G.nx : (uint32_t)(G.nx * G.ny));
+    const uint32_t n = ax == 0 ? (uint32_t)G.nx : (ax == 1 ? (uint32_t)G.ny : (uint32_t)G.nz);
+    const float snap = up ? 0.0f : (ax == 0 ? G.hx : (ax == 1 ? G.hy : G.hz));
+    const uint32_t idx = (ax == 0 ? h.g0 : (ax == 1 ? h.g1 : h.g2)) + (up ? 1u : 0xffffffffu);
+    h.g3 += up ? stride : 0u - stride;
+    h.g0 = ax == 0 ? idx : h.g0; h.g1 = ax == 1 ? idx : h.g1; h.g2 = ax == 2 ? idx : h.g2;
+    h.rx = ax == 0 ? snap : h.rx; h.ry = ax == 1 ? snap : h.ry; h.rz = ax == 2 ? snap : h.rz;
+    return idx >= n;
 }
 
 // per-thread counters that live for the whole kernel (flushed once at its end)
@@ -363,7 +361,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
         StepOut o;
         const float Eb = h.E; const uint32_t st = h.step;
         const float lat = fmaxf(fabsf(h.ux), fabsf(h.uy));        // direction of travel during the step
-        const int cause = step_physics(P, h, m, d, c.k0, c.k1, o);
+        const int cause = step_physics(P, h, m, d, c.K, o);
         h.rx = fmaf(-o.s, lat, h.rx);                              // brass budget (meaningless, and unused, in the range shifter)
         if (cause == CONT) {
             // C4-8: move along the OLD direction, then rotate
@@ -436,7 +434,7 @@ __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, fl
     const Medium m = { mv.x * c.rsp_scale, mv.w * c.inv_rsp_scale, mv.y, mv.z, P.za_w * mv.y };
     StepOut o;
     const float Eb = h.E; const uint32_t st = h.step;
-    int cause = step_physics(P, h, m, d, c.k0, c.k1, o);
+    int cause = step_physics(P, h, m, d, c.K, o);
     if (cause == CONT) {
         // C4-8: move along the OLD direction, then rotate
         h.rx = fmaf(o.s, h.lx, fmaf(o.s, h.ux, h.rx));
