@@ -301,7 +301,8 @@ def run_b200(args):
             e.close()
         return h2d, d2h
 
-    e2e_step()
+    for _ in range(2):                                   # warm-up: allocator cache, page-locked staging
+        e2e_step()
     dist.barrier(world)
     torch.cuda.synchronize()
     t0 = time.perf_counter()

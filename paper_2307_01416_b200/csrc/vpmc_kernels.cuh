@@ -139,7 +139,7 @@ template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreAr
 constexpr int kBlock = 256;
 constexpr int kWarps = kBlock / 32;
 #ifndef VPK_REFILL_MIN
-#define VPK_REFILL_MIN 8
+#define VPK_REFILL_MIN 6
 #endif
 constexpr int kRefillMin = VPK_REFILL_MIN;   // S6b: free lanes are refilled once at least this many of a warp's lanes are free
 

@@ -209,15 +209,18 @@ __device__ __forceinline__ float face_distance(const DevGrid &G, const Hist &h, 
 // on that axis BEFORE the scattering of this step.  Returns true if the history left the grid.
 __device__ __forceinline__ bool cross_face(const DevGrid &G, Hist &h, int ax, bool up)
 {
-    // selects instead of a three-way branch: the lanes of a warp cross different faces
-    const uint32_t stride = ax == 0 ? 1u : (ax == 1 ? (uint32_t)G.nx : (uint32_t)(G.nx * G.ny));
-    const uint32_t n = ax == 0 ? (uint32_t)G.nx : (ax == 1 ? (uint32_t)G.ny : (uint32_t)G.nz);
-    const float snap = up ? 0.0f : (ax == 0 ? G.hx : (ax == 1 ? G.hy : G.hz));
-    const uint32_t idx = (ax == 0 ? h.g0 : (ax == 1 ? h.g1 : h.g2)) + (up ? 1u : 0xffffffffu);
-    h.g3 += up ? stride : 0u - stride;
-    h.g0 = ax == 0 ? idx : h.g0; h.g1 = ax == 1 ? idx : h.g1; h.g2 = ax == 2 ? idx : h.g2;
-    h.rx = ax == 0 ? snap : h.rx; h.ry = ax == 1 ? snap : h.ry; h.rz = ax == 2 ? snap : h.rz;
-    return idx >= n;
+    // a three-way branch on purpose: the select-only version measured twice the instructions (profiles/r1_README.md)
+    if (ax == 0) {
+        if (up) { h.g0 += 1u; h.g3 += 1u; h.rx = 0.0f; } else { h.g0 -= 1u; h.g3 -= 1u; h.rx = G.hx; }
+        return h.g0 >= (uint32_t)G.nx;
+    } else if (ax == 1) {
+        if (up) { h.g1 += 1u; h.g3 += (uint32_t)G.nx; h.ry = 0.0f; } else { h.g1 -= 1u; h.g3 -= (uint32_t)G.nx; h.ry = G.hy; }
+        return h.g1 >= (uint32_t)G.ny;
+    } else {
+        const uint32_t nxy = (uint32_t)(G.nx * G.ny);
+        if (up) { h.g2 += 1u; h.g3 += nxy; h.rz = 0.0f; } else { h.g2 -= 1u; h.g3 -= nxy; h.rz = G.hz; }
+        return h.g2 >= (uint32_t)G.nz;
+    }
 }
 
 // per-thread counters that live for the whole kernel (flushed once at its end)
