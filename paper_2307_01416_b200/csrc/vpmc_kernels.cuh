@@ -511,22 +511,39 @@ __device__ __forceinline__ int tile_column(const CsrCols &cc, int tile)
     return lo;
 }
 
-// first element of this thread in its tile -> (e, bx, by, bz); returns the number of elements it owns (0..kPerThread)
-__device__ __forceinline__ int tile_thread_range(const CsrCols &cc, int tile, int c, const int4 dm, long long &e, int &bx, int &by, int &bz)
+// first element of this thread in its tile (a box has < 2^31 elements) and the number of elements it owns (0..kPerThread)
+__device__ __forceinline__ int tile_thread_range(const CsrCols &cc, int tile, int c, const int4 dm, unsigned int &e)
 {
-    const long long vol = (long long)dm.x * dm.y * dm.z;
-    e = (long long)(tile - __ldg(cc.tile0 + c)) * kTile + (long long)threadIdx.x * kPerThread;
+    const unsigned int vol = (unsigned int)dm.x * (unsigned int)dm.y * (unsigned int)dm.z;
+    e = (unsigned int)(tile - __ldg(cc.tile0 + c)) * kTile + threadIdx.x * kPerThread;
     if (e >= vol) return 0;
-    const long long row = e / dm.x;
-    bx = (int)(e - row * dm.x);
-    bz = (int)(row / dm.y);
-    by = (int)(row - (long long)bz * dm.y);
-    const long long left = vol - e;
-    return left < kPerThread ? (int)left : kPerThread;
+    const unsigned int left = vol - e;
+    return left < (unsigned)kPerThread ? (int)left : kPerThread;
+}
+// box coordinates of element e (two 32-bit divisions: only taken by threads that need a voxel index)
+__device__ __forceinline__ void box_decode(unsigned int e, const int4 dm, int &bx, int &by, int &bz)
+{
+    const unsigned int row = e / (unsigned)dm.x;
+    bx = (int)(e - row * (unsigned)dm.x);
+    bz = (int)(row / (unsigned)dm.y);
+    by = (int)(row - (unsigned)bz * (unsigned)dm.y);
 }
 __device__ __forceinline__ void box_next(const int4 dm, int &bx, int &by, int &bz)
 {
     if (++bx == dm.x) { bx = 0; if (++by == dm.y) { by = 0; ++bz; } }
+}
+// the thread's kPerThread = 8 consecutive elements: two 16-byte loads when it owns all eight and they are aligned (always
+// the case inside a box: offsets and tiles are multiples of 8 elements), element-wise otherwise; missing elements read 0
+__device__ __forceinline__ void load8(const float *p, int cnt, float x[kPerThread])
+{
+    static_assert(kPerThread == 8, "load8 assumes 8 elements per thread");
+    if (cnt == kPerThread && (reinterpret_cast<size_t>(p) & 15) == 0) {
+        const float4 a = *reinterpret_cast<const float4 *>(p), b = *reinterpret_cast<const float4 *>(p + 4);
+        x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+    } else {
+#pragma unroll
+        for (int i = 0; i < kPerThread; ++i) x[i] = (i < cnt) ? p[i] : 0.0f;
+    }
 }
 
 template <bool CONVERT>
@@ -538,22 +555,37 @@ csr_max_kernel(const CsrCols cc, float *__restrict__ data, const short *__restri
         const int c = tile_column(cc, tile);
         if (cc.skip && __ldg(cc.skip + c)) continue;
         const int4 lo = __ldg(cc.lo + c), dm = __ldg(cc.dim + c);
-        long long e; int bx = 0, by = 0, bz = 0;
-        const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
+        unsigned int e;
+        const int cnt = tile_thread_range(cc, tile, c, dm, e);
         float *p = data + __ldg(cc.offset + c) + e;
+        float x[kPerThread];
+        load8(p, cnt, x);
         float mx = 0.0f;
-        for (int i = 0; i < cnt; ++i) {
-            float x = p[i];
-            if (CONVERT && x != 0.0f) {
-                const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
-                int t = (int)__ldg(hu + v) - hu_min;
-                t = min(max(t, 0), n_lut - 1);
-                x = __fdiv_rn(coef * x, fmaxf(__ldg(lut + t).y, rho_min));
-                p[i] = x;
+        bool any = false;
+#pragma unroll
+        for (int i = 0; i < kPerThread; ++i) any = any || (x[i] != 0.0f);
+        if (CONVERT && any) {
+            int bx, by, bz;
+            box_decode(e, dm, bx, by, bz);
+#pragma unroll
+            for (int i = 0; i < kPerThread; ++i) {
+                if (x[i] != 0.0f) {
+                    const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
+                    int t = (int)__ldg(hu + v) - hu_min;
+                    t = min(max(t, 0), n_lut - 1);
+                    x[i] = __fdiv_rn(coef * x[i], fmaxf(__ldg(lut + t).y, rho_min));
+                }
+                box_next(dm, bx, by, bz);
             }
-            mx = fmaxf(mx, x);
-            if (CONVERT) box_next(dm, bx, by, bz);
+            if (cnt == kPerThread && (reinterpret_cast<size_t>(p) & 15) == 0) {
+                *reinterpret_cast<float4 *>(p) = make_float4(x[0], x[1], x[2], x[3]);
+                *reinterpret_cast<float4 *>(p + 4) = make_float4(x[4], x[5], x[6], x[7]);
+            } else {
+                for (int i = 0; i < cnt; ++i) p[i] = x[i];
+            }
         }
+#pragma unroll
+        for (int i = 0; i < kPerThread; ++i) mx = fmaxf(mx, x[i]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
         if ((threadIdx.x & 31) == 0 && mx > 0.0f) atomicMax(colmax_bits + c, __float_as_uint(mx));
@@ -572,11 +604,13 @@ csr_count_kernel(const CsrCols cc, const float *__restrict__ data, const unsigne
         unsigned int k = 0;
         if (!(cc.skip && __ldg(cc.skip + c))) {
             const int4 dm = __ldg(cc.dim + c);
-            long long e; int bx, by, bz;
-            const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
-            const float *p = data + __ldg(cc.offset + c) + e;
+            unsigned int e;
+            const int cnt = tile_thread_range(cc, tile, c, dm, e);
             const float thr = rel_thr * __uint_as_float(__ldg(colmax_bits + c));
-            for (int i = 0; i < cnt; ++i) k += csr_keep(p[i], thr) ? 1u : 0u;
+            float x[kPerThread];
+            load8(data + __ldg(cc.offset + c) + e, cnt, x);
+#pragma unroll
+            for (int i = 0; i < kPerThread; ++i) k += csr_keep(x[i], thr) ? 1u : 0u;
         }
         k = __reduce_add_sync(0xffffffffu, k);
         if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = k;
@@ -630,14 +664,14 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
         const int c = tile_column(cc, tile);
         if (cc.skip && __ldg(cc.skip + c)) continue;          // block-uniform
         const int4 lo = __ldg(cc.lo + c), dm = __ldg(cc.dim + c);
-        long long e; int bx = 0, by = 0, bz = 0;
-        const int cnt = tile_thread_range(cc, tile, c, dm, e, bx, by, bz);
-        const float *p = data + __ldg(cc.offset + c) + e;
+        unsigned int e;
+        const int cnt = tile_thread_range(cc, tile, c, dm, e);
         const float thr = rel_thr * __uint_as_float(__ldg(colmax_bits + c));
         float x[kPerThread];
+        load8(data + __ldg(cc.offset + c) + e, cnt, x);
         unsigned int k = 0;
 #pragma unroll
-        for (int i = 0; i < kPerThread; ++i) { x[i] = (i < cnt) ? p[i] : 0.0f; k += csr_keep(x[i], thr) ? 1u : 0u; }
+        for (int i = 0; i < kPerThread; ++i) k += csr_keep(x[i], thr) ? 1u : 0u;
         unsigned int inc = k;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(0xffffffffu, inc, o); if ((threadIdx.x & 31) >= o) inc += y; }
@@ -646,6 +680,8 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
         unsigned int woff = 0;
         for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += wsum[w];
         long long pos = __ldg(col_base + c) + (long long)__ldg(tile_off + tile) + woff + inc - k;
+        int bx = 0, by = 0, bz = 0;
+        if (k) box_decode(e, dm, bx, by, bz);
 #pragma unroll
         for (int i = 0; i < kPerThread; ++i) {
             if (csr_keep(x[i], thr)) {

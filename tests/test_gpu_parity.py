@@ -142,6 +142,25 @@ def test_dose_parity(bind, case, N):
     eng.close()
 
 
+def test_small_calibration_uses_the_shared_memory_table(bind):
+    """A calibration spanning <= 1024 HU keeps the material table in shared memory (voxel_kernel<*, true>); HU outside the
+    node range clamp to the end nodes (S:8c-C5)."""
+    O = orc()
+    w = hetero_case()
+    w["calib"] = {"hu": np.array([-200, 0, 300], dtype=np.float32), "rsp": np.array([0.8, 1.0, 1.2], dtype=np.float32),
+                  "rho": np.array([0.8, 1.0, 1.25], dtype=np.float32), "xsp": None}
+    N = 100_000
+    eng = bind.Engine(w)
+    d_gpu = eng.dose(N, 6).cpu().numpy().astype(np.float64)
+    tg = eng.tallies().as_dict()
+    d_orc, to = O.dose(oracle_problem(w), N, 6)
+    to = to.as_dict()
+    assert np.abs(d_gpu - d_orc).max() < 1e-3 * d_orc.max()
+    for k in ("n_stopped_ct", "n_stopped_brass", "n_nuclear", "n_escaped"):
+        assert abs(int(tg[k]) - int(to[k])) <= 2
+    eng.close()
+
+
 def test_dose_host_entry_and_determinism(bind):
     w = wl.config1()
     eng = bind.Engine(w)
