@@ -111,6 +111,7 @@ typedef struct {
     int32_t ivox[3];            /* voxel at step start (CT) else -1 */
     double r[3], u[3];          /* after the step; beam frame in the beam line, CT frame from the CT-entry drift on */
     double E_before, E_after, s;
+    double t_rad, tau, tau_star; /* carried scattering depth and nuclear optical depth after the step; threshold */
 } orc_step_rec;
 
 /* ------------------------------------------------------------------ C1 */
@@ -142,8 +143,18 @@ double orc_u01(uint32_t x)
     return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0);
 }
 
+/* Test hook (tests/test_oracle_geometry.py, hand-traced histories with MCS on): when set, the
+ * transport block (purpose 0) of step k < n is u[4k..4k+3] instead of the Philox output.  No arithmetic here. */
+static const double *g_inject_u = NULL;
+static int32_t g_inject_n = 0;
+void orc_inject_uniforms(const double *u, int32_t n_steps) { g_inject_u = u; g_inject_n = u ? n_steps : 0; }
+
 static void draw4(uint64_t hid, uint32_t step, uint32_t purpose, uint64_t seed, double u[4])
 {
+    if (purpose == 0u && g_inject_u && step < (uint32_t)g_inject_n) {
+        for (int i = 0; i < 4; ++i) u[i] = g_inject_u[4 * (size_t)step + i];
+        return;
+    }
     uint32_t ctr[4] = { (uint32_t)hid, (uint32_t)(hid >> 32), step, purpose };
     uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
     uint32_t o[4];
@@ -226,6 +237,7 @@ static void trace_put(tracer *t, uint64_t hid, const hist *h, uint32_t step, int
     q->hid = hid; q->step = (int32_t)step; q->region = region; q->cause = cause;
     for (int a = 0; a < 3; ++a) { q->ivox[a] = iv ? iv[a] : -1; q->r[a] = h->r[a]; q->u[a] = h->u[a]; }
     q->E_before = Eb; q->E_after = Ea; q->s = s;
+    q->t_rad = h->t_rad; q->tau = h->tau; q->tau_star = h->tau_star;
 }
 
 static double highland_A(double t, double c_log)

@@ -104,11 +104,13 @@ class Tallies(C.Structure):
 class StepRec(C.Structure):
     _fields_ = [("hid", C.c_uint64), ("step", C.c_int32), ("region", C.c_int32), ("cause", C.c_int32),
                 ("ivox", C.c_int32 * 3), ("r", C.c_double * 3), ("u", C.c_double * 3),
-                ("E_before", C.c_double), ("E_after", C.c_double), ("s", C.c_double)]
+                ("E_before", C.c_double), ("E_after", C.c_double), ("s", C.c_double),
+                ("t_rad", C.c_double), ("tau", C.c_double), ("tau_star", C.c_double)]
 
 
 STEP_DTYPE = np.dtype([("hid", "<u8"), ("step", "<i4"), ("region", "<i4"), ("cause", "<i4"), ("ivox", "<i4", 3),
-                       ("r", "<f8", 3), ("u", "<f8", 3), ("E_before", "<f8"), ("E_after", "<f8"), ("s", "<f8")],
+                       ("r", "<f8", 3), ("u", "<f8", 3), ("E_before", "<f8"), ("E_after", "<f8"), ("s", "<f8"),
+                       ("t_rad", "<f8"), ("tau", "<f8"), ("tau_star", "<f8")],
                       align=True)
 
 _lib = None
@@ -346,6 +348,22 @@ def trace(pb: Problem, hids, n_or_hps: int, seed: int, sc: Scenario | None = Non
     assert rc == 0
     assert (nrec <= max_steps).all(), "max_steps too small"
     return [recs[i, :nrec[i]] for i in range(hids.size)]
+
+
+class injected_uniforms:
+    """Context manager of the oracle's test hook: the transport block (purpose 0) of step k is u[k] (4 numbers)
+    for k < len(u); later steps draw from Philox as usual."""
+
+    def __init__(self, u):
+        self.u = np.ascontiguousarray(np.asarray(u, dtype=np.float64).reshape(-1, 4))
+
+    def __enter__(self):
+        lib().orc_inject_uniforms(C.c_void_p(self.u.ctypes.data), C.c_int32(self.u.shape[0]))
+        return self
+
+    def __exit__(self, *exc):
+        lib().orc_inject_uniforms(None, C.c_int32(0))
+        return False
 
 
 # ----------------------------------------------------------------------------- C6 estimators (numpy)
