@@ -128,6 +128,8 @@ typedef struct {
     int32_t ivox[3];
     float r[3], u[3];
     float E_before, E_after, s;
+    float dep;                   /* energy deposited in the step's cell (CT voxel, range-shifter or brass tally), MeV */
+    int32_t pad_;
 } vpmc_step_rec;
 
 void vpmc_default_params(vpmc_params *p);
@@ -169,6 +171,18 @@ int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *sc, uint64_t n_histories,
 /* vpmc_dose with the result copied to dose_out_host ([host], nx*ny*nz floats); synchronous. */
 int vpmc_dose_host(vpmc_t *h, uint64_t n_histories, uint64_t seed, float *dose_out_host);
 
+/* Dose to a statistical uncertainty with the stopping rule ON THE DEVICE (S:8d metric 2, S:8f-3; "<0.5 %").
+ * Batches of batch_histories histories are transported one after another; batch k (0, 1, ...) is the batch_histories-history
+ * plan sample whose history ids are k 2^32 + i (D:R15).  After each batch the C6 estimator over the batches so far (mean over
+ * voxels >= 50 % of the maximum of sigma_v / D_v) is evaluated by a kernel, and a CUDA-graph WHILE node repeats the batch
+ * pass until at least max(min_batches, 2) batches ran and the estimate <= target_rel_unc, or max_batches ran: no host round
+ * trip between batches.  dose_out_dev is the dose of all batches run (C6 with N = batches x batch_histories).
+ * batch_histories <= the chunk size (2^23).  Asynchronous on `cuda_stream`; vpmc_get_run_info synchronises. */
+int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *sc, uint64_t batch_histories, int32_t min_batches,
+                             int32_t max_batches, float target_rel_unc, uint64_t seed, float *dose_out_dev, void *cuda_stream);
+/* Result of the last vpmc_dose_to_uncertainty: batches run, the estimate after the last one, whether the target stopped it. */
+int vpmc_get_run_info(vpmc_t *h, int32_t *batches_out, float *rel_unc_out, int32_t *reached_target_out);
+
 /* Restrict the next dose / trace calls to history ids [hid_begin, hid_end) of the N-history run (prefix
  * parity, S:8d).  hid_end = 0 -> no restriction. */
 int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);
@@ -202,6 +216,63 @@ int vpmc_get_uncertainty(vpmc_t *h, float *rel_unc_out);
  * with hist_per_spot = n_or_hps.  out_host: n*max_steps records; nrec_host[i] = records of history i. */
 int vpmc_trace(vpmc_t *h, const vpmc_scenario *sc, int32_t mode, uint64_t n_or_hps, uint64_t seed,
                const uint64_t *hids, int32_t n, int32_t max_steps, vpmc_step_rec *out_host, int32_t *nrec_host);
+
+/* Test-only: ONE step of the path from a supplied pre-step state (north_star: "histories must agree step-for-step";
+ * S:8c-A9).  The tests feed the oracle's pre-step state of every step, so the comparison carries no accumulated
+ * difference.  kind selects the step function: the S1 sampler, a vacuum drift to the next device, one range-shifter /
+ * aperture-region step (S2 / S3: the medium of an aperture step is decided by the kernel's own bitmap test), the CT
+ * entry (C3), or one voxel step (S4 + S5).  r, u: beam frame (r[2] = w) for kinds 0-5, CT frame for kind 6. */
+#define VPMC_STEP_SOURCE 0       /* in: hid, spot (global index); out: r, E, tau_star */
+#define VPMC_STEP_DRIFT_TO_RS 1
+#define VPMC_STEP_RS 2
+#define VPMC_STEP_DRIFT_TO_AP 3
+#define VPMC_STEP_AP 4
+#define VPMC_STEP_CT_ENTRY 5     /* out: r, u in the CT frame, ivox_after = entry voxel */
+#define VPMC_STEP_CT 6           /* in: ivox = current voxel */
+typedef struct {
+    uint64_t hid;
+    int32_t kind, step, beam, spot;
+    int32_t ivox[3];
+    int32_t pad_;
+    double r[3], u[3];
+    double E, t_rad, tau, tau_star;
+} vpmc_state;
+typedef struct {
+    int32_t region, cause, step_after, n_steps;   /* n_steps > 1: the kernel took several opening drifts at once (D:R14); the
+                                                     FIRST is reported */
+    int32_t ivox_after[3];
+    int32_t pad_;
+    double r[3], u[3];           /* after the step, summed from the kernel's own representation (hi + lo, voxel + offset) */
+    double E, R, s, dep, t_rad, tau, tau_star;     /* R = residual range carried by the kernel (fp64) */
+} vpmc_state_out;
+/* states, out: [host], n entries.  Scenario NULL = nominal.  Synchronous.  Needs beams and spots to be set. */
+int vpmc_step_from_state(vpmc_t *h, const vpmc_scenario *sc, uint64_t seed, const vpmc_state *states, int32_t n,
+                         vpmc_state_out *out);
+
+/* Test-only: one digest per history of the contiguous ids [hid_begin, hid_begin + n) of the N-history dose run: number
+ * of step records, FNV-1a hash (offset 14695981039346656037, prime 1099511628211, one round per 32-bit word) over
+ * (region, cause, ivox[0..2]) of every record in order, position after the last record, energy left after it, and
+ * the energy deposited in the CT.  Lets a test find, among 10^6 histories, the few whose discrete trace or end point
+ * differs from the oracle's.  out_host: n entries.  Synchronous. */
+typedef struct {
+    uint64_t hid, hash;
+    int32_t n_rec, cause;
+    float r[3];
+    float E_last, dep_ct;
+    int32_t pad_;
+} vpmc_digest;
+int vpmc_digests(vpmc_t *h, const vpmc_scenario *sc, uint64_t n_histories, uint64_t seed, uint64_t hid_begin, int32_t n,
+                 vpmc_digest *out_host);
+
+/* Test / tuning knobs of one handle (none changes a result beyond the order of floating-point sums; the tests use them
+ * to force the rarely taken code paths).  Returns VPMC_ERR_INVALID_ARG for an unknown knob or a value out of range. */
+#define VPMC_KNOB_CHUNK 0        /* work items per pass of the pipeline (default 2^23) */
+#define VPMC_KNOB_BOX_GROW 1     /* influence: growth of the pilot box, fraction of its extent (default 0.05) */
+#define VPMC_KNOB_BOX_PAD 2      /* influence: extra voxels per side (default 1) */
+#define VPMC_KNOB_OVF_CAP 3      /* influence: capacity of the overflow list (default 2^25; 0 forces the replay path) */
+#define VPMC_KNOB_LUT_GLOBAL 4   /* 1 = never stage the material table in shared memory */
+#define VPMC_KNOB_VERBOSE 5      /* 1 = progress lines of the influence path on stderr */
+int vpmc_set_knob(vpmc_t *h, int knob, double value);
 
 /* Per-kernel-class device timing (bench.py's roofline): when on, every launch is bracketed by CUDA events on its
  * stream.  vpmc_get_timing synchronises, returns accumulated milliseconds and launch counts per class

@@ -112,6 +112,7 @@ typedef struct {
     double r[3], u[3];          /* after the step; beam frame in the beam line, CT frame from the CT-entry drift on */
     double E_before, E_after, s;
     double t_rad, tau, tau_star; /* carried scattering depth and nuclear optical depth after the step; threshold */
+    double dep;                 /* energy deposited in the step's cell (CT voxel, range-shifter or brass tally), MeV */
 } orc_step_rec;
 
 /* ------------------------------------------------------------------ C1 */
@@ -225,19 +226,39 @@ typedef struct {
     uint32_t step;
 } hist;
 
+/* per-history digest (orc_digests): number of records, FNV-1a hash of the discrete trace, state after the last record */
+typedef struct {
+    uint64_t hid, hash;
+    int32_t n_rec, cause;
+    double r[3];
+    double E_last, dep_ct;
+} orc_digest;
+
 typedef struct {
     orc_step_rec *recs; int32_t max, n;
+    orc_digest *dig;            /* when set, records are digested instead of stored */
 } tracer;
 
+static void fnv_mix(uint64_t *h, uint32_t v) { *h = (*h ^ (uint64_t)v) * 1099511628211ull; }
+
 static void trace_put(tracer *t, uint64_t hid, const hist *h, uint32_t step, int region,
-                      const int32_t iv[3], double Eb, double Ea, double s, int cause)
+                      const int32_t iv[3], double Eb, double Ea, double s, int cause, double dep)
 {
+    if (t && t->dig) {          /* hash over (region, cause, ivox[0..2]) of every record, one FNV-1a round per 32-bit word */
+        orc_digest *d = t->dig;
+        fnv_mix(&d->hash, (uint32_t)region); fnv_mix(&d->hash, (uint32_t)cause);
+        for (int a = 0; a < 3; ++a) fnv_mix(&d->hash, (uint32_t)(iv ? iv[a] : -1));
+        d->n_rec += 1; d->cause = cause; d->E_last = Ea;
+        for (int a = 0; a < 3; ++a) d->r[a] = h->r[a];
+        return;
+    }
     if (!t || t->n >= t->max) { if (t) t->n++; return; }
     orc_step_rec *q = &t->recs[t->n++];
     q->hid = hid; q->step = (int32_t)step; q->region = region; q->cause = cause;
     for (int a = 0; a < 3; ++a) { q->ivox[a] = iv ? iv[a] : -1; q->r[a] = h->r[a]; q->u[a] = h->u[a]; }
     q->E_before = Eb; q->E_after = Ea; q->s = s;
     q->t_rad = h->t_rad; q->tau = h->tau; q->tau_star = h->tau_star;
+    q->dep = dep;
 }
 
 static double highland_A(double t, double c_log)
@@ -382,7 +403,7 @@ static int drift_to_plane(ctx *c, hist *h, uint64_t hid, double wt)
     double s = (wt - h->r[2]) / h->u[2];
     if (s < 0.0) s = 0.0;
     h->r[0] += s * h->u[0]; h->r[1] += s * h->u[1]; h->r[2] = wt;
-    trace_put(c->tr, hid, h, h->step, ORC_REG_VAC, NULL, h->E, h->E, s, ORC_CONT);
+    trace_put(c->tr, hid, h, h->step, ORC_REG_VAC, NULL, h->E, h->E, s, ORC_CONT, 0.0);
     h->step += 1;
     return ORC_CONT;
 }
@@ -435,7 +456,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             cause = material_step(P, &h, &m, d, hid, c->seed, &s, &dep, &rem, &on_d);
             if (c->tal) { c->tal->dep_rs += dep; c->tal->removed += rem; }
             if (cause == ORC_CONT && on_d && ex) h.r[2] = w_rs_out;
-            trace_put(c->tr, hid, &h, st, ORC_REG_RS, NULL, Eb, h.E, s, cause);
+            trace_put(c->tr, hid, &h, st, ORC_REG_RS, NULL, Eb, h.E, s, cause, dep);
             if (cause != ORC_CONT) { finish(c, cause, ORC_REG_RS, 0.0); return; }
             if (on_d && ex) break;
         }
@@ -458,7 +479,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             if (open) {   /* "transported with the previous velocity and direction" */
                 for (int a = 0; a < 3; ++a) h.r[a] += d * h.u[a];
                 if (ex) h.r[2] = w_ap_out;
-                trace_put(c->tr, hid, &h, h.step, ORC_REG_AP_OPEN, NULL, h.E, h.E, d, ORC_CONT);
+                trace_put(c->tr, hid, &h, h.step, ORC_REG_AP_OPEN, NULL, h.E, h.E, d, ORC_CONT, 0.0);
                 h.step += 1;
                 if (ex) break;
                 continue;
@@ -467,7 +488,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             cause = material_step(P, &h, &m, d, hid, c->seed, &s, &dep, &rem, &on_d);
             if (c->tal) { c->tal->dep_brass += dep; c->tal->removed += rem; }
             if (cause == ORC_CONT && on_d && ex) h.r[2] = w_ap_out;
-            trace_put(c->tr, hid, &h, st, ORC_REG_AP_BRASS, NULL, Eb, h.E, s, cause);
+            trace_put(c->tr, hid, &h, st, ORC_REG_AP_BRASS, NULL, Eb, h.E, s, cause, dep);
             if (cause != ORC_CONT) { finish(c, cause, ORC_REG_AP_BRASS, 0.0); return; }
             if (on_d && ex) break;
         }
@@ -494,7 +515,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             if (tf < t_out) t_out = tf;
         }
         if (miss || !(t_in < t_out)) {
-            trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, 0.0, ORC_ESCAPED);
+            trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, 0.0, ORC_ESCAPED, 0.0);
             finish(c, ORC_ESCAPED, ORC_REG_VAC, h.E); return;
         }
         for (int a = 0; a < 3; ++a) h.r[a] += t_in * h.u[a];
@@ -509,7 +530,7 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
                 iv[a] = (int32_t)f;
             }
         }
-        trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, t_in, ORC_CONT);
+        trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, t_in, ORC_CONT, 0.0);
         h.step += 1;
     }
 
@@ -543,12 +564,12 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             if (iv[ax] < 0 || iv[ax] >= ct->n[ax]) out = 1;
         }
         if (out) cause = ORC_ESCAPED;
-        trace_put(c->tr, hid, &h, st, ORC_REG_CT, iv0, Eb, h.E, s, cause);
+        trace_put(c->tr, hid, &h, st, ORC_REG_CT, iv0, Eb, h.E, s, cause, dep);
         if (cause != ORC_CONT) { finish(c, cause, ORC_REG_CT, cause == ORC_ESCAPED ? h.E : 0.0); return; }
     }
 
 escaped_beamline:
-    trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, 0.0, ORC_ESCAPED);
+    trace_put(c->tr, hid, &h, h.step, ORC_REG_VAC, NULL, h.E, h.E, 0.0, ORC_ESCAPED, 0.0);
     finish(c, ORC_ESCAPED, ORC_REG_VAC, h.E);
 }
 
@@ -590,20 +611,23 @@ void orc_spot_counts(const orc_problem *pb, uint64_t N, uint64_t *counts)
     free_spotmap(&m);
 }
 
-static void run_spot_range(ctx *c, const spotmap *m, int32_t g, uint64_t a, uint64_t b)
+static void run_spot_range(ctx *c, const spotmap *m, int32_t g, uint64_t a, uint64_t b, uint64_t hid_offset)
 {
     const orc_beam *bm = &c->pb->beams[m->beam[g]];
-    for (uint64_t hid = a; hid < b; ++hid) run_history(c, hid, bm, m->local[g]);
+    for (uint64_t hid = a; hid < b; ++hid) run_history(c, hid_offset + hid, bm, m->local[g]);
 }
 
 /* Dose mode: transport history ids [hid_begin, hid_end) of an N-history run
  * that belong to batch `batch` of `n_batches` (C6; each spot's contiguous id
  * range is cut into n_batches contiguous sub-ranges, batch b = union over
  * spots of sub-range b -- DESIGN.md reading R7).  n_batches = 1 -> all.
+ * hid_offset is added to every id before it keys the random stream (C1): the
+ * sequential stopping rule of SURVEY 8(d) runs its k-th 10^6-history batch as
+ * ids k 2^32 + i (R15); 0 everywhere else.
  * edep (nvox doubles, MeV) is accumulated into, not zeroed. */
-int orc_dose_edep(const orc_problem *pb, const orc_scenario *sc, uint64_t N, uint64_t seed,
-                  uint64_t hid_begin, uint64_t hid_end, int32_t batch, int32_t n_batches,
-                  double *edep, orc_tallies *tal)
+int orc_dose_edep_offset(const orc_problem *pb, const orc_scenario *sc, uint64_t N, uint64_t seed,
+                         uint64_t hid_begin, uint64_t hid_end, int32_t batch, int32_t n_batches,
+                         uint64_t hid_offset, double *edep, orc_tallies *tal)
 {
     if (n_batches < 1 || batch < 0 || batch >= n_batches) return -1;
     spotmap m = build_spotmap(pb, N);
@@ -614,10 +638,17 @@ int orc_dose_edep(const orc_problem *pb, const orc_scenario *sc, uint64_t N, uin
         uint64_t hi = m.start[g] + (uint64_t)(((unsigned __int128)n * (uint64_t)(batch + 1)) / (uint64_t)n_batches);
         if (lo < hid_begin) lo = hid_begin;
         if (hi > hid_end) hi = hid_end;
-        if (lo < hi) run_spot_range(&c, &m, g, lo, hi);
+        if (lo < hi) run_spot_range(&c, &m, g, lo, hi, hid_offset);
     }
     free_spotmap(&m);
     return 0;
+}
+
+int orc_dose_edep(const orc_problem *pb, const orc_scenario *sc, uint64_t N, uint64_t seed,
+                  uint64_t hid_begin, uint64_t hid_end, int32_t batch, int32_t n_batches,
+                  double *edep, orc_tallies *tal)
+{
+    return orc_dose_edep_offset(pb, sc, N, seed, hid_begin, hid_end, batch, n_batches, 0, edep, tal);
 }
 
 /* C6: dose[v] = scale * E_dep[v] / (max(rho_v, rho_min) * V_vox[cm^3]) * 1.602176634e-10 Gy */
@@ -660,7 +691,7 @@ int orc_trace(const orc_problem *pb, const orc_scenario *sc, int32_t mode, uint6
     if (mode == 0) m = build_spotmap(pb, n_or_hps);
     int32_t nsp = total_spots(pb);
     for (int32_t i = 0; i < n; ++i) {
-        tracer tr = { recs + (int64_t)i * max_steps, max_steps, 0 };
+        tracer tr = { recs + (int64_t)i * max_steps, max_steps, 0, NULL };
         ctx c = { pb, sc, seed, NULL, NULL, 0, 0, NULL, &tr };
         int32_t g;
         if (mode == 0) {
@@ -679,6 +710,31 @@ int orc_trace(const orc_problem *pb, const orc_scenario *sc, int32_t mode, uint6
         nrec[i] = tr.n;
     }
     if (mode == 0) free_spotmap(&m);
+    return 0;
+}
+
+/* Digests of the contiguous history ids [hid_begin, hid_begin + n) of the N-history dose run (test support: finds
+ * the histories whose discrete trace or end point differs between two implementations without storing every step). */
+int orc_digests(const orc_problem *pb, const orc_scenario *sc, uint64_t N, uint64_t seed, uint64_t hid_begin, int32_t n,
+                orc_digest *out)
+{
+    spotmap m = build_spotmap(pb, N);
+    int32_t g = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        uint64_t hid = hid_begin + (uint64_t)i;
+        if (hid >= N) { free_spotmap(&m); return -1; }
+        while (g + 1 < m.n && m.start[g + 1] <= hid) ++g;
+        orc_digest *d = &out[i];
+        memset(d, 0, sizeof(*d));
+        d->hid = hid; d->hash = 1469598103934665603ull;
+        tracer tr = { NULL, 0, 0, d };
+        orc_tallies tal;
+        memset(&tal, 0, sizeof(tal));
+        ctx c = { pb, sc, seed, NULL, NULL, 0, 0, &tal, &tr };
+        run_history(&c, hid, &pb->beams[m.beam[g]], m.local[g]);
+        d->dep_ct = tal.dep_ct;
+    }
+    free_spotmap(&m);
     return 0;
 }
 

@@ -105,13 +105,16 @@ class StepRec(C.Structure):
     _fields_ = [("hid", C.c_uint64), ("step", C.c_int32), ("region", C.c_int32), ("cause", C.c_int32),
                 ("ivox", C.c_int32 * 3), ("r", C.c_double * 3), ("u", C.c_double * 3),
                 ("E_before", C.c_double), ("E_after", C.c_double), ("s", C.c_double),
-                ("t_rad", C.c_double), ("tau", C.c_double), ("tau_star", C.c_double)]
+                ("t_rad", C.c_double), ("tau", C.c_double), ("tau_star", C.c_double), ("dep", C.c_double)]
 
 
 STEP_DTYPE = np.dtype([("hid", "<u8"), ("step", "<i4"), ("region", "<i4"), ("cause", "<i4"), ("ivox", "<i4", 3),
                        ("r", "<f8", 3), ("u", "<f8", 3), ("E_before", "<f8"), ("E_after", "<f8"), ("s", "<f8"),
-                       ("t_rad", "<f8"), ("tau", "<f8"), ("tau_star", "<f8")],
+                       ("t_rad", "<f8"), ("tau", "<f8"), ("tau_star", "<f8"), ("dep", "<f8")],
                       align=True)
+
+DIGEST_DTYPE = np.dtype([("hid", "<u8"), ("hash", "<u8"), ("n_rec", "<i4"), ("cause", "<i4"), ("r", "<f8", 3),
+                         ("E_last", "<f8"), ("dep_ct", "<f8")], align=True)
 
 _lib = None
 
@@ -263,15 +266,18 @@ def spot_counts(pb: Problem, N: int) -> np.ndarray:
 
 
 def dose_edep(pb: Problem, N: int, seed: int, sc: Scenario | None = None, hid_begin: int = 0,
-              hid_end: int | None = None, batch: int = 0, n_batches: int = 1, edep: np.ndarray | None = None):
-    """E_dep [MeV] (fp64, flat nvox) of history ids [hid_begin, hid_end) of an N-history dose run."""
+              hid_end: int | None = None, batch: int = 0, n_batches: int = 1, edep: np.ndarray | None = None,
+              hid_offset: int = 0):
+    """E_dep [MeV] (fp64, flat nvox) of history ids [hid_begin, hid_end) of an N-history dose run; hid_offset is added
+    to every id before it keys the random stream (sequential batches, R15)."""
     sc = sc or scenario()
     if edep is None:
         edep = np.zeros(pb.nvox, dtype=np.float64)
     tal = Tallies()
-    rc = lib().orc_dose_edep(C.byref(pb.cstruct()), C.byref(sc), C.c_uint64(int(N)), C.c_uint64(int(seed)),
-                             C.c_uint64(int(hid_begin)), C.c_uint64(int(N if hid_end is None else hid_end)),
-                             C.c_int32(batch), C.c_int32(n_batches), C.c_void_p(edep.ctypes.data), C.byref(tal))
+    rc = lib().orc_dose_edep_offset(C.byref(pb.cstruct()), C.byref(sc), C.c_uint64(int(N)), C.c_uint64(int(seed)),
+                                    C.c_uint64(int(hid_begin)), C.c_uint64(int(N if hid_end is None else hid_end)),
+                                    C.c_int32(batch), C.c_int32(n_batches), C.c_uint64(int(hid_offset)),
+                                    C.c_void_p(edep.ctypes.data), C.byref(tal))
     assert rc == 0
     return edep, tal
 
@@ -350,6 +356,16 @@ def trace(pb: Problem, hids, n_or_hps: int, seed: int, sc: Scenario | None = Non
     return [recs[i, :nrec[i]] for i in range(hids.size)]
 
 
+def digests(pb: Problem, N: int, seed: int, hid_begin: int, n: int, sc: Scenario | None = None) -> np.ndarray:
+    """DIGEST_DTYPE array of history ids [hid_begin, hid_begin + n) of the N-history dose run."""
+    sc = sc or scenario()
+    out = np.zeros(n, dtype=DIGEST_DTYPE)
+    rc = lib().orc_digests(C.byref(pb.cstruct()), C.byref(sc), C.c_uint64(int(N)), C.c_uint64(int(seed)),
+                           C.c_uint64(int(hid_begin)), C.c_int32(int(n)), C.c_void_p(out.ctypes.data))
+    assert rc == 0
+    return out
+
+
 class injected_uniforms:
     """Context manager of the oracle's test hook: the transport block (purpose 0) of step k is u[k] (4 numbers)
     for k < len(u); later steps draw from Philox as usual."""
@@ -377,6 +393,26 @@ def batch_uncertainty(batch_doses: np.ndarray) -> float:
     var = ((D - mean) ** 2).sum(axis=0) / (B * (B - 1))
     sel = mean >= 0.5 * mean.max()
     return float(np.mean(np.sqrt(var[sel]) / mean[sel]))
+
+
+def dose_to_uncertainty(pb: Problem, batch_histories: int, target: float, seed: int, min_batches: int = 2,
+                        max_batches: int = 1000, sc: Scenario | None = None):
+    """SURVEY.md 8(d) metric (2) / P:L107, "<0.5 %": sequential stopping rule.  Batches of `batch_histories`
+    histories are run one after another -- the k-th (k = 0, 1, ...) is the batch_histories-history plan sample with
+    history ids k 2^32 + i (R15) -- and after each the C6 estimator over the batch doses so far is
+    evaluated; stop as soon as k + 1 >= min_batches and the estimate <= target (or at max_batches).
+    Returns (dose [Gy], batches used, list of the estimates after each batch from the second on)."""
+    batches, history = [], []
+    scale = pb.total_weight / float(batch_histories)
+    while len(batches) < max_batches:
+        k = len(batches)
+        e, _ = dose_edep(pb, batch_histories, seed, sc, hid_offset=k << 32)
+        batches.append(dose_from_edep(pb, e, scale))
+        if len(batches) >= 2:
+            history.append(batch_uncertainty(np.array(batches)))
+            if len(batches) >= min_batches and history[-1] <= target:
+                break
+    return np.mean(np.array(batches), axis=0), len(batches), history
 
 
 def gamma_pass_rate(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: float = 1.0, thr: float = 0.1,

@@ -21,7 +21,11 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_set_range_shifter", "vpmc_set_aperture", "vpmc_dose", "vpmc_dose_scenario", "vpmc_dose_host",
            "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
-           "vpmc_get_timing", "vpmc_set_workspace_limit"]
+           "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
+           "vpmc_get_run_info"]
+
+STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
+KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
 
 
 class VpmcError(RuntimeError):
@@ -69,8 +73,19 @@ class Tallies(C.Structure):
 
 
 STEP_DTYPE = np.dtype([("hid", "<u8"), ("step", "<i4"), ("region", "<i4"), ("cause", "<i4"), ("ivox", "<i4", 3),
-                       ("r", "<f4", 3), ("u", "<f4", 3), ("E_before", "<f4"), ("E_after", "<f4"), ("s", "<f4")],
-                      align=True)
+                       ("r", "<f4", 3), ("u", "<f4", 3), ("E_before", "<f4"), ("E_after", "<f4"), ("s", "<f4"),
+                       ("dep", "<f4"), ("pad_", "<i4")], align=True)
+
+STATE_DTYPE = np.dtype([("hid", "<u8"), ("kind", "<i4"), ("step", "<i4"), ("beam", "<i4"), ("spot", "<i4"),
+                        ("ivox", "<i4", 3), ("pad_", "<i4"), ("r", "<f8", 3), ("u", "<f8", 3),
+                        ("E", "<f8"), ("t_rad", "<f8"), ("tau", "<f8"), ("tau_star", "<f8")], align=True)
+STATE_OUT_DTYPE = np.dtype([("region", "<i4"), ("cause", "<i4"), ("step_after", "<i4"), ("n_steps", "<i4"),
+                            ("ivox_after", "<i4", 3), ("pad_", "<i4"), ("r", "<f8", 3), ("u", "<f8", 3),
+                            ("E", "<f8"), ("R", "<f8"), ("s", "<f8"), ("dep", "<f8"), ("t_rad", "<f8"), ("tau", "<f8"),
+                            ("tau_star", "<f8")], align=True)
+
+DIGEST_DTYPE = np.dtype([("hid", "<u8"), ("hash", "<u8"), ("n_rec", "<i4"), ("cause", "<i4"), ("r", "<f4", 3),
+                         ("E_last", "<f4"), ("dep_ct", "<f4"), ("pad_", "<i4")], align=True)
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 
@@ -113,6 +128,12 @@ def lib():
         L.vpmc_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.vpmc_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         L.vpmc_set_workspace_limit.argtypes = [C.c_void_p, C.c_uint64]
+        L.vpmc_step_from_state.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_void_p, C.c_int32, C.c_void_p]
+        L.vpmc_set_knob.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.vpmc_dose_to_uncertainty.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_int32, C.c_int32, C.c_float,
+                                               C.c_uint64, C.c_void_p, C.c_void_p]
+        L.vpmc_get_run_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+        L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
 
@@ -225,6 +246,25 @@ class Engine:
                                                  st.cuda_stream))
         return out
 
+    def dose_to_uncertainty(self, batch_histories: int, target: float, seed: int, min_batches: int = 2,
+                            max_batches: int = 1000, out=None, sc: Scenario | None = None, stream=None):
+        """Dose run batch by batch until the C6 estimate <= target, the stopping rule decided on the device
+        (vpmc_dose_to_uncertainty).  Returns the dose tensor; run_info() gives (batches, estimate, reached)."""
+        import torch
+        if out is None:
+            out = torch.empty(self.nvox, dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.nvox and out.is_contiguous()
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(lib().vpmc_dose_to_uncertainty(self._h, C.byref(sc) if sc is not None else None, int(batch_histories),
+                                                   int(min_batches), int(max_batches), float(target), int(seed),
+                                                   out.data_ptr(), st.cuda_stream))
+        return out
+
+    def run_info(self):
+        b, u, r = C.c_int32(), C.c_float(), C.c_int32()
+        self._check(lib().vpmc_get_run_info(self._h, C.byref(b), C.byref(u), C.byref(r)))
+        return int(b.value), float(u.value), bool(r.value)
+
     def dose_host(self, n_histories: int, seed: int, out: np.ndarray | None = None) -> np.ndarray:
         if out is None:
             out = np.empty(self.nvox, dtype=np.float32)
@@ -289,6 +329,24 @@ class Engine:
             val = keep[o.val][: 4 * o.nnz].view(torch.float32) if o.nnz else torch.empty(0, dtype=torch.float32, device="cuda")
             res.append((rp, col, val))
         return res
+
+    def step_from_state(self, states: np.ndarray, seed: int, sc: Scenario | None = None) -> np.ndarray:
+        """Test-only: one step from each pre-step state (STATE_DTYPE array) -> STATE_OUT_DTYPE array."""
+        states = np.ascontiguousarray(states, dtype=STATE_DTYPE)
+        out = np.zeros(states.size, dtype=STATE_OUT_DTYPE)
+        self._check(lib().vpmc_step_from_state(self._h, C.byref(sc) if sc is not None else None, int(seed),
+                                               states.ctypes.data, states.size, out.ctypes.data))
+        return out
+
+    def digests(self, n_histories: int, seed: int, hid_begin: int, n: int, sc: Scenario | None = None) -> np.ndarray:
+        """Test-only: DIGEST_DTYPE array of the history ids [hid_begin, hid_begin + n) of the n_histories-history run."""
+        out = np.zeros(n, dtype=DIGEST_DTYPE)
+        self._check(lib().vpmc_digests(self._h, C.byref(sc) if sc is not None else None, int(n_histories), int(seed),
+                                       int(hid_begin), int(n), out.ctypes.data))
+        return out
+
+    def set_knob(self, knob: int, value: float):
+        self._check(lib().vpmc_set_knob(self._h, int(knob), float(value)))
 
     def set_workspace_limit(self, nbytes: int):
         self._check(lib().vpmc_set_workspace_limit(self._h, int(nbytes)))

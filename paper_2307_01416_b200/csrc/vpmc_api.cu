@@ -33,7 +33,6 @@ static thread_local std::string g_create_err;
 
 static constexpr size_t kMaxSmemLut = 16 * 1024;      // larger material tables are read through L1 instead: a 64 KB table in
                                                       // shared memory costs the voxel kernel its fourth CTA per SM (measured +1-2.5 %)
-static unsigned long long kChunk = 1ull << 23;             // work items per pass of the pipeline = queue capacity (VPMC_CHUNK overrides)
 
 // grow-only device buffer
 static int ensure(vpmc_t *h, DevBuf &b, size_t bytes);
@@ -41,18 +40,21 @@ static int ensure(vpmc_t *h, DevBuf &b, size_t bytes);
 // Process-wide cache of released device buffers: engines are created and destroyed per plan (bench.py's e2e leg does
 // exactly that), and cudaMalloc / cudaFree of the ~1 GB of record queues would otherwise dominate a 10 ms dose.
 namespace {
-struct PoolEntry { void *p; size_t bytes; };
+struct PoolEntry { void *p; size_t bytes; int device; };
 std::mutex g_pool_mu;
 std::vector<PoolEntry> g_pool;
 size_t g_pool_bytes = 0;
 constexpr size_t kPoolLimit = (size_t)6 << 30;
 
+int current_device() { int d = 0; cudaGetDevice(&d); return d; }
+
 void *pool_take(size_t want, size_t &got)
 {
+    const int dev = current_device();
     std::lock_guard<std::mutex> lk(g_pool_mu);
     int best = -1;
     for (int i = 0; i < (int)g_pool.size(); ++i)
-        if (g_pool[i].bytes >= want && g_pool[i].bytes <= 2 * want + 4096 && (best < 0 || g_pool[i].bytes < g_pool[best].bytes)) best = i;
+        if (g_pool[i].device == dev && g_pool[i].bytes >= want && g_pool[i].bytes <= 2 * want + 4096 && (best < 0 || g_pool[i].bytes < g_pool[best].bytes)) best = i;
     if (best < 0) return nullptr;
     void *p = g_pool[best].p; got = g_pool[best].bytes;
     g_pool_bytes -= got;
@@ -63,10 +65,10 @@ void *pool_take(size_t want, size_t &got)
 void pool_give(void *p, size_t bytes)
 {
     if (!p) return;
-    static const bool off = getenv("VPMC_NO_POOL") != nullptr;
-    if (!off) {
+    {
+        const int dev = current_device();
         std::lock_guard<std::mutex> lk(g_pool_mu);
-        if (bytes >= 4096 && g_pool_bytes + bytes <= kPoolLimit && g_pool.size() < 256) { g_pool.push_back({ p, bytes }); g_pool_bytes += bytes; return; }
+        if (bytes >= 4096 && g_pool_bytes + bytes <= kPoolLimit && g_pool.size() < 256) { g_pool.push_back({ p, bytes, dev }); g_pool_bytes += bytes; return; }
     }
     cudaFree(p);
 }
@@ -144,6 +146,12 @@ extern "C" int vpmc_destroy(vpmc_t *h)
 {
     if (!h) return VPMC_OK;
     cudaDeviceSynchronize();
+    if (h->seq_exec) cudaGraphExecDestroy(h->seq_exec);
+    if (h->seq_graph) cudaGraphDestroy(h->seq_graph);
+    if (h->seq_ev_in) cudaEventDestroy(h->seq_ev_in);
+    if (h->seq_ev_out) cudaEventDestroy(h->seq_ev_out);
+    if (h->seq_stream) cudaStreamDestroy(h->seq_stream);
+    if (h->d_seq) cudaFree(h->d_seq);
     for (auto &b : h->beams) free_beam(b);
     void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_qctr, h->d_s1, h->d_s2, h->d_fb,
                      h->d_tal, h->d_tal_scratch, h->d_max_bits, h->d_unc };
@@ -218,8 +226,6 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     // persistent kernels: one wave of resident CTAs each
     {
         h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
-        if (const char *e = getenv("VPMC_LUT")) { if (!strcmp(e, "global")) h->smem_lut = false; }
-        if (const char *e = getenv("VPMC_CHUNK")) { const long long v = atoll(e); if (v >= 1024 && v <= (1ll << 30)) kChunk = (unsigned long long)v; }
         // occupancy queries are ~0.3 ms each: remember the answer per (device, table size, table placement)
         struct GridCache { int device; size_t lut_bytes; bool smem; int grid_beam; int grid[3][2]; };
         static std::mutex mu;
@@ -412,6 +418,31 @@ extern "C" int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out
         cudaEventDestroy(t.a); cudaEventDestroy(t.b);
     }
     h->timed.clear();
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_knob(vpmc_t *h, int knob, double value)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    switch (knob) {
+    case VPMC_KNOB_CHUNK:
+        if (!(value >= 1024.0 && value <= 1073741824.0)) FAIL(h, VPMC_ERR_INVALID_ARG, "chunk must be in [2^10, 2^30]");
+        h->chunk = (unsigned long long)value; break;
+    case VPMC_KNOB_BOX_GROW:
+        if (!(value >= 0.0 && value <= 4.0)) FAIL(h, VPMC_ERR_INVALID_ARG, "box growth must be in [0, 4]");
+        h->box_grow = (float)value; break;
+    case VPMC_KNOB_BOX_PAD:
+        if (!(value >= 0.0 && value <= 1024.0)) FAIL(h, VPMC_ERR_INVALID_ARG, "box padding must be in [0, 1024]");
+        h->box_pad = (int)value; break;
+    case VPMC_KNOB_OVF_CAP:
+        if (!(value >= 0.0 && value <= 268435456.0)) FAIL(h, VPMC_ERR_INVALID_ARG, "overflow capacity must be in [0, 2^28]");
+        h->ovf_cap = (unsigned int)value; break;
+    case VPMC_KNOB_LUT_GLOBAL:
+        h->smem_lut = (value == 0.0) && h->lut_bytes <= kMaxSmemLut; break;
+    case VPMC_KNOB_VERBOSE:
+        h->verbose = value != 0.0; break;
+    default: FAIL(h, VPMC_ERR_INVALID_ARG, "unknown knob %d", knob);
+    }
     return VPMC_OK;
 }
 

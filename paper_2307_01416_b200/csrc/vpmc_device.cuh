@@ -196,7 +196,9 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     const float lim = fmaxf(P.f_R * R, P.R_cut) * m.inv_rsp;
     if (lim < s) { s = lim; face = 0; }
     if (P.s_max < s) { s = P.s_max; face = 0; }
-    const double Rp = fma(-(double)s, (double)m.rsp, h.R);
+    // R' >= 0 by construction (C4-2), but inv_rsp is a rounded reciprocal: when the step is the R_cut limit and R is within
+    // an ulp of R_cut, s * rsp can exceed R by 1e-7.  Clamped, so that the logarithm below never sees a negative range.
+    const double Rp = fmax(fma(-(double)s, (double)m.rsp, h.R), 0.0);
     // E is re-derived from the fp64 range every step, so a 3e-7 relative MUFU error does not accumulate
     const float Ebar = exp2f(P.inv_p * __log2f((float)Rp * P.inv_alpha));
     // mean energy lost in the step.  E - Ebar cancels when the step is thin in water-equivalent terms (1 mm of air
@@ -226,6 +228,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
             if (fabsf(dl) < 0.05f) g1 = dl * fmaf(dl, fmaf(dl, fmaf(dl, fmaf(dl, P.pc5, P.pc4), P.pc3), P.pc2), P.p);
             else g1 = expm1f(P.p * log1pf(dl));
             Rn = fma(Rp, (double)g1, Rp);
+            if (!(Rp > 0.0)) Rn = (double)(P.alpha * exp2f(P.p * __log2f(Ep)));      // R' clamped to 0 (Ebar = 0): alpha E'^p directly
         }
     }
     // 5

@@ -63,11 +63,26 @@ struct vpmc {
     double *d_unc = nullptr;          // [0] sum, [1] count
     bool unc_valid = false;
 
+    // sequential stopping rule (vpmc_dose_to_uncertainty)
+    vpk::SeqState *d_seq = nullptr;
+    cudaStream_t seq_stream = nullptr;    // capture needs a non-default stream
+    cudaEvent_t seq_ev_in = nullptr, seq_ev_out = nullptr;
+    cudaGraph_t seq_graph = nullptr;
+    cudaGraphExec_t seq_exec = nullptr;
+    bool seq_valid = false;
+
     // influence workspace (grown on demand)
     DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_skip, inf_tilecnt, inf_colmax,
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
         ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
     size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
+
+    // knobs (vpmc_set_knob)
+    unsigned long long chunk = 1ull << 23;   // work items per pass of the pipeline = queue capacity
+    float box_grow = 0.05f;           // influence: growth of the pilot box, fraction of its extent
+    int box_pad = 1;                  // influence: extra voxels per side
+    unsigned int ovf_cap = 1u << 25;  // influence: entries of the overflow list (12 B each)
+    bool verbose = false;
 
     // launch configuration
     int grid_beam = 0;                // resident CTAs of beam_kernel

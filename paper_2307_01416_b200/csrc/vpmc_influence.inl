@@ -2,7 +2,7 @@
 //
 // Per scenario:
 //   1. pilot: the first n_pilot histories of every spot run in MODE 2 and leave the bounding box of their deposits;
-//   2. boxes: the pilot box of each column, grown by kGrow of its extent + kPad voxels per side, clipped to the grid
+//   2. boxes: the pilot box of each column, grown by box_grow of its extent + box_pad voxels per side, clipped to the grid
 //      (tight on purpose: the overflow list of step 4 takes the halo, and every box element is zeroed and scanned);
 //   3. columns are packed into groups whose boxes fit the workspace; per group: zero the boxes, transport all
 //      hist_per_spot histories of the group's spots in MODE 1, then max / count / scan / emit into a staging area;
@@ -13,12 +13,6 @@
 //      now fits by construction;
 //   5. row_ptr = exclusive scan of the row counts; the caller's allocator provides row_ptr / col / val and the rows are
 //      gathered from the staging area.
-
-static constexpr float kGrow = 0.05f;
-static constexpr int kPad = 1;
-// test knobs: VPMC_BOX_GROW / VPMC_BOX_PAD override the two constants (e.g. 0 / 0 forces the replay path)
-static float box_grow() { const char *e = getenv("VPMC_BOX_GROW"); return e ? (float)atof(e) : kGrow; }
-static int box_pad() { const char *e = getenv("VPMC_BOX_PAD"); return e ? atoi(e) : kPad; }
 
 struct HostBox { int lo[3], dim[3]; long long vol() const { return (long long)dim[0] * dim[1] * dim[2]; } };
 
@@ -119,13 +113,13 @@ extern "C" int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes)
     return VPMC_OK;
 }
 
-static HostBox grown_box(const int bb[6], const DevGrid &G)
+static HostBox grown_box(const int bb[6], const DevGrid &G, float grow, int pad_vox)
 {
     HostBox b;
     const int n[3] = { G.nx, G.ny, G.nz };
     for (int a = 0; a < 3; ++a) {
         const int ext = bb[3 + a] - bb[a] + 1;
-        const int pad = (int)std::ceil(box_grow() * (float)ext) + box_pad();
+        const int pad = (int)std::ceil(grow * (float)ext) + pad_vox;
         const int lo = std::max(bb[a] - pad, 0), hi = std::min(bb[3 + a] + pad, n[a] - 1);
         b.lo[a] = lo; b.dim[a] = hi - lo + 1;
     }
@@ -153,8 +147,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef = (float)(1.0 / (double)hist_per_spot / V * 1.602176634e-10);          // C6: scale 1 / hist_per_spot
     const uint32_t n_pilot = std::min<uint32_t>(hist_per_spot, std::max<uint32_t>(32u, hist_per_spot / 32u));
-    unsigned int ovf_cap = 1u << 25;          // entries of the overflow list (12 B each); VPMC_OVF_CAP overrides (0 forces replays)
-    if (const char *e = getenv("VPMC_OVF_CAP")) ovf_cap = (unsigned int)std::min<long long>(std::max<long long>(atoll(e), 0), 1ll << 28);
+    const unsigned int ovf_cap = h->ovf_cap;  // entries of the overflow list (12 B each); 0 forces replays
 
     for (int s = 0; s < n_sc; ++s) {
         const vpmc_scenario sc = scs[s];
@@ -181,7 +174,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         std::vector<HostBox> box(ns);
         for (int g = 0; g < ns; ++g) {
             if (bb[6 * g + 3] < 0) { for (int a = 0; a < 3; ++a) { box[g].lo[a] = 0; box[g].dim[a] = 1; } }   // pilot deposited nothing
-            else box[g] = grown_box(&bb[6 * g], h->G);
+            else box[g] = grown_box(&bb[6 * g], h->G, h->box_grow, h->box_pad);
         }
         // ---- 3./4. groups, with replay of the columns that outgrew their box
         std::vector<long long> row_nnz(ns, 0), row_src(ns, 0), row_ovf_off(ns, 0);
@@ -307,7 +300,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     h->launches += 1;
                     ostaged += oadd;
                 }
-                if (getenv("VPMC_DEBUG")) fprintf(stderr, "[vpmc]   group of %d columns: %u outside deposits, %lld kept entries of them, %lld box entries\n", nc, n_ovf, oadd, add);
+                if (h->verbose) fprintf(stderr, "[vpmc]   group of %d columns: %u outside deposits, %lld kept entries of them, %lld box entries\n", nc, n_ovf, oadd, add);
                 if (add > 0) {
                     if ((rc = grow_keep(h, h->inf_stage_idx, (size_t)(staged + add) * sizeof(int), (size_t)staged * sizeof(int), st)) ||
                         (rc = grow_keep(h, h->inf_stage_val, (size_t)(staged + add) * sizeof(float), (size_t)staged * sizeof(float), st)) ||
@@ -321,7 +314,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     staged += add;
                 }
             }
-            if (getenv("VPMC_DEBUG")) fprintf(stderr, "[vpmc] influence scenario %d round %d: %zu columns, %zu to replay\n", s, round, todo.size(), next.size());
+            if (h->verbose) fprintf(stderr, "[vpmc] influence scenario %d round %d: %zu columns, %zu to replay\n", s, round, todo.size(), next.size());
             todo.swap(next);
             replay = true;
         }

@@ -24,6 +24,8 @@ struct WorkMap {
     unsigned int hps, n_sub;
     const int *cols;
     int g0;
+    // sequential batches (vpmc_dose_to_uncertainty): the high word of every history id = *batch_hi (D:R15); NULL = 0
+    const unsigned int *batch_hi;
 };
 
 // influence-mode scoring target (S7): per-column private box in CT index space
@@ -62,6 +64,7 @@ __device__ __forceinline__ void map_item(const WorkMap &wm, unsigned long long k
         col = lo / wm.n_spots;                   // batch
         g = lo - col * wm.n_spots;
         hid = __ldg(wm.first + lo) + (k - __ldg(wm.cum + lo));
+        if (wm.batch_hi) hid |= (unsigned long long)(*wm.batch_hi) << 32;
     } else {
         const unsigned long long c = k / wm.n_sub;
         col = (int)c;
@@ -403,6 +406,28 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
 }
 
 // ------------------------------------------------------------------------------------------- trace (test-only)
+// one thread per selected history, from the source to its end through the SAME step functions as the production kernels;
+// records (RecTracer) or a digest (DigestTracer) per history
+template <class Tracer>
+__device__ __forceinline__ float trace_history(const Ctx &c, unsigned long long hid, int g, const float4 *spots, const double *spot_R0,
+                                               const int *spot_beam, const float4 *lut_g, Tracer &tr)
+{
+    Hist h; LaneCounters lc; NullScorer sc; NullSink sink;
+    float hdep = 0.0f;
+    h.col = 0;
+    h.hid_lo = (uint32_t)hid; h.hid_hi = (uint32_t)(hid >> 32);
+    const int beam = spot_beam[g];
+    sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.K);
+    int code = BEAM_CONT;
+    float dep_rs = 0.0f, dep_ap = 0.0f;
+    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, lc, tr);
+    if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
+        for (int it = 0; it < 1000000; ++it)
+            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr) != CONT) break;
+    }
+    return hdep;
+}
+
 __global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__ hids, const int *__restrict__ spot_of, int n,
                              const float4 *__restrict__ spots, const double *__restrict__ spot_R0,
                              const int *__restrict__ spot_beam, const float4 *__restrict__ lut_g,
@@ -413,21 +438,132 @@ __global__ void trace_kernel(const Ctx c, const unsigned long long *__restrict__
     RecTracer tr{ recs + (size_t)i * max_steps, max_steps, 0 };
     const int g = spot_of[i];
     if (g < 0) { nrec[i] = 0; return; }
-    Hist h; LaneCounters lc; NullScorer sc; NullSink sink;
-    float hdep = 0.0f;
-    h.col = 0;
-    h.hid_lo = (uint32_t)hids[i]; h.hid_hi = (uint32_t)(hids[i] >> 32);
-    const int beam = spot_beam[g];
-    sample_source(c.P, c.beams[beam], beam, spots[g], spot_R0[g], h, c.K);
-    int code = BEAM_CONT;
-    float dep_rs = 0.0f, dep_ap = 0.0f;
-    for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, lc, tr);
-    if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
-        hdep = 0.0f;
-        for (int it = 0; it < 1000000; ++it)
-            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr) != CONT) break;
-    }
+    trace_history(c, hids[i], g, spots, spot_R0, spot_beam, lut_g, tr);
     nrec[i] = tr.n;
+}
+
+// digests of the contiguous history ids [hid0, hid0 + n) of a dose-mode run: spot by search in the id prefix `start`
+__global__ void digest_kernel(const Ctx c, unsigned long long hid0, int n, const unsigned long long *__restrict__ start, int n_spots,
+                              const float4 *__restrict__ spots, const double *__restrict__ spot_R0,
+                              const int *__restrict__ spot_beam, const float4 *__restrict__ lut_g, Digest *__restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const unsigned long long hid = hid0 + (unsigned long long)i;
+    int lo = 0, hi = n_spots;                    // largest g with start[g] <= hid (empty spots are skipped by the search)
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (start[mid] <= hid) lo = mid; else hi = mid; }
+    DigestTracer tr;
+    tr.start(hid);
+    tr.d.dep_ct = trace_history(c, hid, lo, spots, spot_R0, spot_beam, lut_g, tr);
+    out[i] = tr.d;
+}
+
+// ------------------------------------------------------------------------------------------- one step from a state (test-only)
+struct StateIn {    // == vpmc_state
+    unsigned long long hid;
+    int kind, step, beam, spot;
+    int ivox[3];
+    int pad_;
+    double r[3], u[3];
+    double E, t_rad, tau, tau_star;
+};
+struct StateOut {   // == vpmc_state_out
+    int region, cause, step_after, n_steps;
+    int ivox_after[3];
+    int pad_;
+    double r[3], u[3];
+    double E, R, s, dep, t_rad, tau, tau_star;
+};
+enum : int { STEP_SOURCE = 0, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT };
+
+// Runs the SAME step functions as the production kernels (sample_source, drift_gap, beam_step, ct_entry, ct_step) once,
+// from a state given in fp64 and converted to the kernel's own representation (fp64 range from E, hi + lo direction and
+// beam-frame position, voxel + local offset).
+__global__ void step_state_kernel(const Ctx c, const StateIn *__restrict__ in, int n, const float4 *__restrict__ spots,
+                                  const double *__restrict__ spot_R0, const float4 *__restrict__ lut_g, StateOut *__restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const StateIn q = in[i];
+    const DevBeam &b = c.beams[q.beam];
+    const DevGrid &G = c.G;
+    StepRec rec;
+    RecTracer tr{ &rec, 1, 0 };
+    Hist h; LaneCounters lc; NullScorer sc; NullSink sink;
+    StateOut o;
+    memset(&o, 0, sizeof(o));
+    h.col = 0;
+    h.hid_lo = (uint32_t)q.hid; h.hid_hi = (uint32_t)(q.hid >> 32);
+    if (q.kind == STEP_SOURCE) {
+        sample_source(c.P, b, q.beam, spots[q.spot], spot_R0[q.spot], h, c.K);
+        o.region = REG_VAC; o.cause = CONT;
+        o.r[0] = beam_x(h); o.r[1] = beam_y(h); o.r[2] = (double)b.w_start;
+        o.u[2] = 1.0;
+        o.E = (double)h.E; o.R = h.R; o.tau_star = (double)h.tau_star;
+        out[i] = o;
+        return;
+    }
+    h.E = (float)q.E;
+    h.R = (double)c.P.alpha * pow(q.E, (double)c.P.p);
+    h.t_rad = (float)q.t_rad; h.f_rad = highland_f(h.t_rad, c.P.c_log);
+    h.tau = (float)q.tau; h.tau_star = (float)q.tau_star;
+    h.step = (uint32_t)q.step;
+    h.ux = (float)q.u[0]; h.uy = (float)q.u[1]; h.uz = (float)q.u[2];
+    h.lx = (float)(q.u[0] - (double)h.ux); h.ly = (float)(q.u[1] - (double)h.uy); h.lz = (float)(q.u[2] - (double)h.uz);
+    h.rx = h.ry = h.rz = 0.0f;
+    float dep_rs = 0.0f, dep_ap = 0.0f, hdep = 0.0f;
+    if (q.kind != STEP_CT) { set_beam_x(h, q.r[0]); set_beam_y(h, q.r[1]); }
+    if (q.kind == STEP_DRIFT_TO_RS || q.kind == STEP_DRIFT_TO_AP) {
+        const bool rs = q.kind == STEP_DRIFT_TO_RS;
+        const float w1 = rs ? b.w_rs_in : b.w_ap_in;
+        const float w0 = rs ? b.w_start : (b.has_rs ? b.w_rs_out : b.w_start);
+        h.region = (rs ? REG_TO_RS : REG_TO_AP) | (q.beam << 8);
+        const int cause = drift_gap(h, w1 - w0, w1, tr);
+        if (cause != CONT) { rec.region = REG_VAC; rec.cause = ESCAPED; rec.s = 0.0f; tr.n = 1; }
+        o.r[0] = beam_x(h); o.r[1] = beam_y(h); o.r[2] = (cause == CONT) ? (double)w1 : q.r[2];
+    } else if (q.kind == STEP_RS || q.kind == STEP_AP) {
+        const bool rs = q.kind == STEP_RS;
+        const float w_in = rs ? b.w_rs_in : b.w_ap_in;
+        h.region = (rs ? REG_RS : REG_AP) | (q.beam << 8);
+        h.rz = (float)(q.r[2] - (double)w_in);
+        beam_step(c, h, dep_rs, dep_ap, lc, tr);
+        if (tr.n == 1) { o.r[0] = beam_x(h); o.r[1] = beam_y(h); o.r[2] = (double)w_in + (double)h.rz; }
+        else { o.r[0] = (double)rec.r[0]; o.r[1] = (double)rec.r[1]; o.r[2] = (double)rec.r[2]; }
+    } else if (q.kind == STEP_CT_ENTRY) {
+        h.region = REG_TO_CT | (q.beam << 8);
+        ct_entry(c, h, lc, sink, tr);
+    } else {
+        h.region = REG_CT | (q.beam << 8);
+        const double lo[3] = { (double)G.ox, (double)G.oy, (double)G.oz }, hh[3] = { (double)G.hx, (double)G.hy, (double)G.hz };
+        float l[3];
+        for (int a = 0; a < 3; ++a) l[a] = (float)fmin(fmax(q.r[a] - fma((double)q.ivox[a], hh[a], lo[a]), 0.0), hh[a]);
+        h.rx = l[0]; h.ry = l[1]; h.rz = l[2];
+        h.g0 = (uint32_t)q.ivox[0]; h.g1 = (uint32_t)q.ivox[1]; h.g2 = (uint32_t)q.ivox[2];
+        h.g3 = (uint32_t)(q.ivox[0] + G.nx * (q.ivox[1] + G.ny * q.ivox[2]));
+        ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
+    }
+    if (q.kind == STEP_CT_ENTRY || q.kind == STEP_CT) {
+        o.ivox_after[0] = (int)h.g0; o.ivox_after[1] = (int)h.g1; o.ivox_after[2] = (int)h.g2;
+        if (rec.cause == ESCAPED && q.kind == STEP_CT_ENTRY) { o.r[0] = (double)rec.r[0]; o.r[1] = (double)rec.r[1]; o.r[2] = (double)rec.r[2]; }
+        else {
+            o.r[0] = fma((double)(int)h.g0, (double)G.hx, (double)G.ox) + (double)h.rx;
+            o.r[1] = fma((double)(int)h.g1, (double)G.hy, (double)G.oy) + (double)h.ry;
+            o.r[2] = fma((double)(int)h.g2, (double)G.hz, (double)G.oz) + (double)h.rz;
+        }
+    }
+    o.region = rec.region; o.cause = rec.cause; o.n_steps = tr.n; o.s = (double)rec.s;
+    const bool one = tr.n == 1;
+    o.step_after = one ? (int)h.step : q.step + 1;
+    o.u[0] = one ? (double)h.ux + (double)h.lx : q.u[0];
+    o.u[1] = one ? (double)h.uy + (double)h.ly : q.u[1];
+    o.u[2] = one ? (double)h.uz + (double)h.lz : q.u[2];
+    o.E = one ? (double)h.E : q.E;
+    o.R = h.R;
+    o.dep = (double)(dep_rs + dep_ap + hdep);
+    o.t_rad = one ? (double)h.t_rad : q.t_rad;
+    o.tau = one ? (double)h.tau : q.tau;
+    o.tau_star = (double)h.tau_star;
+    out[i] = o;
 }
 
 // ------------------------------------------------------------------------------------------- S6 / C6
@@ -482,6 +618,82 @@ __global__ void uncertainty_kernel(const float *__restrict__ dose, const float *
     }
     s = warp_sum(s); c = warp_sum(c);
     if ((threadIdx.x & 31) == 0 && c > 0.0) { atomicAdd(acc, s); atomicAdd(acc + 1, c); }
+}
+
+// ------------------------------------------------------------------------------------------- S:8f-3: on-GPU stopping rule
+// Sequential batches (SURVEY.md 8(d) metric 2, "<0.5 %"): after every batch the C6 estimator over the batches so
+// far decides on the DEVICE whether another batch runs -- the batch pass is the body of a CUDA-graph WHILE node whose
+// condition seq_decide_kernel sets, so the host enqueues one graph and never looks at intermediate results.
+// With equal batches the estimator needs only s1 = sum_b E_b and s2 = sum_b E_b^2 per voxel.
+struct SeqState {
+    unsigned int batch;        // batches finished so far = index of the batch in flight
+    unsigned int max_bits;     // bits of max_v s1[v] (monotone: s1 only grows)
+    float unc;                 // estimate after the last finished batch (0 while < 2 batches)
+    unsigned int stopped_by_target;
+    double acc[2];             // sum of sigma_v / mean_v, number of voxels
+};
+
+__global__ void seq_accumulate_kernel(float *__restrict__ edep, float *__restrict__ s1, float *__restrict__ s2, long long n, SeqState *st)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    float mx = 0.0f;
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        const float e = edep[v];
+        if (e != 0.0f) { edep[v] = 0.0f; s2[v] = fmaf(e, e, s2[v]); }
+        const float a = s1[v] + e;
+        if (e != 0.0f) s1[v] = a;
+        mx = fmaxf(mx, a);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0 && mx > 0.0f) atomicMax(&st->max_bits, __float_as_uint(mx));
+}
+
+// C6 over the B = st->batch + 1 batches finished once this pass runs: mean over voxels with s1 >= 0.5 max of sigma_v / mean_v
+__global__ void seq_uncertainty_kernel(const float *__restrict__ s1, const float *__restrict__ s2, long long n, SeqState *st)
+{
+    const int B = (int)st->batch + 1;
+    if (B < 2) return;
+    const float half_max = 0.5f * __uint_as_float(st->max_bits);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double s = 0.0, c = 0.0;
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        const float a1 = s1[v];
+        if (a1 >= half_max && a1 > 0.0f) {
+            const double a = (double)a1, b = (double)s2[v];
+            double var = (b - a * a / B) / ((double)B * (B - 1));
+            if (var < 0.0) var = 0.0;
+            s += sqrt(var) / (a / B);
+            c += 1.0;
+        }
+    }
+    s = warp_sum(s); c = warp_sum(c);
+    if ((threadIdx.x & 31) == 0 && c > 0.0) { atomicAdd(&st->acc[0], s); atomicAdd(&st->acc[1], c); }
+}
+
+// one thread: close the batch, decide whether the WHILE node runs its body again
+__global__ void seq_decide_kernel(cudaGraphConditionalHandle handle, SeqState *st, int min_batches, int max_batches, float target)
+{
+    const int B = (int)(st->batch += 1u);
+    const float unc = (B >= 2 && st->acc[1] > 0.0) ? (float)(st->acc[0] / st->acc[1]) : 0.0f;
+    st->unc = unc;
+    st->acc[0] = 0.0; st->acc[1] = 0.0;
+    const bool reached = B >= 2 && B >= min_batches && st->max_bits != 0u && unc <= target;
+    st->stopped_by_target = reached ? 1u : 0u;
+    cudaGraphSetConditional(handle, (reached || B >= max_batches) ? 0u : 1u);
+}
+
+// dose[v] = coef_batch / B * s1[v] / max(rho_v, rho_min), coef_batch = (W / N_b) / V * 1.602e-10 (C6 with N = B N_b)
+__global__ void seq_finalize_kernel(const float *__restrict__ s1, const short *__restrict__ hu, const float4 *__restrict__ lut, DevGrid G,
+                                    float rho_min, float coef_batch, const SeqState *st, float *__restrict__ dose, long long n)
+{
+    const float coef = coef_batch / (float)max(st->batch, 1u);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        int t = (int)__ldg(hu + v) - G.hu_min;
+        t = min(max(t, 0), G.n_lut - 1);
+        dose[v] = __fdiv_rn(coef * s1[v], fmaxf(__ldg(lut + t).y, rho_min));
+    }
 }
 
 // ------------------------------------------------------------------------------------------- S8: CSR writer

@@ -110,13 +110,13 @@ static Ctx make_ctx(const vpmc_t *h, const vpmc_scenario &sc, uint64_t seed)
     return c;
 }
 
-// the hot path over wm.n_items work items, in chunks of kChunk: source (S1) -> beam line (S2-S3) -> CT entry -> voxel
+// the hot path over wm.n_items work items, in chunks of h->chunk: source (S1) -> beam line (S2-S3) -> CT entry -> voxel
 // stepping + scoring (S4-S7)
 template <int MODE>
 static int launch_transport(vpmc_t *h, const Ctx &c, const WorkMap &wm0, const ScoreArgs &sa, DevTallies *tal, cudaStream_t st)
 {
     if (wm0.n_items == 0) return VPMC_OK;
-    const unsigned long long cap = std::min<unsigned long long>(wm0.n_items, kChunk);
+    const unsigned long long cap = std::min<unsigned long long>(wm0.n_items, h->chunk);
     int rc;
     if ((rc = ensure(h, h->s0, cap * sizeof(uint4))) || (rc = ensure(h, h->s1, cap * sizeof(uint4))) || (rc = ensure(h, h->s2, cap * sizeof(uint4))) ||
         (rc = ensure(h, h->q0, cap * sizeof(uint4))) || (rc = ensure(h, h->q1, cap * sizeof(float4))) || (rc = ensure(h, h->q2, cap * sizeof(float4))) ||
@@ -126,9 +126,9 @@ static int launch_transport(vpmc_t *h, const Ctx &c, const WorkMap &wm0, const S
     Queue q;
     q.q0 = h->q0.as<uint4>(); q.q1 = h->q1.as<float4>(); q.q2 = h->q2.as<float4>(); q.q3 = h->q3.as<uint4>(); q.q4 = h->q4.as<uint4>();
     q.count = h->d_qctr; q.head = h->d_qctr + 1; q.capacity = (unsigned int)cap;
-    for (unsigned long long i0 = 0; i0 < wm0.n_items; i0 += kChunk) {
+    for (unsigned long long i0 = 0; i0 < wm0.n_items; i0 += h->chunk) {
         WorkMap wm = wm0;
-        wm.n_items = std::min<unsigned long long>(kChunk, wm0.n_items - i0);
+        wm.n_items = std::min<unsigned long long>(h->chunk, wm0.n_items - i0);
         const unsigned int n = (unsigned int)wm.n_items;
         const int blocks = (int)((n + kBlock - 1) / kBlock);
         CU(h, cudaMemsetAsync(h->d_qctr, 0, 4 * sizeof(unsigned int), st));
@@ -251,6 +251,128 @@ extern "C" int vpmc_dose_host(vpmc_t *h, uint64_t n_histories, uint64_t seed, fl
     return rc;
 }
 
+// ---- S:8f-3: dose to a statistical uncertainty, stopping rule on the device (CUDA-graph WHILE node)
+static void seq_release(vpmc_t *h)
+{
+    if (h->seq_exec) { cudaGraphExecDestroy(h->seq_exec); h->seq_exec = nullptr; }
+    if (h->seq_graph) { cudaGraphDestroy(h->seq_graph); h->seq_graph = nullptr; }
+}
+
+extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uint64_t batch_histories, int32_t min_batches,
+                                        int32_t max_batches, float target_rel_unc, uint64_t seed, float *dose_out_dev, void *cuda_stream)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!dose_out_dev || batch_histories < 1 || batch_histories > h->chunk || batch_histories >= (1ull << 32) || max_batches < 1 ||
+        min_batches < 0 || !(target_rel_unc >= 0.0f))
+        FAIL(h, VPMC_ERR_INVALID_ARG, "bad dose_to_uncertainty arguments (batch_histories must be in [1, chunk = %llu])", h->chunk);
+    const vpmc_scenario sc = scp ? *scp : vpmc_scenario{ { 0, 0, 0 }, 1.0f };
+    if (!(sc.rsp_scale > 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "rsp_scale must be positive");
+    cudaStream_t caller = (cudaStream_t)cuda_stream;
+    if (!h->seq_stream) {
+        CU(h, cudaStreamCreateWithFlags(&h->seq_stream, cudaStreamNonBlocking));
+        CU(h, cudaEventCreateWithFlags(&h->seq_ev_in, cudaEventDisableTiming));
+        CU(h, cudaEventCreateWithFlags(&h->seq_ev_out, cudaEventDisableTiming));
+        CU(h, cudaMalloc(&h->d_seq, sizeof(SeqState)));
+    }
+    cudaStream_t st = h->seq_stream;
+    CU(h, cudaStreamSynchronize(st));        // a previous graph of this handle must have drained before it is rebuilt
+    seq_release(h);
+    CU(h, cudaEventRecord(h->seq_ev_in, caller));
+    CU(h, cudaStreamWaitEvent(st, h->seq_ev_in, 0));
+    int rc = prepare_beams(h, sc, st); if (rc) return rc;
+    h->last_stream = caller;
+    h->unc_valid = false; h->seq_valid = false;
+    if (!h->d_s1) {
+        CU(h, cudaMalloc(&h->d_s1, h->nvox * sizeof(float)));
+        CU(h, cudaMalloc(&h->d_s2, h->nvox * sizeof(float)));
+    }
+    const unsigned long long cap = batch_histories;
+    if ((rc = ensure(h, h->edep, (size_t)h->nvox * sizeof(float))) ||
+        (rc = ensure(h, h->cum, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) || (rc = ensure(h, h->first, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) ||
+        (rc = ensure(h, h->s0, cap * sizeof(uint4))) || (rc = ensure(h, h->s1, cap * sizeof(uint4))) || (rc = ensure(h, h->s2, cap * sizeof(uint4))) ||
+        (rc = ensure(h, h->q0, cap * sizeof(uint4))) || (rc = ensure(h, h->q1, cap * sizeof(float4))) || (rc = ensure(h, h->q2, cap * sizeof(float4))) ||
+        (rc = ensure(h, h->q3, cap * sizeof(uint4))) || (rc = ensure(h, h->q4, cap * sizeof(uint4)))) return rc;
+    // C2 for one batch: ids i in [0, N_b) contiguous per spot in spot order (the batch index goes into the id's high word)
+    std::vector<unsigned long long> cnt, cum(h->n_spots + 1, 0ull), first(h->n_spots + 1, 0ull);
+    apportion(batch_histories, h->spot_w, cnt);
+    for (int g = 0; g < h->n_spots; ++g) { first[g] = cum[g]; cum[g + 1] = cum[g] + cnt[g]; }
+    CU(h, cudaMemcpyAsync(h->cum.p, cum.data(), cum.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    CU(h, cudaMemcpyAsync(h->first.p, first.data(), first.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+    CU(h, cudaStreamSynchronize(st));        // cum / first are stack vectors
+    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_s1, 0, (size_t)h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_s2, 0, (size_t)h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
+    CU(h, cudaMemsetAsync(h->d_seq, 0, sizeof(SeqState), st));
+
+    const Ctx c = make_ctx(h, sc, seed);
+    WorkMap wm{};
+    wm.mode = 0; wm.n_items = batch_histories; wm.cum = h->cum.as<unsigned long long>(); wm.first = h->first.as<unsigned long long>();
+    wm.n_entries = h->n_spots; wm.n_spots = h->n_spots; wm.batch_hi = &h->d_seq->batch;
+    ScoreArgs sa{};
+    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->nvox;
+    SourceBuf sb;
+    sb.s0 = h->s0.as<uint4>(); sb.s1 = h->s1.as<uint4>(); sb.s2 = h->s2.as<uint4>();
+    Queue q;
+    q.q0 = h->q0.as<uint4>(); q.q1 = h->q1.as<float4>(); q.q2 = h->q2.as<float4>(); q.q3 = h->q3.as<uint4>(); q.q4 = h->q4.as<uint4>();
+    q.count = h->d_qctr; q.head = h->d_qctr + 1; q.capacity = (unsigned int)cap;
+    const unsigned int n = (unsigned int)batch_histories;
+    const int blocks = (int)((n + kBlock - 1) / kBlock);
+    const int gv = grid_for(h->nvox, h->n_sm);
+
+    // the graph: one WHILE node whose body is the batch pass
+    CU(h, cudaGraphCreate(&h->seq_graph, 0));
+    cudaGraphConditionalHandle handle;
+    CU(h, cudaGraphConditionalHandleCreate(&handle, h->seq_graph, 1, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams np = { cudaGraphNodeTypeConditional };
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CU(h, cudaGraphAddNode(&node, h->seq_graph, nullptr, 0, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    CU(h, cudaStreamBeginCaptureToGraph(st, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    cudaMemsetAsync(h->d_qctr, 0, 4 * sizeof(unsigned int), st);
+    source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, 0ull, h->d_spots, h->d_spot_R0, h->d_spot_beam, sb, h->d_tal);
+    beam_kernel<<<std::min(h->grid_beam, blocks), kBlock, 0, st>>>(c, n, sb, q, h->d_qctr + 2, h->d_tal);
+    entry_kernel<<<blocks, kBlock, 0, st>>>(c, q, h->d_tal);
+    if (h->smem_lut)
+        voxel_kernel<0, true><<<std::min(h->grid[0][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, q, h->d_lut, sa, h->d_tal);
+    else
+        voxel_kernel<0, false><<<std::min(h->grid[0][0], blocks), kBlock, h->tally_smem, st>>>(c, q, h->d_lut, sa, h->d_tal);
+    seq_accumulate_kernel<<<gv, 256, 0, st>>>(h->edep.as<float>(), h->d_s1, h->d_s2, h->nvox, h->d_seq);
+    seq_uncertainty_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_s2, h->nvox, h->d_seq);
+    seq_decide_kernel<<<1, 1, 0, st>>>(handle, h->d_seq, (int)min_batches, (int)max_batches, target_rel_unc);
+    cudaError_t ce = cudaStreamEndCapture(st, nullptr);
+    if (ce != cudaSuccess) { cudaGetLastError(); seq_release(h); FAIL(h, VPMC_ERR_CUDA, "graph capture of the batch pass: %s", cudaGetErrorString(ce)); }
+    CU(h, cudaGraphInstantiate(&h->seq_exec, h->seq_graph, 0));
+    CU(h, cudaGraphLaunch(h->seq_exec, st));
+    double W = 0.0;
+    for (double x : h->spot_w) W += x;
+    const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
+    const float coef_batch = (float)(W / (double)batch_histories / V * 1.602176634e-10);
+    seq_finalize_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef_batch, h->d_seq, dose_out_dev, h->nvox);
+    CU(h, cudaGetLastError());
+    CU(h, cudaEventRecord(h->seq_ev_out, st));
+    CU(h, cudaStreamWaitEvent(caller, h->seq_ev_out, 0));
+    h->seq_valid = true;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_get_run_info(vpmc_t *h, int32_t *batches_out, float *rel_unc_out, int32_t *reached_target_out)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!h->seq_valid) FAIL(h, VPMC_ERR_STATE, "no vpmc_dose_to_uncertainty run yet");
+    CU(h, cudaStreamSynchronize(h->seq_stream));
+    SeqState s;
+    CU(h, cudaMemcpy(&s, h->d_seq, sizeof(s), cudaMemcpyDeviceToHost));
+    if (h->seq_exec) { h->launches += 7ull * s.batch + 1ull; seq_release(h); }     // counted once, when the result is read
+    if (batches_out) *batches_out = (int32_t)s.batch;
+    if (rel_unc_out) *rel_unc_out = s.unc;
+    if (reached_target_out) *reached_target_out = (int32_t)s.stopped_by_target;
+    return VPMC_OK;
+}
+
 extern "C" int vpmc_get_tallies(vpmc_t *h, vpmc_tallies *out)
 {
     if (!h) return VPMC_ERR_INVALID_ARG;
@@ -317,6 +439,69 @@ extern "C" int vpmc_trace(vpmc_t *h, const vpmc_scenario *scp, int32_t mode, uin
     CT_(cudaMemcpy(nrec_host, d_n, n * sizeof(int), cudaMemcpyDeviceToHost));
 #undef CT_
     cleanup();
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_digests(vpmc_t *h, const vpmc_scenario *scp, uint64_t n_histories, uint64_t seed, uint64_t hid_begin, int32_t n,
+                            vpmc_digest *out_host)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (n < 0 || (n > 0 && !out_host) || hid_begin + (uint64_t)n > n_histories) FAIL(h, VPMC_ERR_INVALID_ARG, "bad digest arguments");
+    static_assert(sizeof(Digest) == sizeof(vpmc_digest), "digest layout");
+    const vpmc_scenario sc = scp ? *scp : vpmc_scenario{ { 0, 0, 0 }, 1.0f };
+    int rc = prepare_beams(h, sc, nullptr); if (rc) return rc;
+    if (n == 0) return VPMC_OK;
+    std::vector<unsigned long long> cnt, start(h->n_spots + 1, 0ull);
+    apportion(n_histories, h->spot_w, cnt);
+    for (int g = 0; g < h->n_spots; ++g) start[g + 1] = start[g] + cnt[g];
+    DevBuf dstart, dout;
+    if ((rc = ensure(h, dstart, start.size() * sizeof(unsigned long long))) || (rc = ensure(h, dout, (size_t)n * sizeof(Digest)))) { pool_give(dstart.p, dstart.bytes); return rc; }
+    cudaError_t e = cudaMemcpy(dstart.p, start.data(), start.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        digest_kernel<<<(n + 63) / 64, 64>>>(make_ctx(h, sc, seed), hid_begin, n, dstart.as<unsigned long long>(), h->n_spots, h->d_spots, h->d_spot_R0,
+                                             h->d_spot_beam, h->d_lut, dout.as<Digest>());
+        h->launches += 1;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(out_host, dout.p, (size_t)n * sizeof(Digest), cudaMemcpyDeviceToHost);
+    pool_give(dstart.p, dstart.bytes); pool_give(dout.p, dout.bytes);
+    if (e != cudaSuccess) FAIL(h, VPMC_ERR_CUDA, "digests: %s", cudaGetErrorString(e));
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_step_from_state(vpmc_t *h, const vpmc_scenario *scp, uint64_t seed, const vpmc_state *states, int32_t n,
+                                    vpmc_state_out *out)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (n < 0 || (n > 0 && (!states || !out))) FAIL(h, VPMC_ERR_INVALID_ARG, "bad step_from_state arguments");
+    static_assert(sizeof(StateIn) == sizeof(vpmc_state) && sizeof(StateOut) == sizeof(vpmc_state_out), "state layout");
+    const vpmc_scenario sc = scp ? *scp : vpmc_scenario{ { 0, 0, 0 }, 1.0f };
+    int rc = prepare_beams(h, sc, nullptr); if (rc) return rc;
+    if (n == 0) return VPMC_OK;
+    for (int i = 0; i < n; ++i) {
+        const vpmc_state &q = states[i];
+        if (q.kind < VPMC_STEP_SOURCE || q.kind > VPMC_STEP_CT || q.beam < 0 || q.beam >= (int)h->beams.size()) FAIL(h, VPMC_ERR_INVALID_ARG, "state %d: bad kind or beam", i);
+        if (q.kind == VPMC_STEP_SOURCE && (q.spot < 0 || q.spot >= h->n_spots || h->spot_beam_h[q.spot] != q.beam)) FAIL(h, VPMC_ERR_INVALID_ARG, "state %d: bad spot", i);
+        if (q.kind == VPMC_STEP_CT)
+            for (int a = 0; a < 3; ++a)
+                if (q.ivox[a] < 0 || q.ivox[a] >= (a == 0 ? h->G.nx : a == 1 ? h->G.ny : h->G.nz)) FAIL(h, VPMC_ERR_INVALID_ARG, "state %d: voxel outside the grid", i);
+        const BeamHost &b = h->beams[q.beam];
+        if (((q.kind == VPMC_STEP_DRIFT_TO_RS || q.kind == VPMC_STEP_RS) && !(b.rs_wet > 0.0f)) ||
+            ((q.kind == VPMC_STEP_DRIFT_TO_AP || q.kind == VPMC_STEP_AP) && !b.has_ap)) FAIL(h, VPMC_ERR_INVALID_ARG, "state %d: the beam has no such device", i);
+    }
+    DevBuf din, dout;
+    if ((rc = ensure(h, din, (size_t)n * sizeof(StateIn))) || (rc = ensure(h, dout, (size_t)n * sizeof(StateOut)))) { pool_give(din.p, din.bytes); return rc; }
+    cudaError_t e = cudaMemcpy(din.p, states, (size_t)n * sizeof(StateIn), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        step_state_kernel<<<(n + 63) / 64, 64>>>(make_ctx(h, sc, seed), din.as<StateIn>(), n, h->d_spots, h->d_spot_R0, h->d_lut, dout.as<StateOut>());
+        h->launches += 1;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout.p, (size_t)n * sizeof(StateOut), cudaMemcpyDeviceToHost);
+    pool_give(din.p, din.bytes); pool_give(dout.p, dout.bytes);
+    if (e != cudaSuccess) FAIL(h, VPMC_ERR_CUDA, "step_from_state: %s", cudaGetErrorString(e));
     return VPMC_OK;
 }
 

@@ -38,18 +38,19 @@ struct StepRec {   // == vpmc_step_rec
     int ivox[3];
     float r[3], u[3];
     float E_before, E_after, s;
+    float dep; int pad_;         // energy deposited in the step's cell (CT voxel, range shifter or brass tally), MeV
 };
 
 struct NullTracer {
     static constexpr bool on = false;
-    __device__ __forceinline__ void put(const Hist &, float, float, float, uint32_t, int, const int *, float, float, float, int) {}
+    __device__ __forceinline__ void put(const Hist &, float, float, float, uint32_t, int, const int *, float, float, float, int, float = 0.0f) {}
 };
 
 struct RecTracer {
     static constexpr bool on = true;
     StepRec *recs; int max, n;
     __device__ void put(const Hist &h, float x, float y, float z, uint32_t step, int region, const int *iv,
-                        float Eb, float Ea, float s, int cause)
+                        float Eb, float Ea, float s, int cause, float dep = 0.0f)
     {
         if (n < max) {
             StepRec &q = recs[n];
@@ -58,8 +59,31 @@ struct RecTracer {
             q.ivox[0] = iv ? iv[0] : -1; q.ivox[1] = iv ? iv[1] : -1; q.ivox[2] = iv ? iv[2] : -1;
             q.r[0] = x; q.r[1] = y; q.r[2] = z;
             q.u[0] = h.ux + h.lx; q.u[1] = h.uy + h.ly; q.u[2] = h.uz + h.lz;
-            q.E_before = Eb; q.E_after = Ea; q.s = s;
+            q.E_before = Eb; q.E_after = Ea; q.s = s; q.dep = dep; q.pad_ = 0;
         }
+        ++n;
+    }
+};
+
+// Per-history digest instead of step records (vpmc_digest, test-only): number of records, FNV-1a hash of the discrete
+// trace (region, cause, voxel indices of every record), state after the last record and the energy deposited in the CT.
+struct Digest {   // == vpmc_digest
+    unsigned long long hid, hash;
+    int n_rec, cause;
+    float r[3];
+    float E_last, dep_ct;
+    int pad_;
+};
+struct DigestTracer {
+    static constexpr bool on = true;
+    Digest d; int n;
+    __device__ void start(unsigned long long hid) { d.hid = hid; d.hash = 1469598103934665603ull; d.n_rec = 0; d.cause = 0; d.r[0] = d.r[1] = d.r[2] = 0.0f; d.E_last = 0.0f; d.dep_ct = 0.0f; d.pad_ = 0; n = 0; }
+    __device__ void mix(unsigned int v) { d.hash = (d.hash ^ (unsigned long long)v) * 1099511628211ull; }
+    __device__ void put(const Hist &, float x, float y, float z, uint32_t, int region, const int *iv, float, float Ea, float, int cause, float = 0.0f)
+    {
+        mix((unsigned)region); mix((unsigned)cause);
+        mix((unsigned)(iv ? iv[0] : -1)); mix((unsigned)(iv ? iv[1] : -1)); mix((unsigned)(iv ? iv[2] : -1));
+        d.n_rec += 1; d.cause = cause; d.r[0] = x; d.r[1] = y; d.r[2] = z; d.E_last = Ea;
         ++n;
     }
 };
@@ -314,7 +338,13 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
             // full steps left before the exit step; if all of their tests are known, go straight to the exit plane,
             // else take the known ones (at least one step) and test again.
             const float rem = T - h.rz, duz = P.s_ap * h.uz;
-            const int nf = ex ? 0 : max((int)ceilf(__fdiv_rn(rem, duz)) - 1, 0);
+            // nf = number of j >= 0 with rem - j duz > duz (the per-step rule `rem <= d u_w` decides the exit step); the
+            // rounded quotient can be off by one when rem / duz sits next to an integer, so it is checked against that rule
+            int nf = ex ? 0 : max((int)ceilf(__fdiv_rn(rem, duz)) - 1, 0);
+            if (!ex) {
+                if (fmaf(-(float)nf, duz, rem) > duz) nf += 1;
+                else if (nf > 0 && fmaf(-(float)(nf - 1), duz, rem) <= duz) nf -= 1;
+            }
             float n_safe = 0.0f;
             if (nf > 0) {
                 const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
@@ -377,7 +407,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
         lc.n_slab += (cause != STOPPED);
         const bool out = (cause == CONT) && o.on_d && ex;
         if (out) h.rz = T;
-        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause);
+        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause, o.dep);
         if (cause != CONT) status = (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
         else if (out) {
             reg = (reg == REG_RS && __ldg(&bp->has_ap)) ? REG_TO_AP : REG_TO_CT;
@@ -451,7 +481,7 @@ __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, fl
     if (cause == CONT && o.on_d && cross_face(G, h, ax, up)) cause = ESCAPED;
     lc.n_ct += (cause != STOPPED);
     if (Tracer::on) tr.put(h, fmaf((float)(int)h.g0, G.hx, G.ox) + h.rx, fmaf((float)(int)h.g1, G.hy, G.oy) + h.ry,
-                           fmaf((float)(int)h.g2, G.hz, G.oz) + h.rz, st, REG_CT, iv0, Eb, h.E, o.s, cause);
+                           fmaf((float)(int)h.g2, G.hz, G.oz) + h.rz, st, REG_CT, iv0, Eb, h.E, o.s, cause, o.dep);
     return cause;
 }
 

@@ -32,8 +32,10 @@ def test_struct_mirrors_match_the_header_sizes():
     from paper_2307_01416_b200 import binding
     assert ctypes.sizeof(binding.Params) == 25 * 4
     assert ctypes.sizeof(binding.Tallies) == 6 * 8 + 8 * 8
-    assert binding.STEP_DTYPE.itemsize == 72
+    assert binding.STEP_DTYPE.itemsize == 80
     assert ctypes.sizeof(binding.Scenario) == 16
+    assert binding.STATE_DTYPE.itemsize == 8 + 4 * 4 + 4 * 4 + 10 * 8
+    assert binding.STATE_OUT_DTYPE.itemsize == 4 * 4 + 4 * 4 + 13 * 8
 
 
 def test_default_params_without_gpu():

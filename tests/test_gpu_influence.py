@@ -1,17 +1,15 @@
 """GPU parity of the influence path (S7, S8): per-spot columns under scenarios and the CSR writer.
 
-Tolerances (SURVEY.md 8(c)-A10, DESIGN.md 4):
-  * the writer alone is bit-exact: fed the oracle's fp32 column it returns the oracle's (col, val) row;
-  * end to end a column of H histories holds ~f H re-dealt histories (f ~ 1e-3), each of which moves one
-    history's deposit -- about 1 / n_v of the voxel's value, n_v ~ H / 40 histories through the hottest voxel -- so per
-    entry the test asserts: column sums within 2e-3 relative, >= 95 % of the entries kept by both sides within 1e-3 of
-    the column maximum and all of them within TOL_ENTRY = 2e-2 of it, and an entry kept by one side only must be
-    explainable by that tolerance (its value lies within TOL_ENTRY max of the threshold); row order, index order
-    and types are exact.  The 1e-3 bar itself is asserted where the statistics carry it: on the weighted sum of the
+Tolerances (SURVEY.md 8(c)-A10, DESIGN.md 4.3):
+  * (i) the writer alone is bit-exact: fed the oracle's fp32 column it returns the oracle's (col, val) row;
+  * (ii) end to end, the kept sets are equal except for entries whose value lies within +-0.1 % of the threshold
+    (counted) -- and except in voxels visited by a RE-DEALT history: a history whose discrete trace differs between
+    the two paths (a near-tie flip, tests/test_gpu_parity.py) moves its own deposits.  Those histories are found by
+    tracing every history of the column on both sides, counted and bounded, and the voxels either version of them
+    visits are the only ones exempt; everywhere else values agree to 1e-5 of the column maximum (fp32 sums);
+  * row order, index order, uniqueness and types are always exact; the 1e-3 dose bar holds on the weighted sum of the
     columns (= the plan dose of all H n_spots histories).
 """
-import os
-
 import numpy as np
 import pytest
 
@@ -46,37 +44,80 @@ def check_csr_structure(rp, col, val, n_rows, nvox):
     assert (val > 0).all()
 
 
-TOL_ENTRY = 2e-2
+DRIFT_MM = 1e-5       # a history is "drifted" once its traced position differs from the oracle's by more than this (0.01 um)
+S_MAX = 15.0          # MeV / mm of water: stopping power at the R_cut energy (2.35 MeV), the largest a step can see
 
 
-def compare_rows(gpu, ref, nvox, rel_thr):
-    """gpu/ref = (row_ptr, col, val).  Returns (#entries kept by one side only, #of those within 0.1 % of threshold,
-    summed dense gpu column, summed dense reference column)."""
-    grp, gc, gv = gpu
-    orp, oc, ov = ref
-    assert (grp.shape == orp.shape)
-    only, near = 0, 0
-    sum_a = np.zeros(nvox); sum_b = np.zeros(nvox)
-    for r in range(orp.size - 1):
-        a = np.zeros(nvox, dtype=np.float64); b = np.zeros(nvox, dtype=np.float64)
-        a[gc[grp[r]:grp[r + 1]]] = gv[grp[r]:grp[r + 1]]
-        b[oc[orp[r]:orp[r + 1]]] = ov[orp[r]:orp[r + 1]]
-        mx = b.max() if b.size else 0.0
-        if mx == 0.0:
-            assert a.max() == 0.0
-            continue
-        thr = rel_thr * mx
-        both = (a > 0) & (b > 0)
-        dev = np.abs(a[both] - b[both]) / mx
-        assert dev.max() <= TOL_ENTRY and np.mean(dev <= 1e-3) >= 0.95, (r, dev.max(), np.mean(dev <= 1e-3))
-        assert abs(a.sum() - b.sum()) <= 2e-3 * b.sum()
-        one = (a > 0) != (b > 0)
-        # kept by one side only: the kept value must lie within the entry tolerance of the threshold
-        assert (np.maximum(a[one], b[one]) <= thr + TOL_ENTRY * mx).all()
-        only += int(one.sum())
-        near += int((np.abs(np.maximum(a[one], b[one]) - thr) <= 1e-3 * thr).sum())
-        sum_a += a; sum_b += b
-    return only, near, sum_a, sum_b
+def flagged_histories(bind, eng, O, pb, g, hps, seed, sc, nvox, n_xy, chunk=2500):
+    """Traces every history of column g on both sides.  A history is FLAGGED when its discrete trace differs (a near-tie
+    flip, after which its random deflections are re-dealt) or when its position has drifted by more than DRIFT_MM (the
+    accumulated difference of DESIGN.md 4.2); every other history is the oracle's history up to the energy a 0.01 um
+    shift of a voxel boundary moves (DRIFT_MM x stopping power).  Returns (#re-dealt, #drifted, E_dep difference CUDA - oracle of the flagged histories per voxel [MeV],
+    mask of the voxels they visit)."""
+    delta = np.zeros(nvox, dtype=np.float64)
+    mask = np.zeros(nvox, dtype=bool)
+    n_re = n_drift = 0
+    sc_g = bind.scenario(sc[0], sc[1])
+    sc_o = O.scenario(sc[0], float(np.float32(sc[1])))
+    gamma_loc = float(pb.params.gamma_loc)
+    for i0 in range(0, hps, chunk):
+        hids = np.uint64(g) * np.uint64(hps) + np.arange(i0, min(i0 + chunk, hps), dtype=np.uint64)
+        a_all = eng.trace(hids, hps, seed, sc=sc_g, mode=1, max_steps=1000)
+        b_all = O.trace(pb, hids, hps, seed, sc_o, mode=1, max_steps=1000)
+        for a, b in zip(a_all, b_all):
+            same = (len(a) == len(b) and (a["region"] == b["region"]).all() and (a["ivox"] == b["ivox"]).all()
+                    and (a["cause"] == b["cause"]).all())
+            if same and float(np.abs(a["r"] - b["r"]).max()) <= DRIFT_MM:
+                continue
+            n_re += 0 if same else 1
+            n_drift += 1 if same else 0
+            for t, sign in ((a, +1.0), (b, -1.0)):
+                ct = t["region"] == O.REG_CT
+                iv = t["ivox"][ct].astype(np.int64)
+                v = iv[:, 0] + n_xy[0] * (iv[:, 1] + n_xy[1] * iv[:, 2])
+                np.add.at(delta, v, sign * t["dep"][ct].astype(np.float64))
+                mask[v] = True
+    return n_re, n_drift, delta, mask
+
+
+def compare_row(O, pb, a_cv, b_dense, delta_edep, touched, nvox, rel_thr, hps):
+    """A10(ii) for one row.  a_cv = the CUDA row (col, val); b_dense = the oracle's dense fp32 column; delta_edep = the
+    energy the FLAGGED histories account for (their traced deposits, CUDA minus oracle, MeV), `touched` = the voxels they
+    visit.  With pred = b_dense + dose(delta_edep) and tol_v = 2e-4 pred_v + dose_v(3 x DRIFT_MM x S_MAX x RSP_max) (what
+    unflagged histories can move) + 1e-7 max (fp32 sums):
+      * every kept value equals pred within tol;
+      * the kept set equals {pred >= threshold} except for entries within 0.1 % of the threshold + tol;
+      * outside the voxels of flagged histories pred IS the oracle's column, so there this is A10(ii) as written, up to
+        the 0.01 um the unflagged histories may have moved.
+    Returns (#one-sided entries at the threshold, #kept-set differences against the plain oracle row that the flagged
+    histories explain)."""
+    a = np.zeros(nvox, dtype=np.float64)
+    a[a_cv[0]] = a_cv[1]
+    b = b_dense.astype(np.float64)
+    mx = b.max()
+    if mx == 0.0:
+        assert a.max() == 0.0
+        return 0, 0
+    pred = b + O.dose_from_edep(pb, delta_edep, 1.0 / hps)
+    mxp = max(pred.max(), mx)
+    thr = rel_thr * float(np.float32(a.max()))            # the CUDA row's own threshold (its column maximum is kept)
+    tol = 2e-4 * np.abs(pred) + O.dose_from_edep(pb, np.full(nvox, 3.0 * DRIFT_MM * S_MAX * 2.5), 1.0 / hps) + 1e-7 * mxp
+    kept = a > 0
+    assert abs(a.max() - pred.max()) <= 2e-4 * mxp
+    bad = kept & (np.abs(a - pred) > tol)
+    assert not bad.any(), ("kept values differ from oracle + flagged histories", int(bad.sum()), np.flatnonzero(bad)[:5], a[bad][:5], pred[bad][:5])
+    should = pred >= thr
+    one = kept != should
+    near = one & (np.abs(pred - thr) <= 1e-3 * thr + tol)
+    assert not (one & ~near).any(), ("kept set differs away from the threshold", np.flatnonzero(one & ~near)[:5], pred[one & ~near][:5] / thr)
+    thr_o = rel_thr * mx                                    # the plain oracle row's own threshold
+    explained = (kept != ((b > 0) & (b >= thr_o))) & ~near
+    # away from the flagged histories' voxels pred IS the oracle's value, so a difference there can only come from the
+    # threshold itself: the flagged histories moved the column maximum, and the value lies between the two thresholds
+    between = (b >= min(thr, thr_o) * (1.0 - 1e-3) - tol) & (b <= max(thr, thr_o) * (1.0 + 1e-3) + tol)
+    assert not (explained & ~touched & ~between).any(), "a kept-set difference outside the voxels of flagged histories"
+    assert abs(a.sum() - b[b >= rel_thr * mx].sum()) <= 2e-3 * b.sum()
+    return int(near.sum()), int(explained.sum())
 
 
 @pytest.mark.parametrize("n", [1, 7, 2047, 2048, 2049, 100003, 1 << 20])
@@ -120,26 +161,41 @@ SCEN = [((0.0, 0.0, 0.0), 1.0), ((3.0, 0.0, 0.0), 1.0), ((0.0, -3.0, 3.0), 1.035
 def test_influence_parity(bind, case):
     O = orc()
     w = {"hetero": hetero_case, "rs_ap": rs_case, "rotated": rotated_case}[case]()
-    hps, thr, seed = 20000, 1e-4, 9
+    hps, thr, seed = 10000, 1e-4, 9
     eng = bind.Engine(w)
     pb = oracle_problem(w)
     nvox = eng.nvox
     res = eng.influence([bind.scenario(s, k) for s, k in SCEN], hps, thr, seed)
     t = eng.tallies().as_dict()
     assert sum(t[k] for k in ("n_stopped_ct", "n_stopped_rs", "n_stopped_brass", "n_nuclear", "n_escaped")) == len(SCEN) * eng.n_spots * hps
-    tot_only = tot_near = tot_nnz = 0
+    tot_near = tot_ex = tot_nnz = tot_re = tot_drift = 0
     for (shift, scale), (rp, col, val) in zip(SCEN, res):
-        g = (rp.cpu().numpy(), col.cpu().numpy(), val.cpu().numpy())
-        check_csr_structure(*g, eng.n_spots, nvox)
-        ref = O.influence_csr(pb, hps, thr, seed, O.scenario(shift, float(np.float32(scale))))
-        only, near, sa, sb = compare_rows(g, ref, nvox, thr)
-        tot_only += only; tot_near += near; tot_nnz += ref[1].size
+        rp, col, val = rp.cpu().numpy(), col.cpu().numpy(), val.cpu().numpy()
+        assert np.isfinite(val).all()
+        check_csr_structure(rp, col, val, eng.n_spots, nvox)
+        sc_o = O.scenario(shift, float(np.float32(scale)))
+        sa = np.zeros(nvox); sb = np.zeros(nvox); sd = np.zeros(nvox)
+        for g in range(eng.n_spots):
+            b_dense = O.influence_column(pb, g, hps, seed, sc_o)
+            n_re, n_drift, delta, touched = flagged_histories(bind, eng, O, pb, g, hps, seed, (shift, scale), nvox, eng.n[:2])
+            near, ex = compare_row(O, pb, (col[rp[g]:rp[g + 1]], val[rp[g]:rp[g + 1]]), b_dense, delta, touched, nvox, thr, hps)
+            tot_near += near; tot_ex += ex; tot_re += n_re; tot_drift += n_drift; tot_nnz += int(rp[g + 1] - rp[g])
+            sa[col[rp[g]:rp[g + 1]]] += val[rp[g]:rp[g + 1]]; sb += b_dense
+            sd += O.dose_from_edep(pb, delta, 1.0 / hps)
         err_sum = np.abs(sa - sb).max() / sb.max()
-        print(case, shift, scale, "sum of columns: max |d| / max = %.2e" % err_sum)
-        assert err_sum <= (1e-3 if case != "rs_ap" else 1e-2)      # rs_ap: 4e4 histories in all, f ~ 1e-2
-    print(case, "nnz", tot_nnz, "entries kept by one side only", tot_only, "of which within 0.1%% of the threshold", tot_near)
+        err_acc = np.abs(sa - sb - sd).max() / sb.max()
+        print(case, shift, scale, "sum of columns: max |d| / max = %.2e raw, %.2e with the flagged histories' own deposits accounted for" % (err_sum, err_acc))
+        assert err_acc <= 2e-4 + thr * eng.n_spots            # entries below the threshold are missing from the CSR rows
+        # raw bar of north_star (1e-3 of the maximum) where the 1-3 x 10^4 histories of the case allow it; behind the range
+        # shifter f ~ 1e-2 of 2 x 10^4 histories are re-dealt: printed, bounded as a sanity check only
+        assert err_sum <= (1e-3 if case != "rs_ap" else 5e-2)
+    n_hist = len(SCEN) * eng.n_spots * hps
+    print(case, "nnz", tot_nnz, "| histories", n_hist, "re-dealt", tot_re, "drifted >", DRIFT_MM, "mm:", tot_drift,
+          "| one-sided entries at the threshold", tot_near, "| kept-set differences explained by flagged histories", tot_ex)
     assert tot_nnz > 1000
-    assert tot_only <= 0.05 * tot_nnz
+    # sanity bounds only: how many histories two fp32 / fp64 implementations of this method re-deal is a property of the
+    # method (tests/test_method_sensitivity.py); the numbers are printed above and recorded in profiles/
+    assert tot_re <= (3e-2 if case == "rs_ap" else 5e-3) * n_hist
     eng.close()
 
 
@@ -160,20 +216,25 @@ def test_influence_groups_and_replay_give_the_same_matrix(bind):
     base, p_base = run()
     eng.set_workspace_limit(4 * 1024)                   # 1024 box elements: one column per group
     small, p_small = run()
-    os.environ["VPMC_BOX_GROW"] = "0"; os.environ["VPMC_BOX_PAD"] = "0"
-    try:
-        eng.set_workspace_limit(0)
-        overflow, p_ovf = run()                         # tight boxes: the overflow list fills the rows
-        os.environ["VPMC_OVF_CAP"] = "0"                # no list: the replay path
-        replay, p_replay = run()
-    finally:
-        del os.environ["VPMC_BOX_GROW"], os.environ["VPMC_BOX_PAD"]
-        os.environ.pop("VPMC_OVF_CAP", None)
+    eng.set_knob(bind.KNOB_BOX_GROW, 0); eng.set_knob(bind.KNOB_BOX_PAD, 0)
+    eng.set_workspace_limit(0)
+    overflow, p_ovf = run()                             # tight boxes: the overflow list fills the rows
+    eng.set_knob(bind.KNOB_OVF_CAP, 0)                  # no list: the replay path
+    replay, p_replay = run()
     assert p_base == 2 and p_small == 1 + eng.n_spots and p_ovf == 2 and p_replay == 3, (p_base, p_small, p_ovf, p_replay)
+    # the same histories in another launch order: identical structure up to entries at the threshold, values to fp32 sums
+    none = np.zeros(eng.nvox, dtype=bool); zero = np.zeros(eng.nvox)
     for other in (small, overflow, replay):
-        only = compare_rows(other, base, eng.nvox, thr)[0]
-        assert only <= 0.02 * base[1].size
         check_csr_structure(*other, eng.n_spots, eng.nvox)
+        for g in range(eng.n_spots):
+            dense = np.zeros(eng.nvox, dtype=np.float32)
+            dense[base[1][base[0][g]:base[0][g + 1]]] = base[2][base[0][g]:base[0][g + 1]]
+            lo, hi = other[0][g], other[0][g + 1]
+            a = np.zeros(eng.nvox); a[other[1][lo:hi]] = other[2][lo:hi]
+            both = (a > 0) & (dense > 0)
+            assert np.abs(a - dense)[both].max() <= 1e-5 * dense.max()
+            one = (a > 0) != (dense > 0)
+            assert (np.abs(np.maximum(a, dense)[one] - thr * dense.max()) <= 1e-3 * thr * dense.max()).all()
     eng.close()
 
 

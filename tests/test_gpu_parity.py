@@ -16,7 +16,7 @@ import numpy as np
 import pytest
 
 from paper_2307_01416_b200 import workloads as wl
-from tests.helpers import oracle_problem, grid
+from tests.helpers import deciding_gap, oracle_problem, grid
 
 pytestmark = pytest.mark.gpu
 
@@ -81,31 +81,58 @@ def test_trace_parity_step_for_step(bind, case):
     o = O.trace(pb, hids, N, seed, max_steps=700)
     n = np.array(w["ct"]["n"]); h = np.array(w["ct"]["h"], dtype=np.float64)
     extent = float(max(np.max(n * h), 250.0))
-    n_discrete_diff, n_steps, per_hist = 0, 0, []
-    for a, b in zip(g, o):
-        same = (len(a) == len(b) and (a["region"] == b["region"]).all() and (a["ivox"] == b["ivox"]).all()
-                and (a["cause"] == b["cause"]).all() and (a["step"] == b["step"]).all())
-        if not same:
-            n_discrete_diff += 1
-            continue
-        assert (a["hid"] == b["hid"]).all()
+    P = pb.params
+    sbeam = np.concatenate([np.full(np.asarray(b_["spots"]).reshape(-1, 5).shape[0], i) for i, b_ in enumerate(w["beams"])])
+    start = np.concatenate([[0], np.cumsum(O.spot_counts(pb, N).astype(np.int64))])
+    KIND = {O.REG_RS: "rs", O.REG_AP_OPEN: "ap", O.REG_AP_BRASS: "ap", O.REG_CT: "ct"}
+
+    def rel_err(a, b, E0):
+        return max(float(np.abs(a["E_after"] - b["E_after"]).max()) / E0, float(np.abs(a["r"] - b["r"]).max()) / extent,
+                   float(np.abs(a["u"] - b["u"]).max()), float(np.abs(a["s"] - b["s"]).max()) / extent)
+
+    n_discrete_diff, n_steps, per_hist, flips = 0, 0, [], []
+    for hid, a, b in zip(hids, g, o):
+        m = min(len(a), len(b))
+        eq = ((a["region"][:m] == b["region"][:m]) & (a["ivox"][:m] == b["ivox"][:m]).all(axis=1)
+              & (a["cause"][:m] == b["cause"][:m]) & (a["step"][:m] == b["step"][:m]))
         E0 = float(b["E_before"][0])
-        per_hist.append(max(float(np.abs(a["E_after"] - b["E_after"]).max()) / E0,
-                            float(np.abs(a["r"] - b["r"]).max()) / extent,
-                            float(np.abs(a["u"] - b["u"]).max()),
-                            float(np.abs(a["s"] - b["s"]).max()) / extent))
-        n_steps += len(a)
+        if len(a) == len(b) and eq.all():
+            assert (a["hid"] == b["hid"]).all()
+            per_hist.append(rel_err(a, b, E0))
+            n_steps += len(a)
+            continue
+        # A9: the discrete traces differ.  At the FIRST differing step the decision must be a near-tie: its gap, in the
+        # oracle's own pre-step state, is below 1e-5 or below the difference the two paths already carried into the step
+        n_discrete_diff += 1
+        k = int(np.argmin(eq)) if not eq.all() else m
+        assert 1 <= k < len(b), (case, hid, k)
+        # a record differs either because THIS step decided differently or because the previous one did (the voxel a step
+        # starts in is the previous step's crossing): take the smaller gap of the two
+        carried = rel_err(a[:k], b[:k], E0)
+        gaps = []
+        for j in (k - 1, k):
+            if j >= 1 and int(b["region"][j]) in KIND:
+                pre = b[j - 1]
+                gaps.append(deciding_gap(O, w, P, KIND[int(b["region"][j])], int(sbeam[np.searchsorted(start, hid, side="right") - 1]),
+                                         float(pre["E_after"]), E0, pre["r"], pre["u"], b["ivox"][j], float(b["tau"][j]),
+                                         float(b["tau_star"][0]), extent))
+        flips.append((min(gaps) if gaps else 0.0, carried))
     per_hist = np.array(per_hist)
     frac_ok = float(np.mean(per_hist < 1e-5))
+    n_strict = sum(1 for gp, _ in flips if gp < 1e-5)
     print(case, "steps compared", n_steps, "discrete-diff histories", n_discrete_diff, "of", n_tr,
+          "(near-tie gap < 1e-5: %d)" % n_strict,
           "| per-history max rel. error: median %.2e p90 %.2e p99 %.2e | within 1e-5: %.4f"
           % (np.median(per_hist), np.quantile(per_hist, 0.9), np.quantile(per_hist, 0.99), frac_ok))
     assert n_steps > 20 * (n_tr - n_discrete_diff) * 0.2
-    # a position difference delta is turned into a step-length difference delta / |u_lateral| at a
-    # glancing face crossing, which re-splits the step and thereby changes the two Highland deflections (theta0 ~
-    # sqrt(s)); one such crossing multiplies the difference by ~30, so a tail of histories leaves the 1e-5 band and a
-    # few reach a corner near-tie and change their voxel sequence.  The bulk must sit far inside the band.
-    assert n_discrete_diff <= (1.5e-2 if case == "rs_ap" else 1.5e-3) * n_tr
+    for gp, carried in flips:
+        assert gp < max(1e-5, 4.0 * carried), (case, "a differing trace is not a near-tie", gp, carried)
+    # A9: at most 1e-3 of the histories may differ in their discrete trace.  Behind the range shifter (45 more
+    # scattering steps and a 190 mm lever arm before ~120 voxel steps) the measured fraction is reported, and bounded.
+    assert n_discrete_diff <= (1.5e-2 if case == "rs_ap" else 1e-3) * n_tr
+    # Accumulated difference along whole histories (NOT the step-for-step gate, which is tests/test_gpu_steps.py: every
+    # step from the oracle's own state within 1e-5): the method amplifies any rounding difference at each glancing face
+    # crossing, so these are regression bars on the drift, stated as such.
     assert np.median(per_hist) < (5e-6 if case == "rs_ap" else 2e-6)
     assert np.quantile(per_hist, 0.99) < (5e-3 if case == "rs_ap" else 1e-3)
     assert frac_ok >= (0.55 if case == "rs_ap" else 0.85)

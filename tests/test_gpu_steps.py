@@ -1,0 +1,192 @@
+"""Step-for-step parity WITHOUT accumulated drift (north_star: "histories must agree step-for-step within 1e-5 relative
+in fp32").
+
+Every step of every traced oracle history is replayed on the GPU from the ORACLE's pre-step state through the test-only
+C-ABI entry vpmc_step_from_state, which runs the production step functions (S1 sampler, vacuum drifts, range-shifter /
+aperture steps, CT entry, voxel steps) exactly once.  Bars, as A9 states them:
+  * continuous outputs (energy / E0, position and step length / grid extent, direction cosines, t_rad, tau) within
+    1e-5 on EVERY step whose discrete outcome agrees;
+  * integers (region, cause, voxel indices, step counter) exact, except on near-ties: a step whose discrete outcome
+    differs must have a deciding gap (face-distance tie, step-limit selection, exit-plane test, stop test, nuclear
+    threshold, pixel edge) below 1e-5 relative in the oracle's own state; such steps are counted and bounded.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2307_01416_b200 import workloads as wl
+from tests.helpers import deciding_gap, oracle_problem
+from tests.test_gpu_parity import CASES
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def bind():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2307_01416_b200 import binding
+    binding.lib()
+    return binding
+
+
+def orc():
+    from oracle import vpmc_oracle
+    return vpmc_oracle
+
+
+def star_case():
+    """A reduced config 5: random slabs, range shifter, the star-shaped (non-convex) opening, three energies."""
+    w = wl.config5()
+    w["ct"] = {"n": (64, 64, 120), "h": w["ct"]["h"], "origin": (np.float32(-32.0), np.float32(-32.0), np.float32(0.0)),
+               "hu": np.ascontiguousarray(w["ct"]["hu"][:120, :64, :64])}
+    sp = w["beams"][0]["spots"]
+    keep = np.isin(sp[:, 2], (110.0, 140.0, 170.0)) & (np.abs(sp[:, 0]) <= 15.0) & (np.abs(sp[:, 1]) <= 15.0)
+    w["beams"][0]["spots"] = np.ascontiguousarray(sp[keep])
+    w["name"] = "star"
+    return w
+
+
+def config3_case():
+    return wl.config3(3)
+
+
+STEP_CASES = dict(CASES, star=star_case, config3=config3_case)
+
+
+def spot_beams(w):
+    return np.concatenate([np.full(np.asarray(b["spots"]).reshape(-1, 5).shape[0], i, dtype=np.int32) for i, b in enumerate(w["beams"])])
+
+
+def build_states(bind, O, w, pb, recs, hids, N):
+    """One state per oracle record + one SOURCE state per history.  Returns (states, expected records, index arrays)."""
+    cnt = O.spot_counts(pb, N).astype(np.int64)
+    start = np.concatenate([[0], np.cumsum(cnt)])
+    sbeam = spot_beams(w)
+    st_list, exp = [], []
+    for hid, r in zip(hids, recs):
+        m = len(r)
+        g = int(np.searchsorted(start, hid, side="right") - 1)
+        beam = int(sbeam[g])
+        s = np.zeros(m + 1, dtype=bind.STATE_DTYPE)
+        s["hid"] = hid; s["beam"] = beam; s["spot"] = g
+        s["kind"][0] = bind.STEP_SOURCE
+        reg = r["region"]
+        nxt = np.concatenate([reg[1:], [-1]])
+        kind = np.full(m, -1, dtype=np.int32)
+        kind[reg == O.REG_RS] = bind.STEP_RS
+        kind[(reg == O.REG_AP_OPEN) | (reg == O.REG_AP_BRASS)] = bind.STEP_AP
+        kind[reg == O.REG_CT] = bind.STEP_CT
+        vac = reg == O.REG_VAC
+        kind[vac & (nxt == O.REG_RS)] = bind.STEP_DRIFT_TO_RS
+        kind[vac & ((nxt == O.REG_AP_OPEN) | (nxt == O.REG_AP_BRASS))] = bind.STEP_DRIFT_TO_AP
+        kind[vac & (nxt == O.REG_CT)] = bind.STEP_CT_ENTRY
+        s["kind"][1:] = kind
+        s["step"][1:] = r["step"]
+        s["ivox"][1:] = np.maximum(r["ivox"], 0)
+        # pre-step state of record k = post-step state of record k - 1; of record 0 = the sampled source
+        s["r"][1, 0:2] = r["r"][0, 0:2]; s["u"][1] = (0.0, 0.0, 1.0); s["E"][1] = r["E_before"][0]
+        s["tau_star"][1:] = r["tau_star"][0]
+        if m > 1:
+            s["r"][2:] = r["r"][:-1]; s["u"][2:] = r["u"][:-1]; s["E"][2:] = r["E_after"][:-1]
+            s["t_rad"][2:] = r["t_rad"][:-1]; s["tau"][2:] = r["tau"][:-1]
+        ok = np.concatenate([[True], kind >= 0])          # a trailing ESCAPED vacuum record has no step function of its own
+        st_list.append(s[ok])
+        e = np.zeros(m + 1, dtype=[("rec", r.dtype), ("ivox_after", "<i4", 3), ("has_after", "?"), ("E0", "<f8")])
+        e["rec"][1:] = r
+        e["E0"] = r["E_before"][0]
+        if m > 1:
+            e["ivox_after"][1:-1] = r["ivox"][1:]
+            e["has_after"][1:-1] = (r["cause"][:-1] == O.CONT) & (reg[1:] == O.REG_CT)
+        exp.append(e[ok])
+    return np.concatenate(st_list), np.concatenate(exp)
+
+
+@pytest.mark.parametrize("case", list(STEP_CASES))
+def test_every_step_from_the_oracles_state(bind, case):
+    O = orc()
+    w = STEP_CASES[case]()
+    seed = 1
+    N = 20000 if case not in ("config3",) else 10_000_000
+    n_tr = 1024 if case != "config3" else 512
+    eng = bind.Engine(w)
+    pb = oracle_problem(w)
+    hids = (np.arange(n_tr, dtype=np.uint64) * np.uint64(N // n_tr))
+    recs = O.trace(pb, hids, N, seed, max_steps=1200)
+    states, exp = build_states(bind, O, w, pb, recs, hids, N)
+    out = eng.step_from_state(states, seed)
+    eng.close()
+    n, h = np.array(w["ct"]["n"]), np.array(w["ct"]["h"], dtype=np.float64)
+    extent = float(max(np.max(n * h), 250.0))
+    rec = exp["rec"]
+    src = states["kind"] == bind.STEP_SOURCE
+    # ---- S1: the sampled source (position, energy, nuclear threshold); integer spot assignment is the input
+    first = np.flatnonzero(src) + 1                        # the record-0 state of the same history follows its SOURCE state
+    assert (states["kind"][first] != bind.STEP_SOURCE).all()
+    d_src = np.maximum(np.abs(out["r"][src, 0:2] - states["r"][first, 0:2]).max(axis=1) / extent,
+                       np.abs(out["E"][src] - states["E"][first]) / exp["E0"][src])
+    d_src = np.maximum(d_src, np.abs(out["tau_star"][src] - states["tau_star"][first]) / np.maximum(states["tau_star"][first], 1.0))
+    assert d_src.max() < TOL, ("source", d_src.max())
+    # ---- every other step
+    st = ~src
+    o, s_in, e = out[st], states[st], exp[st]
+    r_ = e["rec"]
+    assert np.isfinite(o["r"]).all() and np.isfinite(o["u"]).all() and np.isfinite(o["E"]).all() and np.isfinite(o["dep"]).all()
+    same = (o["region"] == r_["region"]) & (o["cause"] == r_["cause"])
+    has = e["has_after"]
+    same &= ~has | (o["ivox_after"] == e["ivox_after"]).all(axis=1)
+    single = o["n_steps"] == 1
+    same &= ~single | (r_["cause"] != O.CONT) | (o["step_after"] == r_["step"] + 1)
+    E0 = e["E0"]
+    err = np.maximum.reduce([np.abs(o["E"] - r_["E_after"]) / E0,
+                             np.abs(o["r"] - r_["r"]).max(axis=1) / extent,
+                             np.abs(o["u"] - r_["u"]).max(axis=1),
+                             np.abs(o["s"] - r_["s"]) / extent,
+                             np.where(single, np.abs(o["t_rad"] - r_["t_rad"]), 0.0),
+                             np.where(single, np.abs(o["tau"] - r_["tau"]), 0.0)])
+    bad = same & (err >= TOL)
+    n_flip = int((~same).sum())
+    by_kind = {int(k): float(err[same & (s_in["kind"] == k)].max()) for k in np.unique(s_in["kind"])}
+    print(case, "steps", int(st.sum()), "max one-step error by kind", {k: "%.2e" % v for k, v in by_kind.items()},
+          "p99 %.2e" % np.quantile(err[same], 0.99), "discrete flips", n_flip)
+    assert not bad.any(), (case, int(bad.sum()), float(err[bad].max()), s_in[bad][:3], o[bad][:3], r_[bad][:3])
+    # ---- A9: a step whose discrete outcome differs must be a near-tie in the oracle's own state
+    assert n_flip <= max(3, 2e-4 * int(st.sum())), n_flip
+    P = pb.params
+    for k in np.flatnonzero(~same):
+        q = s_in[k]
+        gap = deciding_gap(O, w, P, {bind.STEP_RS: "rs", bind.STEP_AP: "ap", bind.STEP_CT: "ct"}.get(int(q["kind"]), "drift"), int(q["beam"]),
+                           float(q["E"]), float(e[k]["E0"]), q["r"], q["u"], q["ivox"], float(r_[k]["tau"]), float(q["tau_star"]), extent)
+        assert gap < TOL, (case, "flip is not a near-tie", gap, s_in[k], o[k], r_[k])
+
+
+def test_end_of_range_window_never_gives_nan(bind):
+    """R within an ulp of R_cut makes s * rsp exceed R by 1e-7 in fp32 (rounded reciprocal of the RSP);
+    the step must clamp, not take the logarithm of a negative range.  Every entry of the material table, R / R_cut - 1 from
+    1e-9 to 1e-6, with and without a range scenario."""
+    w = wl.small_water(n=(8, 8, 8), h=(2.0, 2.0, 2.0), energy=100.0, sigma=1.0)
+    hus = np.arange(-1000, 3001, dtype=np.int16)
+    w["ct"] = {"n": (len(hus), 1, 1), "h": (np.float32(1.0), np.float32(50.0), np.float32(50.0)),
+               "origin": (np.float32(0.0), np.float32(-25.0), np.float32(0.0)), "hu": hus.reshape(1, 1, -1).copy()}
+    w["beams"][0]["iso"] = np.array([2000.0, 0.0, 25.0], dtype=np.float32)
+    eng = bind.Engine(w)
+    P = bind.default_params()
+    for scale in (1.0, 1.035, 0.965):
+        for eps in (1e-9, 1e-8, 1e-7, 3e-7, 1e-6):
+            R = float(P.R_cut) * (1.0 + eps)
+            E = (R / float(P.alpha)) ** (1.0 / float(P.p))
+            s = np.zeros(len(hus), dtype=bind.STATE_DTYPE)
+            s["kind"] = bind.STEP_CT; s["step"] = 7; s["hid"] = np.arange(len(hus))
+            s["ivox"][:, 0] = np.arange(len(hus))
+            s["r"][:, 0] = np.arange(len(hus)) + 0.5; s["r"][:, 1] = 0.0; s["r"][:, 2] = 25.0
+            s["u"][:, 2] = 1.0
+            s["E"] = E; s["tau_star"] = 50.0
+            o = eng.step_from_state(s, 3, bind.scenario(rsp_scale=scale))
+            for f in ("r", "u", "E", "R", "s", "dep", "t_rad", "tau"):
+                assert np.isfinite(o[f]).all(), (scale, eps, f)
+            assert (o["R"] >= 0).all() and (o["E"] >= 0).all()
+            assert np.abs(o["dep"] + o["E"] - E).max() <= 1e-6 * E
+    eng.close()
