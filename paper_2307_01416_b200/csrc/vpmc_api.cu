@@ -156,7 +156,7 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_qctr, h->d_s1, h->d_s2, h->d_fb,
                      h->d_tal, h->d_tal_scratch, h->d_max_bits, h->d_unc };
     for (void *p : ptrs) if (p) cudaFree(p);
-    DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
+    DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
                        &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n };
@@ -221,25 +221,27 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     CUC(cudaMalloc(&h->d_tal_scratch, sizeof(DevTallies)));
     CUC(cudaMalloc(&h->d_max_bits, sizeof(unsigned int)));
     CUC(cudaMalloc(&h->d_unc, 2 * sizeof(double)));
-    CUC(cudaMalloc(&h->d_qctr, 4 * sizeof(unsigned int)));
+    CUC(cudaMalloc(&h->d_qctr, 8 * sizeof(unsigned int)));
     CUC(cudaMalloc(&h->d_fb, 1024 * sizeof(float)));
     // persistent kernels: one wave of resident CTAs each
     {
         h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
         // occupancy queries are ~0.3 ms each: remember the answer per (device, table size, table placement)
-        struct GridCache { int device; size_t lut_bytes; bool smem; int grid_beam; int grid[3][2]; };
+        struct GridCache { int device; size_t lut_bytes; bool smem; int grid_beam[2]; int grid[3][2]; };
         static std::mutex mu;
         static std::vector<GridCache> cache;
         bool hit = false;
         {
             std::lock_guard<std::mutex> lk(mu);
             for (const GridCache &g : cache)
-                if (g.device == h->device && g.lut_bytes == h->lut_bytes && g.smem == h->smem_lut) { h->grid_beam = g.grid_beam; memcpy(h->grid, g.grid, sizeof(h->grid)); hit = true; }
+                if (g.device == h->device && g.lut_bytes == h->lut_bytes && g.smem == h->smem_lut) { memcpy(h->grid_beam, g.grid_beam, sizeof(h->grid_beam)); memcpy(h->grid, g.grid, sizeof(h->grid)); hit = true; }
         }
         if (!hit) {
             int occ = 0;
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel, kBlock, 0));
-            h->grid_beam = std::max(occ, 1) * h->n_sm;
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel<0>, kBlock, 0));
+            h->grid_beam[0] = std::max(occ, 1) * h->n_sm;
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel<1>, kBlock, 0));
+            h->grid_beam[1] = std::max(occ, 1) * h->n_sm;
             const void *fn[3][2] = { { (const void *)voxel_kernel<0, false>, (const void *)voxel_kernel<0, true> },
                                      { (const void *)voxel_kernel<1, false>, (const void *)voxel_kernel<1, true> },
                                      { (const void *)voxel_kernel<2, false>, (const void *)voxel_kernel<2, true> } };
@@ -251,7 +253,7 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
                     CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn[m][s], kBlock, sm));
                     h->grid[m][s] = std::max(occ, 1) * h->n_sm;
                 }
-            GridCache g; g.device = h->device; g.lut_bytes = h->lut_bytes; g.smem = h->smem_lut; g.grid_beam = h->grid_beam; memcpy(g.grid, h->grid, sizeof(g.grid));
+            GridCache g; g.device = h->device; g.lut_bytes = h->lut_bytes; g.smem = h->smem_lut; memcpy(g.grid_beam, h->grid_beam, sizeof(g.grid_beam)); memcpy(g.grid, h->grid, sizeof(g.grid));
             std::lock_guard<std::mutex> lk(mu);
             cache.push_back(g);
         }
@@ -387,9 +389,9 @@ extern "C" int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t h
 // ---- per-kernel-class timing (events on the launching stream) ----
 struct TimedScope {
     vpmc_t *h; cudaStream_t st; int cls; cudaEvent_t a = nullptr, b = nullptr;
-    TimedScope(vpmc_t *h_, cudaStream_t st_, int cls_) : h(h_), st(st_), cls(cls_)
+    TimedScope(vpmc_t *h_, cudaStream_t st_, int cls_, bool enabled = true) : h(h_), st(st_), cls(cls_)
     {
-        if (h->timing && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) cudaEventRecord(a, st);
+        if (enabled && h->timing && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) cudaEventRecord(a, st);
         else a = nullptr;
     }
     ~TimedScope()

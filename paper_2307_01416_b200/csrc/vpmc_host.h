@@ -51,9 +51,12 @@ struct vpmc {
 
     // work mapping (dose mode): [n_batches * n_spots + 1]
     DevBuf cum, first;
-    DevBuf s0, s1, s2;                // source records of a chunk
-    DevBuf q0, q1, q2, q3, q4;        // survivor queue (grown to the chunk size in use)
-    unsigned int *d_qctr = nullptr;   // [0] queue count, [1] queue head, [2] source-record counter of beam_kernel
+    DevBuf s0, s1, s2;                // range-shifter records of a chunk
+    DevBuf a0, a1, a2, a3, a4;        // queue range shifter -> aperture entry
+    DevBuf b0, b1, b2, b3, b4, b5;    // aperture queue (histories whose next step is a brass step)
+    DevBuf q0, q1, q2, q3, q4;        // CT queue (all grown to the chunk size in use)
+    unsigned int *d_qctr = nullptr;   // counts and heads of the queues of the chunk in flight (vpmc_run.inl)
+    bool any_rs = false, any_ap = false;
 
     // scoring
     DevBuf edep;                      // [n_batches][nvox] E_dep (MeV)
@@ -85,7 +88,7 @@ struct vpmc {
     bool verbose = false;
 
     // launch configuration
-    int grid_beam = 0;                // resident CTAs of beam_kernel
+    int grid_beam[2] = { 0, 0 };      // resident CTAs of beam_kernel<STAGE>
     int grid[3][2] = { { 0, 0 }, { 0, 0 }, { 0, 0 } };   // [mode][smem_lut] resident CTAs of voxel_kernel
     bool smem_lut = false;
     size_t lut_bytes = 0, tally_smem = 0;

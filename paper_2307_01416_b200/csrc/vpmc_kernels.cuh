@@ -1,7 +1,8 @@
 // vpmc_kernels.cuh -- the sm_100a kernels of the hot path.  See DESIGN.md 5:
-//   source_kernel     S1: one thread per work item -> source record
-//   beam_kernel       S2-S3: persistent warps carry histories through range shifter and aperture; free lanes load the
-//                     next source record (warp-aggregated claim); survivors are pushed to a queue
+//   source_kernel     S1 (+ the opening phase of S3 for beams without range shifter): one thread per work item
+//   beam_kernel<0>    S2: persistent warps carry histories through the range shifter; free lanes load the next record
+//   ap_entry_kernel   S3, opening phase of the histories that left the range shifter, one thread per record
+//   beam_kernel<1>    S3: persistent warps, brass steps of the aperture region; survivors are pushed to the CT queue
 //   entry_kernel      CT entry (fp64), one thread per survivor
 //   voxel_kernel      S4-S7: persistent warps pull survivors from the queue, step through the voxels and score;
 //                     MODE 0 the dose grid(s), MODE 1 per-column boxes + overflow list, MODE 2 only column bounding boxes
@@ -150,26 +151,70 @@ constexpr int kRefillMin = VPK_REFILL_MIN;   // S6b: free lanes are refilled onc
 #define VPK_MIN_BLOCKS 4
 #endif
 
-// source records of a chunk, SoA of 16-byte words
+// range-shifter input records of a chunk (histories on the entrance plane of the range shifter: direction +w, nothing
+// accumulated yet), SoA of 16-byte words
 struct SourceBuf {
     uint4 *s0;    // x hi, x lo, y hi, y lo (beam frame, fp32 pairs)
-    uint4 *s1;    // E, tau_star, col | beam << 24, region
+    uint4 *s1;    // E, tau_star, col | beam << 24, step
     uint4 *s2;    // R lo, R hi, hid_lo, hid_hi
+    unsigned int *count;   // records written
 };
 
-// Histories that left the beam line alive, handed from beam_kernel to voxel_kernel: SoA of 16-byte records (80 B per
-// history), written and read coalesced.  beam_kernel writes the beam-frame state on the exit plane of the last device;
-// entry_kernel rewrites q0 (and the direction) as the CT state.
+// Histories handed from one stage to the next: SoA of 16-byte records (80 B per history, 96 B with q5), written and read
+// coalesced.  Three queues per chunk: range shifter -> aperture entry; aperture entry -> aperture kernel (with q5); CT queue.
+// Beam-line stages write the beam-frame state; entry_kernel rewrites q0 (and the direction) of the CT queue as the CT state.
 struct Queue {
     uint4 *q0;    // beam frame: x hi, x lo, y hi, y lo;  CT: local x, y, z (fp32), voxel index (0xffffffff = missed the CT)
     float4 *q1;   // ux, uy, uz, E
     float4 *q2;   // lx, ly, lz, t_rad
     uint4 *q3;    // tau, tau_star, step, col | beam << 24
     uint4 *q4;    // R lo, R hi, hid_lo, hid_hi
+    float4 *q5;   // aperture queue only: brass budget (h.rx), depth inside the aperture region (h.rz), -, -
     unsigned int *count;   // entries pushed
-    unsigned int *head;    // entries claimed by the voxel kernel
+    unsigned int *head;    // entries claimed by the consuming persistent kernel
     unsigned int capacity;
 };
+
+// slot of this lane in a queue: one atomic per warp.  Must be called by all 32 lanes.
+__device__ __forceinline__ unsigned int warp_push_slot(unsigned int *counter, bool want, int lane)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, want);
+    if (m == 0u) return 0u;
+    unsigned base = 0;
+    const int leader = __ffs(m) - 1;
+    if (lane == leader) base = atomicAdd(counter, (unsigned)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    return base + (unsigned)__popc(m & lanemask_lt());
+}
+
+__device__ __forceinline__ void queue_store(const Queue &q, unsigned int slot, const Hist &h)
+{
+    if (slot >= q.capacity) return;
+    q.q0[slot] = make_uint4(h.g0, h.g1, h.g2, h.g3);
+    q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.E);
+    q.q2[slot] = make_float4(h.lx, h.ly, h.lz, h.t_rad);
+    q.q3[slot] = make_uint4(__float_as_uint(h.tau), __float_as_uint(h.tau_star), h.step, (unsigned)h.col | ((unsigned)(h.region >> 8) << 24));
+    const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
+    q.q4[slot] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
+    if (q.q5) q.q5[slot] = make_float4(h.rx, h.rz, 0.0f, 0.0f);
+}
+
+// beam-frame record -> history standing in region `reg` (REG_TO_AP after the range shifter, REG_AP from the aperture queue)
+__device__ __forceinline__ void queue_load_beam(const Queue &q, unsigned int slot, int reg, float c_log, Hist &h)
+{
+    const uint4 p0 = q.q0[slot];
+    const float4 a = q.q1[slot], b = q.q2[slot];
+    const uint4 e = q.q3[slot], f = q.q4[slot];
+    h.g0 = p0.x; h.g1 = p0.y; h.g2 = p0.z; h.g3 = p0.w;
+    h.ux = a.x; h.uy = a.y; h.uz = a.z; h.E = a.w;
+    h.lx = b.x; h.ly = b.y; h.lz = b.z; h.t_rad = b.w; h.f_rad = highland_f(b.w, c_log);
+    h.tau = __uint_as_float(e.x); h.tau_star = __uint_as_float(e.y); h.step = e.z;
+    h.col = (int)(e.w & 0xffffffu); h.region = reg | (int)((e.w >> 24) << 8);
+    h.R = __longlong_as_double((long long)(((unsigned long long)f.y << 32) | f.x));
+    h.hid_lo = f.z; h.hid_hi = f.w;
+    h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
+    if (q.q5) { const float4 g = q.q5[slot]; h.rx = g.x; h.rz = g.y; }
+}
 
 // per-warp flush of the tallies: lane counters into the warp's shared slots, then <= 13 global atomics per warp
 __device__ __forceinline__ void flush_warp_tallies(WarpTally *w, const LaneCounters &lc, DevTallies *tal, int lane)
@@ -184,105 +229,157 @@ __device__ __forceinline__ void flush_warp_tallies(WarpTally *w, const LaneCount
     if (lane < TC_N && w->c[lane]) atomicAdd(&tal->n_stopped_ct + lane, (unsigned long long)w->c[lane]);
 }
 
-// S1: items [item0, item0 + n) -> source records [0, n)
+// a history that ended as ESCAPED in one of the one-thread-per-history kernels (u_w <= 0 in the beam line: never with the
+// closed-form physics at these energies, kept for the rule of C4): booked with plain warp-reduced atomics
+__device__ __forceinline__ void book_escapes_converged(DevTallies *tal, bool esc, float E, unsigned int steps)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, esc);
+    if (m == 0u) return;
+    const double e = warp_sum(esc ? (double)E : 0.0);
+    const unsigned n_dev = __reduce_add_sync(0xffffffffu, esc ? steps : 0u);
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&tal->escaped, e);
+        atomicAdd(&tal->n_escaped, (unsigned long long)__popc(m));
+        atomicAdd(&tal->n_steps_dev, (unsigned long long)n_dev);
+    }
+}
+
+// S1 + the converged part of S3: items [item0, item0 + n) -> sampled histories, each routed to the stage it needs next:
+//   beam with a range shifter        -> range-shifter input record (on its entrance plane);
+//   aperture only, clean transit     -> CT queue (the whole opening phase of P:L87 runs here, converged);
+//   aperture only, brass step due    -> aperture queue;
+//   no device                        -> CT queue.
 __global__ void __launch_bounds__(kBlock)
 source_kernel(const Ctx c, const WorkMap wm, const unsigned long long item0, const float4 *__restrict__ spots,
-              const double *__restrict__ spot_R0, const int *__restrict__ spot_beam, const SourceBuf sb, DevTallies *tal)
+              const double *__restrict__ spot_R0, const int *__restrict__ spot_beam, const SourceBuf sb, const Queue q_ap,
+              const Queue q_ct, DevTallies *tal)
 {
     const unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
     double inc = 0.0;
+    int dest = 0;                      // 1 range shifter, 2 aperture queue, 3 CT queue, 4 escaped
+    Hist h;
+    h.E = 0.0f; h.step = 0u; h.region = 0;
     if (k < wm.n_items) {
-        Hist h;
         int g; unsigned long long hid;
         map_item(wm, item0 + k, g, hid, h.col);
         h.hid_lo = (uint32_t)hid; h.hid_hi = (uint32_t)(hid >> 32);
         const int beam = __ldg(spot_beam + g);
         sample_source(c.P, c.beams[beam], beam, __ldg(spots + g), __ldg(spot_R0 + g), h, c.K);
         inc = (double)h.E;
-        const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
-        sb.s0[k] = make_uint4(h.g0, h.g1, h.g2, h.g3);
-        sb.s1[k] = make_uint4(__float_as_uint(h.E), __float_as_uint(h.tau_star), (unsigned)h.col | ((unsigned)beam << 24), (unsigned)(h.region & 0xff));
-        sb.s2[k] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
+        NullTracer tr;
+        const int reg = h.region & 0xff;
+        if (reg == REG_TO_RS) dest = (rs_enter(c, h, tr) == BEAM_CONT) ? 1 : 4;
+        else if (reg == REG_TO_AP) { const int st = ap_enter(c, h, tr); dest = (st == BEAM_EXIT) ? 3 : (st == BEAM_CONT ? 2 : 4); }
+        else dest = 3;
     }
+    const unsigned s_rs = warp_push_slot(sb.count, dest == 1, lane);
+    const unsigned s_ap = warp_push_slot(q_ap.count, dest == 2, lane);
+    const unsigned s_ct = warp_push_slot(q_ct.count, dest == 3, lane);
+    if (dest == 1) {
+        const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
+        sb.s0[s_rs] = make_uint4(h.g0, h.g1, h.g2, h.g3);
+        sb.s1[s_rs] = make_uint4(__float_as_uint(h.E), __float_as_uint(h.tau_star), (unsigned)h.col | ((unsigned)(h.region >> 8) << 24), h.step);
+        sb.s2[s_rs] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
+    } else if (dest == 2) queue_store(q_ap, s_ap, h);
+    else if (dest == 3) queue_store(q_ct, s_ct, h);
+    book_escapes_converged(tal, dest == 4, h.E, h.step);
     inc = warp_sum(inc);
-    if ((threadIdx.x & 31) == 0 && inc != 0.0) atomicAdd(&tal->incident, inc);
+    if (lane == 0 && inc != 0.0) atomicAdd(&tal->incident, inc);
 }
 
-// S2-S3: persistent warps; every lane carries one history through the beam line with beam_step(); a lane whose history
-// ended or left the beam line loads the next source record (warp-aggregated claim on the item counter).  Survivors are
-// pushed to the queue with one atomic per warp and iteration.
+// Aperture entry of the histories that left the range shifter, one thread per record: vacuum drift to the aperture
+// entrance and the opening phase (ap_enter) -> CT queue (clean transit, or no aperture) | aperture queue (brass step due)
+__global__ void __launch_bounds__(kBlock)
+ap_entry_kernel(const Ctx c, const Queue q_in, const Queue q_ap, const Queue q_ct, DevTallies *tal)
+{
+    const unsigned n_q = min(*q_in.count, q_in.capacity);
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int dest = 0;
+    Hist h;
+    h.E = 0.0f; h.step = 0u;
+    if (i < n_q) {
+        queue_load_beam(q_in, i, REG_TO_AP, c.P.c_log, h);
+        if (__ldg(&c.beams[h.region >> 8].has_ap)) {
+            NullTracer tr;
+            const int st = ap_enter(c, h, tr);
+            dest = (st == BEAM_EXIT) ? 3 : (st == BEAM_CONT ? 2 : 4);
+        } else { h.region = REG_TO_CT | (h.region & ~0xff); dest = 3; }
+    }
+    const unsigned s_ap = warp_push_slot(q_ap.count, dest == 2, lane);
+    const unsigned s_ct = warp_push_slot(q_ct.count, dest == 3, lane);
+    if (dest == 2) queue_store(q_ap, s_ap, h);
+    else if (dest == 3) queue_store(q_ct, s_ct, h);
+    book_escapes_converged(tal, dest == 4, h.E, h.step);
+}
+
+// S2 / S3: persistent warps; every lane carries one history through ONE device -- STAGE 0 the range shifter (input: the
+// range-shifter records), STAGE 1 the brass of the aperture region (input: the aperture queue).  A lane whose history ended
+// or left the device loads the next record (warp-aggregated claim on the input counter); histories that left the device
+// alive are pushed to `out` (STAGE 0: the aperture-entry queue, STAGE 1: the CT queue) with one atomic per warp and pass.
+template <int STAGE>
 __global__ void __launch_bounds__(kBlock, VPK_MIN_BLOCKS)
-beam_kernel(const Ctx c, const unsigned int n_items, const SourceBuf sb, const Queue q, unsigned int *counter, DevTallies *tal)
+beam_kernel(const Ctx c, const SourceBuf sb, const Queue in, const Queue out, unsigned int *head, DevTallies *tal)
 {
     __shared__ WarpTally wt_all[kWarps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x < kWarps * (int)(sizeof(WarpTally) / 4)) reinterpret_cast<unsigned int *>(wt_all)[threadIdx.x] = 0u;
     __syncthreads();
-    const SmemSink sink{ wt_all + warp };
     NullTracer tr;
     LaneCounters lc;
     Hist h;
     h.region = REG_TO_CT; h.col = 0; h.step = 0u; h.E = 0.0f; h.R = 0.0;
-    float dep_rs = 0.0f, dep_ap = 0.0f;
+    float dep = 0.0f;                      // energy deposited in this device so far
+    const unsigned int n_items = (STAGE == 0) ? *sb.count : min(*in.count, in.capacity);
     int pend = BEAM_CONT;                  // status of a finished history whose bookkeeping is still due
     bool alive = false, exhausted = false;
     for (;;) {
         // S6b, event pass: once enough lanes are free, book their finished histories, push the survivors to the queue and
-        // load the next source records -- all of it converged over those lanes
+        // load the next records -- all of it converged over those lanes
         const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
         const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != BEAM_CONT);
         const int n_free = __popc(free_mask);
         if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
-            const unsigned out_mask = __ballot_sync(0xffffffffu, !alive && pend == BEAM_EXIT);
-            if (out_mask) {                // survivors -> queue (one atomic per warp)
-                unsigned base = 0;
-                const int leader = __ffs(out_mask) - 1;
-                if (lane == leader) base = atomicAdd(q.count, (unsigned)__popc(out_mask));
-                base = __shfl_sync(0xffffffffu, base, leader);
-                if (!alive && pend == BEAM_EXIT) {
-                    const unsigned slot = base + __popc(out_mask & lanemask_lt());
-                    if (slot < q.capacity) {
-                        q.q0[slot] = make_uint4(h.g0, h.g1, h.g2, h.g3);
-                        q.q1[slot] = make_float4(h.ux, h.uy, h.uz, h.E);
-                        q.q2[slot] = make_float4(h.lx, h.ly, h.lz, h.t_rad);
-                        q.q3[slot] = make_uint4(__float_as_uint(h.tau), __float_as_uint(h.tau_star), h.step,
-                                                (unsigned)h.col | ((unsigned)(h.region >> 8) << 24));
-                        const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
-                        q.q4[slot] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
-                    }
-                }
-            }
-            if (!alive && pend != BEAM_CONT) { book_beam_end(c.P, h, pend, dep_rs, dep_ap, lc, sink); pend = BEAM_CONT; }
+            const bool push = !alive && pend == BEAM_EXIT;
+            const unsigned slot = warp_push_slot(out.count, push, lane);
+            if (push) queue_store(out, slot, h);
+            book_beam_end(c.P, h, !alive && pend != BEAM_CONT, pend, dep, STAGE == 0 ? TD_DEP_RS : TD_DEP_BRASS, lc, wt_all + warp, lane);
+            pend = alive ? pend : BEAM_CONT;
             if (!exhausted) {
                 unsigned base = 0;
                 const int leader = __ffs(free_mask) - 1;
-                if (lane == leader) base = atomicAdd(counter, (unsigned)n_free);
+                if (lane == leader) base = atomicAdd(head, (unsigned)n_free);
                 base = __shfl_sync(0xffffffffu, base, leader);
                 exhausted = base + (unsigned)n_free >= n_items;
                 if (!alive) {
                     const unsigned k = base + __popc(free_mask & lanemask_lt());
                     if (k < n_items) {
-                        const uint4 a = sb.s0[k], b = sb.s1[k], e = sb.s2[k];
-                        h.g0 = a.x; h.g1 = a.y; h.g2 = a.z; h.g3 = a.w;
-                        h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
-                        h.E = __uint_as_float(b.x); h.tau_star = __uint_as_float(b.y);
-                        h.col = (int)(b.z & 0xffffffu); h.region = (int)b.w | (int)((b.z >> 24) << 8);
-                        h.R = __longlong_as_double((long long)(((unsigned long long)e.y << 32) | e.x));
-                        h.hid_lo = e.z; h.hid_hi = e.w;
-                        h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f; h.step = 0u;
-                        h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
-                        dep_rs = 0.0f; dep_ap = 0.0f;
+                        if (STAGE == 0) {
+                            const uint4 a = sb.s0[k], b = sb.s1[k], e = sb.s2[k];
+                            h.g0 = a.x; h.g1 = a.y; h.g2 = a.z; h.g3 = a.w;
+                            h.rx = 0.0f; h.ry = 0.0f; h.rz = 0.0f;
+                            h.E = __uint_as_float(b.x); h.tau_star = __uint_as_float(b.y);
+                            h.col = (int)(b.z & 0xffffffu); h.region = REG_RS | (int)((b.z >> 24) << 8);
+                            h.step = b.w;
+                            h.R = __longlong_as_double((long long)(((unsigned long long)e.y << 32) | e.x));
+                            h.hid_lo = e.z; h.hid_hi = e.w;
+                            h.tau = 0.0f; h.t_rad = 0.0f; h.f_rad = 1.0f;
+                            h.ux = 0.0f; h.uy = 0.0f; h.uz = 1.0f; h.lx = 0.0f; h.ly = 0.0f; h.lz = 0.0f;
+                        } else queue_load_beam(in, k, REG_AP, c.P.c_log, h);
+                        dep = 0.0f;
                         alive = true;
                     }
                 }
             }
         }
-        if (!__any_sync(0xffffffffu, alive)) {
+        const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+        if (alive_mask == 0u) {
             if (exhausted && !__any_sync(0xffffffffu, pend != BEAM_CONT)) break;
             continue;
         }
         if (alive) {
-            const int status = beam_step(c, h, dep_rs, dep_ap, lc, tr);
+            const int status = (STAGE == 0) ? rs_iter(c, h, dep, lc, tr) : ap_iter(c, h, dep, lc, tr, alive_mask);
             if (status != BEAM_CONT) { alive = false; pend = status; }
         }
     }
@@ -341,7 +438,6 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
     if (SMEM_LUT)
         for (int i = threadIdx.x; i < c.G.n_lut; i += blockDim.x) lut_s[i] = lut_g[i];
     __syncthreads();
-    const SmemSink sink{ wt_all + warp };
     typename ScorerOf<MODE>::type sc = make_scorer<MODE>(sa);
     NullTracer tr;
     LaneCounters lc;
@@ -358,7 +454,9 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != CONT);
         const int n_free = __popc(free_mask);
         if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
-            if (!alive && pend != CONT) { sc.end(h); book_ct_end(c.P, h, pend, hdep, sink); pend = CONT; }
+            if (!alive && pend != CONT) sc.end(h);
+            book_ct_end(c.P, h, !alive && pend != CONT, pend, hdep, wt_all + warp, lane);
+            pend = alive ? pend : CONT;
             if (!exhausted) {
                 unsigned base = 0;
                 const int leader = __ffs(free_mask) - 1;

@@ -110,42 +110,82 @@ static Ctx make_ctx(const vpmc_t *h, const vpmc_scenario &sc, uint64_t seed)
     return c;
 }
 
-// the hot path over wm.n_items work items, in chunks of h->chunk: source (S1) -> beam line (S2-S3) -> CT entry -> voxel
-// stepping + scoring (S4-S7)
+// buffers of one chunk of `cap` work items: range-shifter records, the three queues
+struct ChunkBufs { SourceBuf sb; Queue q_rs_out, q_ap, q_ct; unsigned int *rs_head, *ap_head; };
+
+static int chunk_buffers(vpmc_t *h, unsigned long long cap, ChunkBufs &cb)
+{
+    bool any_rs = false, any_ap = false;
+    for (const BeamHost &b : h->beams) { any_rs = any_rs || b.rs_wet > 0.0f; any_ap = any_ap || b.has_ap; }
+    h->any_rs = any_rs; h->any_ap = any_ap;
+    int rc;
+    DevBuf *ct[5] = { &h->q0, &h->q1, &h->q2, &h->q3, &h->q4 };
+    for (DevBuf *b : ct) if ((rc = ensure(h, *b, cap * 16))) return rc;
+    if (any_rs) {
+        DevBuf *rs[8] = { &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4 };
+        for (DevBuf *b : rs) if ((rc = ensure(h, *b, cap * 16))) return rc;
+    }
+    if (any_ap) {
+        DevBuf *ap[6] = { &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5 };
+        for (DevBuf *b : ap) if ((rc = ensure(h, *b, cap * 16))) return rc;
+    }
+    unsigned int *ctr = h->d_qctr;      // [0] CT count, [1] CT head, [2] rs records, [3] rs head, [4] rs-out count, [5] ap count, [6] ap head
+    cb.sb.s0 = h->s0.as<uint4>(); cb.sb.s1 = h->s1.as<uint4>(); cb.sb.s2 = h->s2.as<uint4>(); cb.sb.count = ctr + 2;
+    cb.rs_head = ctr + 3; cb.ap_head = ctr + 6;
+    Queue &z = cb.q_ct;
+    z.q0 = h->q0.as<uint4>(); z.q1 = h->q1.as<float4>(); z.q2 = h->q2.as<float4>(); z.q3 = h->q3.as<uint4>(); z.q4 = h->q4.as<uint4>(); z.q5 = nullptr;
+    z.count = ctr; z.head = ctr + 1; z.capacity = (unsigned int)cap;
+    Queue &a = cb.q_rs_out;
+    a.q0 = h->a0.as<uint4>(); a.q1 = h->a1.as<float4>(); a.q2 = h->a2.as<float4>(); a.q3 = h->a3.as<uint4>(); a.q4 = h->a4.as<uint4>(); a.q5 = nullptr;
+    a.count = ctr + 4; a.head = nullptr; a.capacity = (unsigned int)cap;
+    Queue &b = cb.q_ap;
+    b.q0 = h->b0.as<uint4>(); b.q1 = h->b1.as<float4>(); b.q2 = h->b2.as<float4>(); b.q3 = h->b3.as<uint4>(); b.q4 = h->b4.as<uint4>(); b.q5 = h->b5.as<float4>();
+    b.count = ctr + 5; b.head = ctr + 6; b.capacity = (unsigned int)cap;
+    return VPMC_OK;
+}
+
+// one chunk of the hot path on stream st: source + opening phase (S1, S3) -> range shifter (S2) -> aperture entry -> brass
+// (S3) -> CT entry -> voxel stepping + scoring (S4-S7).  Plain launches, so the sequence can also be captured into a graph.
+template <int MODE>
+static void enqueue_chunk(vpmc_t *h, const Ctx &c, const WorkMap &wm, unsigned long long i0, const ChunkBufs &cb, const ScoreArgs &sa,
+                          DevTallies *tal, cudaStream_t st, bool timed)
+{
+    const unsigned int n = (unsigned int)wm.n_items;
+    const int blocks = (int)((n + kBlock - 1) / kBlock);
+    cudaMemsetAsync(h->d_qctr, 0, 8 * sizeof(unsigned int), st);
+    {
+        TimedScope ts(h, st, 0, timed);
+        source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, i0, h->d_spots, h->d_spot_R0, h->d_spot_beam, cb.sb, cb.q_ap, cb.q_ct, tal);
+        if (h->any_rs) {
+            beam_kernel<0><<<std::min(h->grid_beam[0], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_rs_out, cb.q_rs_out, cb.rs_head, tal);
+            ap_entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_rs_out, cb.q_ap, cb.q_ct, tal);
+        }
+        if (h->any_ap) beam_kernel<1><<<std::min(h->grid_beam[1], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_ap, cb.q_ct, cb.ap_head, tal);
+    }
+    TimedScope ts(h, st, 1, timed);
+    entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_ct, tal);
+    if (h->smem_lut)
+        voxel_kernel<MODE, true><<<std::min(h->grid[MODE][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, cb.q_ct, h->d_lut, sa, tal);
+    else
+        voxel_kernel<MODE, false><<<std::min(h->grid[MODE][0], blocks), kBlock, h->tally_smem, st>>>(c, cb.q_ct, h->d_lut, sa, tal);
+}
+
+static unsigned int chunk_launches(const vpmc_t *h) { return 3u + (h->any_rs ? 2u : 0u) + (h->any_ap ? 1u : 0u); }
+
+// the hot path over wm.n_items work items, in chunks of h->chunk
 template <int MODE>
 static int launch_transport(vpmc_t *h, const Ctx &c, const WorkMap &wm0, const ScoreArgs &sa, DevTallies *tal, cudaStream_t st)
 {
     if (wm0.n_items == 0) return VPMC_OK;
     const unsigned long long cap = std::min<unsigned long long>(wm0.n_items, h->chunk);
-    int rc;
-    if ((rc = ensure(h, h->s0, cap * sizeof(uint4))) || (rc = ensure(h, h->s1, cap * sizeof(uint4))) || (rc = ensure(h, h->s2, cap * sizeof(uint4))) ||
-        (rc = ensure(h, h->q0, cap * sizeof(uint4))) || (rc = ensure(h, h->q1, cap * sizeof(float4))) || (rc = ensure(h, h->q2, cap * sizeof(float4))) ||
-        (rc = ensure(h, h->q3, cap * sizeof(uint4))) || (rc = ensure(h, h->q4, cap * sizeof(uint4)))) return rc;
-    SourceBuf sb;
-    sb.s0 = h->s0.as<uint4>(); sb.s1 = h->s1.as<uint4>(); sb.s2 = h->s2.as<uint4>();
-    Queue q;
-    q.q0 = h->q0.as<uint4>(); q.q1 = h->q1.as<float4>(); q.q2 = h->q2.as<float4>(); q.q3 = h->q3.as<uint4>(); q.q4 = h->q4.as<uint4>();
-    q.count = h->d_qctr; q.head = h->d_qctr + 1; q.capacity = (unsigned int)cap;
+    ChunkBufs cb;
+    int rc = chunk_buffers(h, cap, cb); if (rc) return rc;
     for (unsigned long long i0 = 0; i0 < wm0.n_items; i0 += h->chunk) {
         WorkMap wm = wm0;
         wm.n_items = std::min<unsigned long long>(h->chunk, wm0.n_items - i0);
-        const unsigned int n = (unsigned int)wm.n_items;
-        const int blocks = (int)((n + kBlock - 1) / kBlock);
-        CU(h, cudaMemsetAsync(h->d_qctr, 0, 4 * sizeof(unsigned int), st));
-        {
-            TimedScope ts(h, st, 0);
-            source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, i0, h->d_spots, h->d_spot_R0, h->d_spot_beam, sb, tal);
-            beam_kernel<<<std::min(h->grid_beam, blocks), kBlock, 0, st>>>(c, n, sb, q, h->d_qctr + 2, tal);
-        }
+        enqueue_chunk<MODE>(h, c, wm, i0, cb, sa, tal, st, true);
         CU(h, cudaGetLastError());
-        TimedScope ts(h, st, 1);
-        entry_kernel<<<blocks, kBlock, 0, st>>>(c, q, tal);
-        if (h->smem_lut)
-            voxel_kernel<MODE, true><<<std::min(h->grid[MODE][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, q, h->d_lut, sa, tal);
-        else
-            voxel_kernel<MODE, false><<<std::min(h->grid[MODE][0], blocks), kBlock, h->tally_smem, st>>>(c, q, h->d_lut, sa, tal);
-        CU(h, cudaGetLastError());
-        h->launches += 4;
+        h->launches += chunk_launches(h);
     }
     return VPMC_OK;
 }
@@ -286,12 +326,10 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
         CU(h, cudaMalloc(&h->d_s1, h->nvox * sizeof(float)));
         CU(h, cudaMalloc(&h->d_s2, h->nvox * sizeof(float)));
     }
-    const unsigned long long cap = batch_histories;
+    ChunkBufs cb;
     if ((rc = ensure(h, h->edep, (size_t)h->nvox * sizeof(float))) ||
         (rc = ensure(h, h->cum, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) || (rc = ensure(h, h->first, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) ||
-        (rc = ensure(h, h->s0, cap * sizeof(uint4))) || (rc = ensure(h, h->s1, cap * sizeof(uint4))) || (rc = ensure(h, h->s2, cap * sizeof(uint4))) ||
-        (rc = ensure(h, h->q0, cap * sizeof(uint4))) || (rc = ensure(h, h->q1, cap * sizeof(float4))) || (rc = ensure(h, h->q2, cap * sizeof(float4))) ||
-        (rc = ensure(h, h->q3, cap * sizeof(uint4))) || (rc = ensure(h, h->q4, cap * sizeof(uint4)))) return rc;
+        (rc = chunk_buffers(h, batch_histories, cb))) return rc;
     // C2 for one batch: ids i in [0, N_b) contiguous per spot in spot order (the batch index goes into the id's high word)
     std::vector<unsigned long long> cnt, cum(h->n_spots + 1, 0ull), first(h->n_spots + 1, 0ull);
     apportion(batch_histories, h->spot_w, cnt);
@@ -311,13 +349,6 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     wm.n_entries = h->n_spots; wm.n_spots = h->n_spots; wm.batch_hi = &h->d_seq->batch;
     ScoreArgs sa{};
     sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->nvox;
-    SourceBuf sb;
-    sb.s0 = h->s0.as<uint4>(); sb.s1 = h->s1.as<uint4>(); sb.s2 = h->s2.as<uint4>();
-    Queue q;
-    q.q0 = h->q0.as<uint4>(); q.q1 = h->q1.as<float4>(); q.q2 = h->q2.as<float4>(); q.q3 = h->q3.as<uint4>(); q.q4 = h->q4.as<uint4>();
-    q.count = h->d_qctr; q.head = h->d_qctr + 1; q.capacity = (unsigned int)cap;
-    const unsigned int n = (unsigned int)batch_histories;
-    const int blocks = (int)((n + kBlock - 1) / kBlock);
     const int gv = grid_for(h->nvox, h->n_sm);
 
     // the graph: one WHILE node whose body is the batch pass
@@ -332,14 +363,7 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     CU(h, cudaGraphAddNode(&node, h->seq_graph, nullptr, 0, &np));
     cudaGraph_t body = np.conditional.phGraph_out[0];
     CU(h, cudaStreamBeginCaptureToGraph(st, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
-    cudaMemsetAsync(h->d_qctr, 0, 4 * sizeof(unsigned int), st);
-    source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, 0ull, h->d_spots, h->d_spot_R0, h->d_spot_beam, sb, h->d_tal);
-    beam_kernel<<<std::min(h->grid_beam, blocks), kBlock, 0, st>>>(c, n, sb, q, h->d_qctr + 2, h->d_tal);
-    entry_kernel<<<blocks, kBlock, 0, st>>>(c, q, h->d_tal);
-    if (h->smem_lut)
-        voxel_kernel<0, true><<<std::min(h->grid[0][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, q, h->d_lut, sa, h->d_tal);
-    else
-        voxel_kernel<0, false><<<std::min(h->grid[0][0], blocks), kBlock, h->tally_smem, st>>>(c, q, h->d_lut, sa, h->d_tal);
+    enqueue_chunk<0>(h, c, wm, 0ull, cb, sa, h->d_tal, st, false);
     seq_accumulate_kernel<<<gv, 256, 0, st>>>(h->edep.as<float>(), h->d_s1, h->d_s2, h->nvox, h->d_seq);
     seq_uncertainty_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_s2, h->nvox, h->d_seq);
     seq_decide_kernel<<<1, 1, 0, st>>>(handle, h->d_seq, (int)min_batches, (int)max_batches, target_rel_unc);
@@ -366,7 +390,7 @@ extern "C" int vpmc_get_run_info(vpmc_t *h, int32_t *batches_out, float *rel_unc
     CU(h, cudaStreamSynchronize(h->seq_stream));
     SeqState s;
     CU(h, cudaMemcpy(&s, h->d_seq, sizeof(s), cudaMemcpyDeviceToHost));
-    if (h->seq_exec) { h->launches += 7ull * s.batch + 1ull; seq_release(h); }     // counted once, when the result is read
+    if (h->seq_exec) { h->launches += (unsigned long long)(chunk_launches(h) + 3u) * s.batch + 1ull; seq_release(h); }     // counted once, when the result is read
     if (batches_out) *batches_out = (int32_t)s.batch;
     if (rel_unc_out) *rel_unc_out = s.unc;
     if (reached_target_out) *reached_target_out = (int32_t)s.stopped_by_target;

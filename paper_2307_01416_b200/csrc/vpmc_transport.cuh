@@ -259,182 +259,278 @@ struct NullScorer {
 struct LutShared { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return p[i]; } };
 struct LutGlobal { const float4 *p; __device__ __forceinline__ float4 operator[](int i) const { return __ldg(p + i); } };
 
-// status of a history after beam_step(): still in the beam line, on the exit plane of the last device, or ended
+// status of a history after an iteration in the beam line: still inside, on the exit plane of its device, or ended
 enum : int { BEAM_CONT = 0, BEAM_EXIT = 1, BEAM_STOPPED = 2, BEAM_NUCLEAR = 3, BEAM_ESCAPED = 4 };
 
-// One iteration of history h in the beam line: pending vacuum drifts, the drifts through the opening (safe-distance
-// skipping makes a clean transit one pass of the loop), then at most ONE slab step (range shifter or brass).  Returns the
-// BEAM_* status; when the history ended, h.region holds the region it ended in and h.E the energy it had left.
-// Nothing is tallied here: the once-per-history bookkeeping is done by book_beam_end() in the kernel's refill pass,
-// where several lanes do it together (a rare per-lane event inside the step loop costs the whole warp a pass).
-// dep_rs / dep_ap = energy deposited so far in range shifter / brass.
-template <class Tracer>
-__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, float &dep_ap, LaneCounters &lc, Tracer &tr)
-{
-    // Single-exit structured control flow on purpose: every lane passes through `if (do_step)`, so lanes that stand in
-    // different regions re-converge BEFORE the expensive slab step.  (With early returns the re-convergence point of the
-    // region branches moves to the end of the function and range-shifter and brass lanes execute the step in turns:
-    // measured 17 of 32 lanes active, profiles/r1c.)
-    const DevParams &P = c.P;
-    int reg = h.region & 0xff;
-    const int beam_bits = h.region & ~0xff;
-    const DevBeam *bp = c.beams + (h.region >> 8);
-    Medium m = { 1.0f, 1.0f, 1.0f, 0.0f, 0.0f };
-    float d = 0.0f, T = 0.0f, w_in = 0.0f;
-    bool ex = false, do_step = false, esc = false;
-    int status = BEAM_CONT;
-    const unsigned conv = __activemask();      // the lanes that entered together re-converge before the slab step
+// The beam line is cut into STAGES, each run by its own kernel so that a warp only ever holds histories that execute the
+// same code:
+//   rs_enter  + rs_iter   range shifter: vacuum drift to its entrance (once), then one slab step per iteration;
+//   ap_enter              vacuum drift to the aperture entrance and the OPENING PHASE: the per-step medium test of P:L87
+//                         and the drifts through the opening, until a brass step is due or the exit plane is reached --
+//                         run converged, one thread per history, by source_kernel / ap_entry_kernel;
+//   ap_iter               one iteration inside the aperture region: brass slab step (the opening phase again only for
+//                         the few histories that scatter back into the opening).
+// beam_step() strings the same functions together for the trace kernels, so a trace records exactly what the production
+// kernels compute.
 
-    if (reg == REG_TO_CT) status = BEAM_EXIT;              // no device at all
-    if (reg == REG_TO_RS) {
-        const float w1 = __ldg(&bp->w_rs_in);
-        w_in = __ldg(&bp->w_start);
-        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else reg = REG_RS;
+// slab geometry, common to range shifter and aperture region: distance to the exit plane, fixed step (C4: d = min(s_rs |
+// s_ap, distance to the exit plane))
+struct SlabGeom { float w_in, T, d; bool ex; };
+
+__device__ __forceinline__ void slab_geometry(const DevParams &P, const DevBeam *bp, bool rs, const Hist &h, SlabGeom &g)
+{
+    const float *wp = rs ? &bp->w_rs_in : &bp->w_ap_in;
+    g.w_in = __ldg(wp);
+    g.T = __ldg(wp + 1) - g.w_in;
+    g.d = rs ? P.s_rs : P.s_ap; g.ex = false;
+    const float rem = g.T - h.rz;
+    if (rem <= g.d * h.uz) { g.d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); g.ex = true; }
+}
+
+// one slab step (range shifter or brass): C4 items 1-8 and 10.  `out` = the history reached the exit plane of the device.
+template <class Tracer>
+__device__ __forceinline__ int slab_step(const Ctx &c, Hist &h, const Medium &m, const SlabGeom &g, int reg, float &dep,
+                                         LaneCounters &lc, Tracer &tr, bool &out)
+{
+    StepOut o;
+    const float Eb = h.E; const uint32_t st = h.step;
+    const float lat = fmaxf(fabsf(h.ux), fabsf(h.uy));        // direction of travel during the step
+    const int cause = step_physics(c.P, h, m, g.d, c.K, o);
+    h.rx = fmaf(-o.s, lat, h.rx);                              // brass budget (meaningless, and unused, in the range shifter)
+    if (cause == CONT) {
+        // C4-8: move along the OLD direction, then rotate
+        pair_axpy(h.g0, h.g1, o.s, h.ux, h.lx);
+        pair_axpy(h.g2, h.g3, o.s, h.uy, h.ly);
+        h.rz = fmaf(o.s, h.uz, h.rz);
+        if (c.P.flags & 1) rotate(h, o.theta, o.uphi);
     }
-    if (reg == REG_TO_AP) {
-        const float w1 = __ldg(&bp->w_ap_in);
-        w_in = __ldg(&bp->has_rs) ? __ldg(&bp->w_rs_out) : __ldg(&bp->w_start);
-        if (drift_gap(h, w1 - w_in, w1, tr) != CONT) esc = true; else { reg = REG_AP; h.rx = 0.0f; }
-    }
-    // slab geometry, common to range shifter and aperture region: distance to the exit plane, fixed step
-    if ((reg == REG_RS || reg == REG_AP) && !esc) {
-        if (!(h.uz > 0.0f)) esc = true;
-        else {
-            const bool rs = reg == REG_RS;
-            const float *wp = rs ? &bp->w_rs_in : &bp->w_ap_in;
-            w_in = __ldg(wp);
-            T = __ldg(wp + 1) - w_in;
-            d = rs ? P.s_rs : P.s_ap; ex = false;
-            const float rem = T - h.rz;
-            if (rem <= d * h.uz) { d = fmaxf(__fdiv_rn(rem, h.uz), 0.0f); ex = true; }
-            m = rs ? Medium{ P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho }
-                   : Medium{ P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
-            // h.rx (free in the beam line) = lateral travel, in mm of the L-infinity norm, over which this history is
-            // KNOWN to stay in brass: while it is positive the per-step test of P:L87 can only answer "brass"
-            do_step = rs || h.rx > 0.0f;
+    dep += o.dep;
+    lc.n_slab += (cause != STOPPED);
+    out = (cause == CONT) && o.on_d && g.ex;
+    if (out) h.rz = g.T;
+    if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), g.w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause, o.dep);
+    return cause;
+}
+
+// u_w <= 0 inside the beam line ends the history as ESCAPED (C4, last paragraph)
+template <class Tracer>
+__device__ __forceinline__ int beam_escape(const Hist &h, float w_in, Tracer &tr)
+{
+    if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
+    return BEAM_ESCAPED;
+}
+
+// pending vacuum drift from the start plane to the range-shifter entrance
+template <class Tracer>
+__device__ __forceinline__ int rs_enter(const Ctx &c, Hist &h, Tracer &tr)
+{
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    const float w1 = __ldg(&bp->w_rs_in), w0 = __ldg(&bp->w_start);
+    if (drift_gap(h, w1 - w0, w1, tr) != CONT) return beam_escape(h, w0, tr);
+    h.region = REG_RS | (h.region & ~0xff);
+    return BEAM_CONT;
+}
+
+// one range-shifter step (S2; homogeneous, energy-only medium)
+template <class Tracer>
+__device__ __forceinline__ int rs_iter(const Ctx &c, Hist &h, float &dep_rs, LaneCounters &lc, Tracer &tr)
+{
+    const DevParams &P = c.P;
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    if (!(h.uz > 0.0f)) return beam_escape(h, __ldg(&bp->w_rs_in), tr);
+    SlabGeom g;
+    slab_geometry(P, bp, true, h, g);
+    const Medium m = { P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
+    bool out;
+    const int cause = slab_step(c, h, m, g, REG_RS, dep_rs, lc, tr, out);
+    if (cause != CONT) return (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
+    if (!out) return BEAM_CONT;
+    h.region = (__ldg(&bp->has_ap) ? REG_TO_AP : REG_TO_CT) | (h.region & ~0xff);
+    return BEAM_EXIT;
+}
+
+// S3, opening phase: the medium under the current (u, v) is tested at the start of every step; in the opening the
+// proton drifts with its previous velocity and direction.  Runs until a brass step is due (returns BEAM_CONT; h.rx = lateral
+// travel, in mm of the L-infinity norm, over which the history is KNOWN to stay in brass, > 0; g = geometry of that step) or
+// the exit plane is reached (BEAM_EXIT, region REG_TO_CT).
+// Safe-distance skipping: every tile within Chebyshev distance k - 1 of the current one is fully open, so the next per-step
+// tests are known to answer "open" as long as the lateral travel stays below (k - 1) tiles.
+template <class Tracer>
+__device__ __forceinline__ int ap_open_phase(const Ctx &c, const DevBeam *bp, Hist &h, SlabGeom &g, Tracer &tr)
+{
+    const DevParams &P = c.P;
+    const float T = g.T, w_in = g.w_in;
+    for (;;) {
+        int ix, iy;
+        if (!aperture_open(bp, beam_xh(h), beam_yh(h), ix, iy)) {
+            // brass: how far is the opening?  (k tiles away -> at least (k - 1) tiles of lateral travel are brass)
+            float budget;
+            if (ix >= 0) {
+                const int k = (int)__ldg(bp->ap_dist_open + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
+                budget = 0.99f * (float)(k - 1) * fminf(__ldg(&bp->ap_tile_u), __ldg(&bp->ap_tile_v));
+            } else {      // outside the bitmap: distance to its rectangle
+                const float x = beam_xh(h), y = beam_yh(h), u0 = __ldg(&bp->ap_u0), v0 = __ldg(&bp->ap_v0);
+                const float u1 = u0 + (float)__ldg(&bp->ap_nx) * __frcp_rn(__ldg(&bp->ap_inv_du)), v1 = v0 + (float)__ldg(&bp->ap_ny) * __frcp_rn(__ldg(&bp->ap_inv_dv));
+                budget = 0.99f * fmaxf(fmaxf(u0 - x, x - u1), fmaxf(v0 - y, y - v1));
+            }
+            h.rx = fmaxf(budget, 1e-30f);          // > 0: the step that follows this test IS a brass step
+            return BEAM_CONT;
         }
-    }
-    if (reg == REG_AP && !esc && !do_step) {
-        for (;;) {
-            int ix, iy;
-            if (!aperture_open(bp, beam_xh(h), beam_yh(h), ix, iy)) {
-                // brass: how far is the opening?  (k tiles away -> at least (k - 1) tiles of lateral travel are brass)
-                float budget;
-                if (ix >= 0) {
-                    const int k = (int)__ldg(bp->ap_dist_open + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
-                    budget = 0.99f * (float)(k - 1) * fminf(__ldg(&bp->ap_tile_u), __ldg(&bp->ap_tile_v));
-                } else {      // outside the bitmap: distance to its rectangle
-                    const float x = beam_xh(h), y = beam_yh(h), u0 = __ldg(&bp->ap_u0), v0 = __ldg(&bp->ap_v0);
-                    const float u1 = u0 + (float)__ldg(&bp->ap_nx) * __frcp_rn(__ldg(&bp->ap_inv_du)), v1 = v0 + (float)__ldg(&bp->ap_ny) * __frcp_rn(__ldg(&bp->ap_inv_dv));
-                    budget = 0.99f * fmaxf(fmaxf(u0 - x, x - u1), fmaxf(v0 - y, y - v1));
-                }
-                h.rx = fmaxf(budget, 0.0f);
-                do_step = true;
-                break;
-            }
-            // in the opening the proton is transported with its previous velocity and direction.
-            // Safe-distance skipping: every tile within Chebyshev distance k - 1 of this one is fully open, so the next
-            // per-step tests are known to answer "open" as long as the lateral travel stays below (k - 1) tiles.  nf =
-            // full steps left before the exit step; if all of their tests are known, go straight to the exit plane,
-            // else take the known ones (at least one step) and test again.
-            const float rem = T - h.rz, duz = P.s_ap * h.uz;
-            // nf = number of j >= 0 with rem - j duz > duz (the per-step rule `rem <= d u_w` decides the exit step); the
-            // rounded quotient can be off by one when rem / duz sits next to an integer, so it is checked against that rule
-            int nf = ex ? 0 : max((int)ceilf(__fdiv_rn(rem, duz)) - 1, 0);
-            if (!ex) {
-                if (fmaf(-(float)nf, duz, rem) > duz) nf += 1;
-                else if (nf > 0 && fmaf(-(float)(nf - 1), duz, rem) <= duz) nf -= 1;
-            }
-            float n_safe = 0.0f;
-            if (nf > 0) {
-                const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
-                if (k >= 2) {
-                    const float safe = 0.99f * (float)(k - 1);
-                    const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(P.s_ap * h.ux), 1e-12f));
-                    const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(P.s_ap * h.uy), 1e-12f));
-                    n_safe = floorf(fminf(fminf(nu, nv), 65536.0f));
-                }
-            }
-            const bool whole = n_safe >= (float)nf;            // includes the plain exit step (nf = 0)
-            const int n = whole ? nf : max((int)n_safe, 1);    // full steps taken now
-            if (Tracer::on && n > 0) {     // the same arithmetic, one record per full step
-                const uint32_t g0 = h.g0, g1 = h.g1, g2 = h.g2, g3 = h.g3; const float rz0 = h.rz;
-                for (int j = 1; j <= n; ++j) {
-                    const float sj = (float)j * P.s_ap;
-                    h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3;
-                    pair_axpy(h.g0, h.g1, sj, h.ux, h.lx); pair_axpy(h.g2, h.g3, sj, h.uy, h.ly);
-                    h.rz = fmaf(sj, h.uz, rz0);
-                    tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step + (uint32_t)(j - 1), REG_AP_OPEN, nullptr, h.E, h.E, P.s_ap, CONT);
-                }
-                h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3; h.rz = rz0;
-            }
-            if (whole) {
-                const float rz_nf = fmaf((float)nf * P.s_ap, h.uz, h.rz);                  // depth after the full steps
-                const float d_exit = fmaxf(__fdiv_rn(T - rz_nf, h.uz), 0.0f);
-                const float s_tot = fmaf((float)nf, P.s_ap, d_exit);
-                pair_axpy(h.g0, h.g1, s_tot, h.ux, h.lx); pair_axpy(h.g2, h.g3, s_tot, h.uy, h.ly);
-                h.rz = T;
-                h.step += (uint32_t)(nf + 1);
-                if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + T, h.step - 1u, REG_AP_OPEN, nullptr, h.E, h.E, d_exit, CONT);
-                reg = REG_TO_CT; status = BEAM_EXIT;
-                break;
-            }
-            const float sn = (float)n * P.s_ap;
-            pair_axpy(h.g0, h.g1, sn, h.ux, h.lx); pair_axpy(h.g2, h.g3, sn, h.uy, h.ly);
-            h.rz = fmaf(sn, h.uz, h.rz);
-            h.step += (uint32_t)n;
-            // geometry of the next step
-            d = P.s_ap; ex = false;
-            const float rem2 = T - h.rz;
-            if (rem2 <= d * h.uz) { d = fmaxf(__fdiv_rn(rem2, h.uz), 0.0f); ex = true; }
+        // nf = full steps left before the exit step; if all of their tests are known, go straight to the exit plane, else
+        // take the known ones (at least one step) and test again.
+        const float rem = T - h.rz, duz = P.s_ap * h.uz;
+        // nf = number of j >= 0 with rem - j duz > duz (the per-step rule `rem <= d u_w` decides the exit step); the
+        // rounded quotient can be off by one when rem / duz sits next to an integer, so it is checked against that rule
+        int nf = g.ex ? 0 : max((int)ceilf(__fdiv_rn(rem, duz)) - 1, 0);
+        if (!g.ex) {
+            if (fmaf(-(float)nf, duz, rem) > duz) nf += 1;
+            else if (nf > 0 && fmaf(-(float)(nf - 1), duz, rem) <= duz) nf -= 1;
         }
+        float n_safe = 0.0f;
+        if (nf > 0) {
+            const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
+            if (k >= 2) {
+                const float safe = 0.99f * (float)(k - 1);
+                const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(P.s_ap * h.ux), 1e-12f));
+                const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(P.s_ap * h.uy), 1e-12f));
+                n_safe = floorf(fminf(fminf(nu, nv), 65536.0f));
+            }
+        }
+        const bool whole = n_safe >= (float)nf;            // includes the plain exit step (nf = 0)
+        const int n = whole ? nf : max((int)n_safe, 1);    // full steps taken now
+        if (Tracer::on && n > 0) {     // the same arithmetic, one record per full step
+            const uint32_t g0 = h.g0, g1 = h.g1, g2 = h.g2, g3 = h.g3; const float rz0 = h.rz;
+            for (int j = 1; j <= n; ++j) {
+                const float sj = (float)j * P.s_ap;
+                h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3;
+                pair_axpy(h.g0, h.g1, sj, h.ux, h.lx); pair_axpy(h.g2, h.g3, sj, h.uy, h.ly);
+                h.rz = fmaf(sj, h.uz, rz0);
+                tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step + (uint32_t)(j - 1), REG_AP_OPEN, nullptr, h.E, h.E, P.s_ap, CONT);
+            }
+            h.g0 = g0; h.g1 = g1; h.g2 = g2; h.g3 = g3; h.rz = rz0;
+        }
+        if (whole) {
+            const float rz_nf = fmaf((float)nf * P.s_ap, h.uz, h.rz);                  // depth after the full steps
+            const float d_exit = fmaxf(__fdiv_rn(T - rz_nf, h.uz), 0.0f);
+            const float s_tot = fmaf((float)nf, P.s_ap, d_exit);
+            pair_axpy(h.g0, h.g1, s_tot, h.ux, h.lx); pair_axpy(h.g2, h.g3, s_tot, h.uy, h.ly);
+            h.rz = T;
+            h.step += (uint32_t)(nf + 1);
+            if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + T, h.step - 1u, REG_AP_OPEN, nullptr, h.E, h.E, d_exit, CONT);
+            h.region = REG_TO_CT | (h.region & ~0xff);
+            return BEAM_EXIT;
+        }
+        const float sn = (float)n * P.s_ap;
+        pair_axpy(h.g0, h.g1, sn, h.ux, h.lx); pair_axpy(h.g2, h.g3, sn, h.uy, h.ly);
+        h.rz = fmaf(sn, h.uz, h.rz);
+        h.step += (uint32_t)n;
+        // geometry of the next step
+        g.d = P.s_ap; g.ex = false;
+        const float rem2 = T - h.rz;
+        if (rem2 <= g.d * h.uz) { g.d = fmaxf(__fdiv_rn(rem2, h.uz), 0.0f); g.ex = true; }
     }
-    __syncwarp(conv);
+}
+
+// pending vacuum drift to the aperture entrance + the opening phase from there.  BEAM_EXIT: clean transit (region
+// REG_TO_CT); BEAM_CONT: the history stands in the aperture region and its next step is a brass step (h.rx > 0).
+template <class Tracer>
+__device__ __forceinline__ int ap_enter(const Ctx &c, Hist &h, Tracer &tr)
+{
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    const float w1 = __ldg(&bp->w_ap_in);
+    const float w0 = __ldg(&bp->has_rs) ? __ldg(&bp->w_rs_out) : __ldg(&bp->w_start);
+    if (drift_gap(h, w1 - w0, w1, tr) != CONT) return beam_escape(h, w0, tr);
+    h.region = REG_AP | (h.region & ~0xff);
+    h.rx = 0.0f;
+    SlabGeom g;
+    slab_geometry(c.P, bp, false, h, g);
+    return ap_open_phase(c, bp, h, g, tr);
+}
+
+// One iteration of a history that stands in the aperture region (S3): the opening phase if its medium is not known to be
+// brass, then at most ONE brass step.  `conv` = the lanes of the warp that called together: they re-converge before the
+// expensive slab step, whatever the opening phase did (0 = no forced re-convergence, for one-thread-per-history callers).
+// dep_ap = energy deposited so far in the brass.
+template <class Tracer>
+__device__ __forceinline__ int ap_iter(const Ctx &c, Hist &h, float &dep_ap, LaneCounters &lc, Tracer &tr, unsigned conv)
+{
+    const DevParams &P = c.P;
+    const DevBeam *bp = c.beams + (h.region >> 8);
+    int status = BEAM_CONT;
+    bool do_step = false;
+    SlabGeom g = { __ldg(&bp->w_ap_in), 0.0f, 0.0f, false };
+    if (!(h.uz > 0.0f)) status = beam_escape(h, g.w_in, tr);
+    else {
+        slab_geometry(P, bp, false, h, g);
+        do_step = h.rx > 0.0f;             // while the budget is positive the per-step test of P:L87 can only answer "brass"
+        if (!do_step) { status = ap_open_phase(c, bp, h, g, tr); do_step = status == BEAM_CONT; }
+    }
+    if (conv) __syncwarp(conv);
     if (do_step) {
-        StepOut o;
-        const float Eb = h.E; const uint32_t st = h.step;
-        const float lat = fmaxf(fabsf(h.ux), fabsf(h.uy));        // direction of travel during the step
-        const int cause = step_physics(P, h, m, d, c.K, o);
-        h.rx = fmaf(-o.s, lat, h.rx);                              // brass budget (meaningless, and unused, in the range shifter)
-        if (cause == CONT) {
-            // C4-8: move along the OLD direction, then rotate
-            pair_axpy(h.g0, h.g1, o.s, h.ux, h.lx);
-            pair_axpy(h.g2, h.g3, o.s, h.uy, h.ly);
-            h.rz = fmaf(o.s, h.uz, h.rz);
-            if (P.flags & 1) rotate(h, o.theta, o.uphi);
-        }
-        if (reg == REG_RS) dep_rs += o.dep; else dep_ap += o.dep;
-        lc.n_slab += (cause != STOPPED);
-        const bool out = (cause == CONT) && o.on_d && ex;
-        if (out) h.rz = T;
-        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, st, reg, nullptr, Eb, h.E, o.s, cause, o.dep);
+        const Medium m = { P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
+        bool out;
+        const int cause = slab_step(c, h, m, g, REG_AP, dep_ap, lc, tr, out);
         if (cause != CONT) status = (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
-        else if (out) {
-            reg = (reg == REG_RS && __ldg(&bp->has_ap)) ? REG_TO_AP : REG_TO_CT;
-            if (reg == REG_TO_CT) status = BEAM_EXIT;
-        }
+        else if (out) { h.region = REG_TO_CT | (h.region & ~0xff); status = BEAM_EXIT; }
     }
-    if (esc) {   // u_w <= 0 inside the beam line (C4, last paragraph)
-        if (Tracer::on) tr.put(h, beam_xh(h), beam_yh(h), w_in + h.rz, h.step, REG_VAC, nullptr, h.E, h.E, 0.0f, ESCAPED);
-        status = BEAM_ESCAPED;
-    }
-    h.region = reg | beam_bits;
     return status;
 }
 
-// once-per-history bookkeeping of the beam line (tallies of S:8b), see beam_step()
-template <class Sink>
-__device__ __forceinline__ void book_beam_end(const DevParams &P, const Hist &h, int status, float dep_rs, float dep_ap,
-                                              LaneCounters &lc, const Sink &sink)
+// One iteration of history h anywhere in the beam line (trace kernels): pending drifts, then the stage's own iteration.
+// Returns the BEAM_* status; when the history ended, h.region holds the region it ended in and h.E the energy it had left.
+// Nothing is tallied here: the once-per-history bookkeeping is done by book_beam_end().
+template <class Tracer>
+__device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, float &dep_ap, LaneCounters &lc, Tracer &tr)
 {
-    sink.add_d(TD_DEP_RS, dep_rs);
-    sink.add_d(TD_DEP_BRASS, dep_ap);
-    if (status == BEAM_EXIT) return;                 // its beam-line steps are booked at the CT entry
-    lc.n_dev += h.step;
-    const int reg = h.region & 0xff;
-    if (status == BEAM_NUCLEAR) { sink.add_d(TD_REMOVED, (1.0f - P.gamma_loc) * h.E); sink.add_c(TC_NUCLEAR, 1u); }
-    else if (status == BEAM_STOPPED) sink.add_c(reg == REG_RS ? TC_STOP_RS : TC_STOP_BRASS, 1u);
-    else { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
+    int reg = h.region & 0xff;
+    if (reg == REG_TO_CT) return BEAM_EXIT;              // no device at all
+    if (reg == REG_TO_RS) {
+        if (rs_enter(c, h, tr) != BEAM_CONT) return BEAM_ESCAPED;
+        reg = REG_RS;
+    }
+    if (reg == REG_RS) {
+        const int st = rs_iter(c, h, dep_rs, lc, tr);
+        if (st != BEAM_EXIT) return st;
+        return ((h.region & 0xff) == REG_TO_CT) ? BEAM_EXIT : BEAM_CONT;      // the aperture follows
+    }
+    if (reg == REG_TO_AP) {
+        const int st = ap_enter(c, h, tr);
+        if (st != BEAM_CONT) return st;
+    }
+    return ap_iter(c, h, dep_ap, lc, tr, 0u);
+}
+
+// ---- once-per-history bookkeeping (tallies of S:8b), done in the kernels' event passes by ALL 32 lanes of the warp together:
+// the lanes with something to book contribute to a shuffle reduction and lane 0 adds the sum to the warp's own slot in
+// shared memory (fp64 atomics on shared memory are compare-and-swap loops that serialise the contributing lanes)
+__device__ __forceinline__ void warp_book_d(WarpTally *w, int lane, int k, bool on, float v)
+{
+    if (__ballot_sync(0xffffffffu, on && v != 0.0f) == 0u) return;
+    double s = on ? (double)v : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) w->d[k] += s;
+}
+__device__ __forceinline__ void warp_book_c(WarpTally *w, int lane, int k, bool on)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, on);
+    if (m != 0u && lane == 0) w->c[k] += (unsigned)__popc(m);
+}
+
+// beam line: `due` = this lane holds a finished history whose bookkeeping is due (status != BEAM_CONT); dep = the energy it
+// deposited in this stage's device (tally k_dep = TD_DEP_RS | TD_DEP_BRASS)
+__device__ __forceinline__ void book_beam_end(const DevParams &P, const Hist &h, bool due, int status, float dep, int k_dep,
+                                              LaneCounters &lc, WarpTally *w, int lane)
+{
+    warp_book_d(w, lane, k_dep, due, dep);
+    const bool ended = due && status != BEAM_EXIT;       // the beam-line steps of a survivor are booked at the CT entry
+    if (ended) lc.n_dev += h.step;
+    const bool nuc = ended && status == BEAM_NUCLEAR, stop = ended && status == BEAM_STOPPED, esc = ended && status == BEAM_ESCAPED;
+    warp_book_d(w, lane, TD_REMOVED, nuc, (1.0f - P.gamma_loc) * h.E);
+    warp_book_c(w, lane, TC_NUCLEAR, nuc);
+    warp_book_c(w, lane, k_dep == TD_DEP_RS ? TC_STOP_RS : TC_STOP_BRASS, stop);
+    warp_book_d(w, lane, TD_ESCAPED, esc, h.E);
+    warp_book_c(w, lane, TC_ESCAPED, esc);
 }
 
 // CT entry of a history that left the beam line (region REG_TO_CT): books the beam-line step count and, on a miss,
@@ -485,14 +581,16 @@ __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, fl
     return cause;
 }
 
-// once-per-history bookkeeping of the CT stage
-template <class Sink>
-__device__ __forceinline__ void book_ct_end(const DevParams &P, const Hist &h, int cause, float hdep, const Sink &sink)
+// CT stage: `due` = this lane holds a finished history (cause != CONT); hdep = energy it deposited in the CT
+__device__ __forceinline__ void book_ct_end(const DevParams &P, const Hist &h, bool due, int cause, float hdep, WarpTally *w, int lane)
 {
-    sink.add_d(TD_DEP_CT, hdep);
-    if (cause == NUCLEAR) { sink.add_d(TD_REMOVED, (1.0f - P.gamma_loc) * h.E); sink.add_c(TC_NUCLEAR, 1u); }
-    else if (cause == ESCAPED) { sink.add_d(TD_ESCAPED, h.E); sink.add_c(TC_ESCAPED, 1u); }
-    else sink.add_c(TC_STOP_CT, 1u);
+    warp_book_d(w, lane, TD_DEP_CT, due, hdep);
+    const bool nuc = due && cause == NUCLEAR, esc = due && cause == ESCAPED;
+    warp_book_d(w, lane, TD_REMOVED, nuc, (1.0f - P.gamma_loc) * h.E);
+    warp_book_c(w, lane, TC_NUCLEAR, nuc);
+    warp_book_d(w, lane, TD_ESCAPED, esc, h.E);
+    warp_book_c(w, lane, TC_ESCAPED, esc);
+    warp_book_c(w, lane, TC_STOP_CT, due && !nuc && !esc);
 }
 
 }  // namespace vpk
