@@ -183,9 +183,25 @@ int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *sc, uint64_t batch_
 /* Result of the last vpmc_dose_to_uncertainty: batches run, the estimate after the last one, whether the target stopped it. */
 int vpmc_get_run_info(vpmc_t *h, int32_t *batches_out, float *rel_unc_out, int32_t *reached_target_out);
 
+/* Test-only: the device tables S0 builds from an opening bitmap (D:5.2).  dims_out[4] = {words per row, rows, tiles in u,
+ * tiles in v}; bits_out_host: rows x words packed bitmap (bit ix & 31 of word ix >> 5); dist_out_host: 2 maps of tiles_v x
+ * tiles_u bytes -- Chebyshev distance in tiles (capped at 255) to the nearest tile that is not fully open, with everything
+ * outside the bitmap brass, then to the nearest tile holding any open pixel.  Any output pointer may be NULL. */
+int vpmc_get_aperture_tables(vpmc_t *h, int beam, uint32_t *bits_out_host, uint8_t *dist_out_host, int32_t *dims_out);
+
 /* Restrict the next dose / trace calls to history ids [hid_begin, hid_end) of the N-history run (prefix
  * parity, S:8d).  hid_end = 0 -> no restriction. */
 int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);
+
+/* Multi-GPU sharding (S:8e): this handle computes shard `index` of `count` of the following dose / influence calls.
+ * Dose: of every (spot, batch) id range [a, b) of the N-history run only the ids [a + (b - a) index / count,
+ * a + (b - a)(index + 1) / count) are transported, with the scale W / N of the full run, so the SUM of the dose grids of
+ * the `count` shards is the dose of the full run (same history ids, same random streams; equal up to the order of
+ * floating-point additions) and every shard holds the same mix of spots.  Influence: only the rows (spots) g with
+ * n_spots index / count <= g < n_spots (index + 1) / count are computed; the other rows of the returned CSR are empty, so
+ * the full matrix is the concatenation of the shards' entries, row_ptr offset by the exclusive sum of the shards' nnz.
+ * No exchange happens inside the library.  (0, 1) = everything (default). */
+int vpmc_set_shard(vpmc_t *h, int32_t index, int32_t count);
 
 /* Influence matrices: for each of n_sc scenarios and each spot j (history ids
  * j*hist_per_spot + i), the dose column per unit weight, entries >= rel_threshold * column max (and > 0) kept,
@@ -195,6 +211,14 @@ int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);
 int vpmc_influence(vpmc_t *h, const vpmc_scenario *sc, int32_t n_sc, uint32_t hist_per_spot,
                    float rel_threshold, uint64_t seed, vpmc_csr *out, vpmc_alloc_fn alloc, void *user,
                    void *cuda_stream);
+
+/* Counts of the last vpmc_influence call (bench.py's writer roofline, S:8d): elements of the per-column boxes that were
+ * zeroed and scanned (all groups, scenarios and replays), deposits that went to the overflow list and how many of its
+ * entries were kept, columns replayed, groups run. */
+typedef struct {
+    uint64_t box_elements, ovf_deposits, ovf_kept, columns_replayed, groups, nnz;
+} vpmc_influence_stats;
+int vpmc_get_influence_stats(vpmc_t *h, vpmc_influence_stats *out);
 
 /* The CSR writer alone (S:8a-S8, D:R10): one row from a dense fp32 column [device] of n voxels.  With
  * col_out/val_out NULL only counts.  *nnz_out [host].  Synchronous. */
@@ -276,11 +300,18 @@ int vpmc_set_knob(vpmc_t *h, int knob, double value);
 
 /* Per-kernel-class device timing (bench.py's roofline): when on, every launch is bracketed by CUDA events on its
  * stream.  vpmc_get_timing synchronises, returns accumulated milliseconds and launch counts per class
- * (0 beam_kernel S1-S3, 1 voxel_kernel S4-S7 incl. the influence pilot, 2 dose conversion / uncertainty passes S6,
- * 3 CSR writer passes S8) and resets. */
-#define VPMC_N_KERNEL_CLASSES 4
+ * (0 beam_kernel: the persistent range-shifter / brass kernels S2-S3, 1 voxel_kernel S4-S7 incl. the influence pilot,
+ * 2 dose conversion / uncertainty passes S6, 3 CSR writer passes S8, 4 the one-thread-per-item stage kernels: source +
+ * opening phase S1/S3, aperture entry, CT entry) and resets. */
+#define VPMC_N_KERNEL_CLASSES 5
 int vpmc_set_timing(vpmc_t *h, int on);
 int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out);
+
+/* Measurement (S:8d (iii)): ceiling of global fp32 RED throughput on this device -- about n_ops atomicAdd(float) to
+ * pseudo-random elements of a buffer of buffer_bytes (a power of two; 4 MB stays L2-resident), issued by one resident wave of
+ * threads.  Returns the kernel's duration (CUDA events) and the exact number of REDs issued; bench.py reports the dose
+ * scorer's RED rate against it.  Synchronous, default stream. */
+int vpmc_bench_red(vpmc_t *h, uint64_t buffer_bytes, uint64_t n_ops, double *ms_out, uint64_t *n_ops_out);
 
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int vpmc_get_launch_count(vpmc_t *h, uint64_t *out);

@@ -22,7 +22,7 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
-           "vpmc_get_run_info"]
+           "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
@@ -70,6 +70,13 @@ class Tallies(C.Structure):
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class InfluenceStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("box_elements", "ovf_deposits", "ovf_kept", "columns_replayed", "groups", "nnz")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
 
 
 STEP_DTYPE = np.dtype([("hid", "<u8"), ("step", "<i4"), ("region", "<i4"), ("cause", "<i4"), ("ivox", "<i4", 3),
@@ -133,6 +140,10 @@ def lib():
         L.vpmc_dose_to_uncertainty.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_int32, C.c_int32, C.c_float,
                                                C.c_uint64, C.c_void_p, C.c_void_p]
         L.vpmc_get_run_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+        L.vpmc_bench_red.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+        L.vpmc_get_aperture_tables.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]
+        L.vpmc_set_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.vpmc_get_influence_stats.argtypes = [C.c_void_p, C.POINTER(InfluenceStats)]
         L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -231,6 +242,10 @@ class Engine:
     def set_history_window(self, begin: int, end: int):
         self._check(lib().vpmc_set_history_window(self._h, int(begin), int(end)))
 
+    def set_shard(self, index: int, count: int):
+        """This handle computes shard `index` of `count` (vpmc_set_shard)."""
+        self._check(lib().vpmc_set_shard(self._h, int(index), int(count)))
+
     # -- hot path
     def dose(self, n_histories: int, seed: int, out=None, sc: Scenario | None = None, stream=None):
         """Dose [Gy] as a torch.float32 CUDA tensor of nvox elements (v = ix + nx*(iy + ny*iz))."""
@@ -290,11 +305,12 @@ class Engine:
         self._check(lib().vpmc_set_timing(self._h, 1 if on else 0))
 
     def timing(self):
-        """{class: (milliseconds, launches)} accumulated since the last call; classes beamline / voxel / scoring / writer."""
-        ms = (C.c_double * 4)()
-        n = (C.c_uint64 * 4)()
+        """{class: (milliseconds, launches)} accumulated since the last call; classes beamline (persistent beam kernels) /
+        voxel / scoring / writer / stage (one-thread-per-item source, aperture-entry and CT-entry kernels)."""
+        ms = (C.c_double * 5)()
+        n = (C.c_uint64 * 5)()
         self._check(lib().vpmc_get_timing(self._h, ms, n))
-        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("beamline", "voxel", "scoring", "writer"))}
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("beamline", "voxel", "scoring", "writer", "stage"))}
 
     def trace(self, hids, n_or_hps: int, seed: int, sc: Scenario | None = None, mode: int = 0, max_steps: int = 1024):
         hids = np.ascontiguousarray(np.asarray(hids, dtype=np.uint64))
@@ -330,6 +346,11 @@ class Engine:
             res.append((rp, col, val))
         return res
 
+    def influence_stats(self) -> dict:
+        st = InfluenceStats()
+        self._check(lib().vpmc_get_influence_stats(self._h, C.byref(st)))
+        return st.as_dict()
+
     def step_from_state(self, states: np.ndarray, seed: int, sc: Scenario | None = None) -> np.ndarray:
         """Test-only: one step from each pre-step state (STATE_DTYPE array) -> STATE_OUT_DTYPE array."""
         states = np.ascontiguousarray(states, dtype=STATE_DTYPE)
@@ -344,6 +365,21 @@ class Engine:
         self._check(lib().vpmc_digests(self._h, C.byref(sc) if sc is not None else None, int(n_histories), int(seed),
                                        int(hid_begin), int(n), out.ctypes.data))
         return out
+
+    def aperture_tables(self, beam: int = 0):
+        """Test-only: (packed bitmap uint32 [rows, words], distance maps uint8 [2, tiles_v, tiles_u]) of a beam's aperture."""
+        dims = (C.c_int32 * 4)()
+        self._check(lib().vpmc_get_aperture_tables(self._h, int(beam), None, None, dims))
+        bits = np.zeros((dims[1], dims[0]), dtype=np.uint32)
+        dist = np.zeros((2, dims[3], dims[2]), dtype=np.uint8)
+        self._check(lib().vpmc_get_aperture_tables(self._h, int(beam), bits.ctypes.data, dist.ctypes.data, dims))
+        return bits, dist
+
+    def bench_red(self, buffer_bytes: int = 4 << 20, n_ops: int = 1 << 30):
+        """fp32 REDs per second into an L2-resident buffer of buffer_bytes (vpmc_bench_red): (ops/s, ops issued)."""
+        ms, n = C.c_double(), C.c_uint64()
+        self._check(lib().vpmc_bench_red(self._h, int(buffer_bytes), int(n_ops), C.byref(ms), C.byref(n)))
+        return n.value / (ms.value * 1e-3), int(n.value)
 
     def set_knob(self, knob: int, value: float):
         self._check(lib().vpmc_set_knob(self._h, int(knob), float(value)))

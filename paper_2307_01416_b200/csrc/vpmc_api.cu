@@ -12,6 +12,7 @@
 #include <cub/cub.cuh>
 
 #include "vpmc_host.h"
+#include "vpmc_setup.cuh"
 
 using namespace vpk;
 
@@ -68,7 +69,7 @@ void pool_give(void *p, size_t bytes)
     {
         const int dev = current_device();
         std::lock_guard<std::mutex> lk(g_pool_mu);
-        if (bytes >= 4096 && g_pool_bytes + bytes <= kPoolLimit && g_pool.size() < 256) { g_pool.push_back({ p, bytes, dev }); g_pool_bytes += bytes; return; }
+        if (g_pool_bytes + bytes <= kPoolLimit && g_pool.size() < 2048) { g_pool.push_back({ p, bytes, dev }); g_pool_bytes += bytes; return; }
     }
     cudaFree(p);
 }
@@ -89,6 +90,40 @@ static int ensure(vpmc_t *h, DevBuf &b, size_t bytes)
     }
     b.bytes = want;
     return VPMC_OK;
+}
+
+// fixed-size device members of a handle: taken from the buffer cache, remembered in h->owned, returned in vpmc_destroy
+static int dev_alloc(vpmc_t *h, void **out, size_t bytes)
+{
+    DevBuf b;
+    int rc = ensure(h, b, bytes); if (rc) { *out = nullptr; return rc; }
+    h->owned.push_back({ b.p, b.bytes });
+    *out = b.p;
+    return VPMC_OK;
+}
+
+// give one member back while the handle lives on (inputs replaced by a later set_* call): whatever may still read it must
+// have finished first
+static void dev_release(vpmc_t *h, void *p)
+{
+    if (!p) return;
+    for (size_t i = 0; i < h->owned.size(); ++i)
+        if (h->owned[i].p == p) {
+            if (h->launched) cudaStreamSynchronize(h->last_stream);
+            if (h->setup_stream) cudaStreamSynchronize(h->setup_stream);
+            pool_give(p, h->owned[i].bytes);
+            h->owned.erase(h->owned.begin() + i);
+            return;
+        }
+}
+
+// the stream of a compute call waits for the set-up work enqueued so far
+static void join_setup(vpmc_t *h, cudaStream_t st)
+{
+    if (!h->setup_pending) return;
+    cudaEventRecord(h->setup_ev, h->setup_stream);
+    cudaStreamWaitEvent(st, h->setup_ev, 0);
+    h->setup_pending = false;
 }
 
 extern "C" const char *vpmc_version(void) { return "vpmc-b200 0.2 (sm_100a)"; }
@@ -135,27 +170,30 @@ static double pl_eval(const vpmc_calib *c, const float *y, double hu)
     return (double)y[k] + t * ((double)y[k + 1] - (double)y[k]);
 }
 
-static void free_beam(BeamHost &b)
+static void free_beam(vpmc_t *h, BeamHost &b)
 {
-    if (b.d_bits) cudaFree(b.d_bits);
-    if (b.d_dist) cudaFree(b.d_dist);
-    b.d_bits = nullptr; b.d_dist = nullptr;
+    dev_release(h, b.d_bits); dev_release(h, b.d_dist); dev_release(h, b.d_ap_tmp);
+    b.d_bits = nullptr; b.d_dist = nullptr; b.d_ap_tmp = nullptr;
 }
 
 extern "C" int vpmc_destroy(vpmc_t *h)
 {
     if (!h) return VPMC_OK;
-    cudaDeviceSynchronize();
+    // only this handle's own streams are drained (no device-wide synchronisation)
+    if (h->launched) cudaStreamSynchronize(h->last_stream);
+    if (h->setup_stream) cudaStreamSynchronize(h->setup_stream);
+    if (h->seq_stream) cudaStreamSynchronize(h->seq_stream);
+    for (auto &t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     if (h->seq_exec) cudaGraphExecDestroy(h->seq_exec);
     if (h->seq_graph) cudaGraphDestroy(h->seq_graph);
     if (h->seq_ev_in) cudaEventDestroy(h->seq_ev_in);
     if (h->seq_ev_out) cudaEventDestroy(h->seq_ev_out);
     if (h->seq_stream) cudaStreamDestroy(h->seq_stream);
-    if (h->d_seq) cudaFree(h->d_seq);
-    for (auto &b : h->beams) free_beam(b);
-    void *ptrs[] = { h->d_hu, h->d_lut, h->d_spots, h->d_spot_R0, h->d_spot_beam, h->d_beams, h->d_qctr, h->d_s1, h->d_s2, h->d_fb,
-                     h->d_tal, h->d_tal_scratch, h->d_max_bits, h->d_unc };
-    for (void *p : ptrs) if (p) cudaFree(p);
+    if (h->setup_ev) cudaEventDestroy(h->setup_ev);
+    if (h->copy_ev) cudaEventDestroy(h->copy_ev);
+    if (h->setup_stream) cudaStreamDestroy(h->setup_stream);
+    for (auto &o : h->owned) pool_give(o.p, o.bytes);
+    h->owned.clear();
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
@@ -212,17 +250,24 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     h->lut_bytes = lut.size() * sizeof(float4);
     h->smem_lut = h->lut_bytes <= kMaxSmemLut;
 #define CUC(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { g_create_err = std::string(#expr) + ": " + cudaGetErrorString(_e); vpmc_destroy(h); return VPMC_ERR_CUDA; } } while (0)
-    CUC(cudaMalloc(&h->d_lut, h->lut_bytes));
-    CUC(cudaMemcpy(h->d_lut, lut.data(), h->lut_bytes, cudaMemcpyHostToDevice));
-    CUC(cudaMalloc(&h->d_hu, nvox * sizeof(short)));
-    CUC(cudaMemcpy(h->d_hu, ct->hu, nvox * sizeof(short), ct->hu_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice));
-    CUC(cudaMalloc(&h->d_tal, sizeof(DevTallies)));
-    CUC(cudaMemset(h->d_tal, 0, sizeof(DevTallies)));
-    CUC(cudaMalloc(&h->d_tal_scratch, sizeof(DevTallies)));
-    CUC(cudaMalloc(&h->d_max_bits, sizeof(unsigned int)));
-    CUC(cudaMalloc(&h->d_unc, 2 * sizeof(double)));
-    CUC(cudaMalloc(&h->d_qctr, 8 * sizeof(unsigned int)));
-    CUC(cudaMalloc(&h->d_fb, 1024 * sizeof(float)));
+#define CUA(ptr, bytes) do { if (dev_alloc(h, (void **)&(ptr), (bytes)) != VPMC_OK) { g_create_err = h->err; vpmc_destroy(h); return VPMC_ERR_ALLOC; } } while (0)
+    CUC(cudaStreamCreateWithFlags(&h->setup_stream, cudaStreamNonBlocking));
+    CUC(cudaEventCreateWithFlags(&h->setup_ev, cudaEventDisableTiming));
+    CUC(cudaEventCreateWithFlags(&h->copy_ev, cudaEventDisableTiming));
+    cudaStream_t ss = h->setup_stream;
+    CUA(h->d_lut, h->lut_bytes);
+    CUA(h->d_hu, nvox * sizeof(short));
+    CUA(h->d_tal, sizeof(DevTallies));
+    CUA(h->d_tal_scratch, sizeof(DevTallies));
+    CUA(h->d_max_bits, sizeof(unsigned int));
+    CUA(h->d_unc, 2 * sizeof(double));
+    CUA(h->d_qctr, 8 * sizeof(unsigned int));
+    CUA(h->d_fb, 1024 * sizeof(float));
+    CUC(cudaMemcpyAsync(h->d_lut, lut.data(), h->lut_bytes, cudaMemcpyHostToDevice, ss));
+    CUC(cudaMemcpyAsync(h->d_hu, ct->hu, nvox * sizeof(short), ct->hu_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ss));
+    CUC(cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), ss));
+    CUC(cudaEventRecord(h->copy_ev, ss));
+    h->setup_pending = true;
     // persistent kernels: one wave of resident CTAs each
     {
         h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
@@ -258,7 +303,9 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
             cache.push_back(g);
         }
     }
+    CUC(cudaEventSynchronize(h->copy_ev));     // the caller's arrays are copied during the call (vpmc.h)
 #undef CUC
+#undef CUA
     *out = h;
     return VPMC_OK;
 }
@@ -319,63 +366,47 @@ extern "C" int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int ma
     int rc = check_beam(h, beam); if (rc) return rc;
     BeamHost &b = h->beams[beam];
     if (!(thickness_mm >= 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "negative thickness");
-    if (thickness_mm == 0) { free_beam(b); b.has_ap = false; h->spots_dirty = true; return VPMC_OK; }
+    if (thickness_mm == 0) { free_beam(h, b); b.has_ap = false; h->spots_dirty = true; return VPMC_OK; }
     if (material != VPMC_BRASS) FAIL(h, VPMC_ERR_INVALID_ARG, "only VPMC_BRASS is supported");
     if (!opening || nx < 1 || ny < 1 || nx > 16384 || ny > 16384 || !(du > 0) || !(dv > 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "bad opening bitmap");
+    // S0 on the device (vpmc_setup.cuh): bitmap packing and the two safe-distance maps.  Tile = 2^kApTileShift
+    // pixels squared; map 0 = Chebyshev distance in tiles to the nearest tile that is not fully open (everything outside the
+    // bitmap is brass), map 1 = to the nearest tile that holds any open pixel; both exact, capped at 255.
     const int rw = (nx + 31) / 32;
-    std::vector<uint32_t> bits((size_t)rw * ny, 0u);          // S0: bitmap packing
-    for (int iy = 0; iy < ny; ++iy)
-        for (int ix = 0; ix < nx; ++ix)
-            if (opening[(size_t)iy * nx + ix]) bits[(size_t)iy * rw + (ix >> 5)] |= 1u << (ix & 31);
-    // S0: safe-distance maps.  Tile = 2^kApTileShift pixels squared; two maps: Chebyshev distance in tiles to
-    // the nearest tile that is not fully open (everything outside the bitmap is brass), and to the nearest tile that holds
-    // any open pixel.  Exact two-pass chamfer for the L-infinity metric on arrays padded by one tile (no bounds tests).
     const int ts = 1 << kApTileShift, ntx = (nx + ts - 1) / ts, nty = (ny + ts - 1) / ts;
-    const int pw = ntx + 2;
-    std::vector<unsigned short> dbr((size_t)pw * (nty + 2), 0), dop((size_t)pw * (nty + 2), 255);
-    for (int ty = 0; ty < nty; ++ty)
-        for (int tx = 0; tx < ntx; ++tx) {
-            bool all = (tx + 1) * ts <= nx && (ty + 1) * ts <= ny, any = false;
-            for (int iy = ty * ts; iy < std::min((ty + 1) * ts, ny); ++iy)
-                for (int ix = tx * ts; ix < std::min((tx + 1) * ts, nx); ++ix) {
-                    const bool o = opening[(size_t)iy * nx + ix] != 0;
-                    all = all && o; any = any || o;
-                }
-            dbr[(size_t)(ty + 1) * pw + tx + 1] = all ? 255 : 0;
-            dop[(size_t)(ty + 1) * pw + tx + 1] = any ? 0 : 255;
-        }
-    for (std::vector<unsigned short> *dm : { &dbr, &dop }) {
-        unsigned short *d = dm->data();
-        for (int ty = 1; ty <= nty; ++ty) {
-            unsigned short *r = d + (size_t)ty * pw, *u = r - pw;
-            for (int tx = 1; tx <= ntx; ++tx) {
-                const unsigned short m = std::min(std::min(u[tx - 1], u[tx]), std::min(u[tx + 1], r[tx - 1]));
-                if (m + 1 < r[tx]) r[tx] = (unsigned short)(m + 1);
-            }
-        }
-        for (int ty = nty; ty >= 1; --ty) {
-            unsigned short *r = d + (size_t)ty * pw, *l = r + pw;
-            for (int tx = ntx; tx >= 1; --tx) {
-                const unsigned short m = std::min(std::min(l[tx + 1], l[tx]), std::min(l[tx - 1], r[tx + 1]));
-                if (m + 1 < r[tx]) r[tx] = (unsigned short)(m + 1);
-            }
-        }
-    }
-    std::vector<unsigned char> dist8((size_t)2 * ntx * nty);
-    for (int ty = 0; ty < nty; ++ty)
-        for (int tx = 0; tx < ntx; ++tx) {
-            dist8[(size_t)ty * ntx + tx] = (unsigned char)std::min<int>(dbr[(size_t)(ty + 1) * pw + tx + 1], 255);
-            dist8[(size_t)ntx * nty + (size_t)ty * ntx + tx] = (unsigned char)std::min<int>(dop[(size_t)(ty + 1) * pw + tx + 1], 255);
-        }
-    free_beam(b);
-    CU(h, cudaMalloc(&b.d_bits, bits.size() * sizeof(uint32_t)));
-    CU(h, cudaMemcpy(b.d_bits, bits.data(), bits.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
-    CU(h, cudaMalloc(&b.d_dist, dist8.size()));
-    CU(h, cudaMemcpy(b.d_dist, dist8.data(), dist8.size(), cudaMemcpyHostToDevice));
+    const size_t npix = (size_t)nx * ny, ntile = (size_t)ntx * nty;
+    free_beam(h, b);
+    int rc2;
+    if ((rc2 = dev_alloc(h, (void **)&b.d_bits, (size_t)rw * ny * sizeof(uint32_t))) || (rc2 = dev_alloc(h, (void **)&b.d_dist, 2 * ntile)) ||
+        (rc2 = dev_alloc(h, (void **)&b.d_ap_tmp, npix + 3 * ntile))) return rc2;
+    unsigned char *d_open = b.d_ap_tmp, *d_flags = d_open + npix, *d_cbr = d_flags + ntile, *d_cop = d_cbr + ntile;
+    cudaStream_t ss = h->setup_stream;
+    CU(h, cudaMemcpyAsync(d_open, opening, npix, cudaMemcpyHostToDevice, ss));
+    CU(h, cudaEventRecord(h->copy_ev, ss));
+    ap_pack_kernel<<<(unsigned)(((size_t)rw * 32 * ny + 255) / 256), 256, 0, ss>>>(d_open, nx, ny, rw, b.d_bits);
+    ap_tile_flags_kernel<<<(unsigned)((ntile + 255) / 256), 256, 0, ss>>>(d_open, nx, ny, kApTileShift, ntx, nty, d_flags);
+    ap_dist_columns_kernel<<<(ntx + 63) / 64, 64, 0, ss>>>(d_flags, ntx, nty, d_cbr, d_cop);
+    ap_dist_rows_kernel<<<(unsigned)((2 * ntile + 255) / 256), 256, 0, ss>>>(d_cbr, d_cop, ntx, nty, b.d_dist);
+    CU(h, cudaGetLastError());
+    h->launches += 4;
+    h->setup_pending = true;
     b.ap_ntx = ntx; b.ap_nty = nty;
     b.has_ap = true; b.ap_T = thickness_mm; b.ap_face = downstream_face_mm > 0 ? downstream_face_mm : 150.0f;
     b.ap_nx = nx; b.ap_ny = ny; b.ap_row_words = rw; b.ap_u0 = u0; b.ap_v0 = v0; b.ap_du = du; b.ap_dv = dv;
     h->spots_dirty = true;
+    CU(h, cudaEventSynchronize(h->copy_ev));       // the caller's bitmap is copied during the call
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_get_aperture_tables(vpmc_t *h, int beam, uint32_t *bits_out_host, uint8_t *dist_out_host, int32_t *dims_out)
+{
+    int rc = check_beam(h, beam); if (rc) return rc;
+    const BeamHost &b = h->beams[beam];
+    if (!b.has_ap) FAIL(h, VPMC_ERR_STATE, "beam %d has no aperture", beam);
+    if (dims_out) { dims_out[0] = b.ap_row_words; dims_out[1] = b.ap_ny; dims_out[2] = b.ap_ntx; dims_out[3] = b.ap_nty; }
+    CU(h, cudaStreamSynchronize(h->setup_stream));
+    if (bits_out_host) CU(h, cudaMemcpy(bits_out_host, b.d_bits, (size_t)b.ap_row_words * b.ap_ny * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    if (dist_out_host) CU(h, cudaMemcpy(dist_out_host, b.d_dist, (size_t)2 * b.ap_ntx * b.ap_nty, cudaMemcpyDeviceToHost));
     return VPMC_OK;
 }
 
@@ -383,6 +414,14 @@ extern "C" int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t h
 {
     if (!h) return VPMC_ERR_INVALID_ARG;
     h->win_lo = hid_begin; h->win_hi = hid_end;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_set_shard(vpmc_t *h, int32_t index, int32_t count)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (count < 1 || index < 0 || index >= count) FAIL(h, VPMC_ERR_INVALID_ARG, "shard %d of %d", index, count);
+    h->shard_index = index; h->shard_count = count;
     return VPMC_OK;
 }
 
@@ -420,6 +459,39 @@ extern "C" int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out
         cudaEventDestroy(t.a); cudaEventDestroy(t.b);
     }
     h->timed.clear();
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_bench_red(vpmc_t *h, uint64_t buffer_bytes, uint64_t n_ops, double *ms_out, uint64_t *n_ops_out)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!ms_out || !n_ops_out || buffer_bytes < 1024 || buffer_bytes > ((uint64_t)1 << 32) || (buffer_bytes & (buffer_bytes - 1)) || n_ops < 1)
+        FAIL(h, VPMC_ERR_INVALID_ARG, "bench_red: buffer_bytes must be a power of two in [2^10, 2^32], n_ops >= 1");
+    DevBuf buf;
+    int rc = ensure(h, buf, (size_t)buffer_bytes); if (rc) return rc;
+    const int grid = h->n_sm * 8, block = 256;
+    const unsigned long long threads = (unsigned long long)grid * block;
+    const unsigned int per = (unsigned int)std::min<unsigned long long>(std::max<unsigned long long>(n_ops / threads, 1ull), 1ull << 24);
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaError_t e = cudaMemset(buf.p, 0, (size_t)buffer_bytes);
+    if (e == cudaSuccess) e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    if (e == cudaSuccess) {
+        red_ceiling_kernel<<<grid, block>>>(buf.as<float>(), (unsigned int)(buffer_bytes / 4 - 1), std::min(per, 64u));   // warm-up: the buffer into L2
+        cudaEventRecord(a);
+        red_ceiling_kernel<<<grid, block>>>(buf.as<float>(), (unsigned int)(buffer_bytes / 4 - 1), per);
+        cudaEventRecord(b);
+        h->launches += 2;
+        e = cudaEventSynchronize(b);
+    }
+    float ms = 0.0f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaDeviceSynchronize();
+    pool_give(buf.p, buf.bytes);
+    if (e != cudaSuccess) FAIL(h, VPMC_ERR_CUDA, "bench_red: %s", cudaGetErrorString(e));
+    *ms_out = (double)ms; *n_ops_out = (uint64_t)per * threads;
     return VPMC_OK;
 }
 

@@ -19,6 +19,7 @@ struct BeamHost {
     float ap_u0 = 0, ap_v0 = 0, ap_du = 1, ap_dv = 1;
     uint32_t *d_bits = nullptr;       // packed opening bitmap on the device
     unsigned char *d_dist = nullptr;  // safe-distance maps of the opening, one byte per tile of 2^kApTileShift pixels: to brass, then to the opening
+    unsigned char *d_ap_tmp = nullptr;    // set-up scratch: the caller's uint8 bitmap, tile flags, column distances
     int ap_ntx = 0, ap_nty = 0;
 };
 
@@ -35,6 +36,16 @@ struct vpmc {
     vpk::DevGrid G;
     long long nvox = 0;
     int device = 0, n_sm = 0;
+
+    // Device memory of the fixed-size members below comes from the process-wide buffer cache (vpmc_api.cu) and goes back to
+    // it in vpmc_destroy.  Set-up work (uploads, S0 kernels) is enqueued on setup_stream; the next compute call makes its
+    // stream wait for it.
+    struct Owned { void *p; size_t bytes; };
+    std::vector<Owned> owned;
+    cudaStream_t setup_stream = nullptr;
+    cudaEvent_t setup_ev = nullptr, copy_ev = nullptr;
+    bool setup_pending = false;
+    bool launched = false;            // some compute call has enqueued work on last_stream
 
     // device-resident inputs
     short *d_hu = nullptr;
@@ -78,6 +89,7 @@ struct vpmc {
     DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_skip, inf_tilecnt, inf_colmax,
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
         ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
+    vpmc_influence_stats inf_stats = {};
     size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
 
     // knobs (vpmc_set_knob)
@@ -94,6 +106,7 @@ struct vpmc {
     size_t lut_bytes = 0, tally_smem = 0;
 
     unsigned long long win_lo = 0, win_hi = 0;
+    int shard_index = 0, shard_count = 1;     // vpmc_set_shard (S:8e)
     cudaStream_t last_stream = nullptr;
     unsigned long long launches = 0;
     bool timing = false;

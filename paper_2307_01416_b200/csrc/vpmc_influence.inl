@@ -106,6 +106,13 @@ extern "C" int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, f
     return VPMC_OK;
 }
 
+extern "C" int vpmc_get_influence_stats(vpmc_t *h, vpmc_influence_stats *out)
+{
+    if (!h || !out) return VPMC_ERR_INVALID_ARG;
+    *out = h->inf_stats;
+    return VPMC_OK;
+}
+
 extern "C" int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes)
 {
     if (!h) return VPMC_ERR_INVALID_ARG;
@@ -137,6 +144,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
     h->unc_valid = false;
     for (int s = 0; s < n_sc; ++s) { out[s].row_ptr = nullptr; out[s].col = nullptr; out[s].val = nullptr; out[s].nnz = 0; out[s].n_rows = 0; }
     CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
+    h->inf_stats = vpmc_influence_stats{};
     size_t limit = h->workspace_limit;
     if (limit == 0) {
         size_t fr = 0, tot = 0;
@@ -155,14 +163,16 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         int rc = prepare_beams(h, sc, st); if (rc) return rc;
         const int ns = h->n_spots;
         const Ctx ctx = make_ctx(h, sc, seed);
+        // S:8e: this handle's rows (vpmc_set_shard); the other rows stay empty
+        const int g_lo = (int)((long long)ns * h->shard_index / h->shard_count), g_hi = (int)((long long)ns * (h->shard_index + 1) / h->shard_count);
         // ---- 1. pilot bounding boxes
         std::vector<int> bb((size_t)ns * 6);
         for (int g = 0; g < ns; ++g) { bb[6 * g] = bb[6 * g + 1] = bb[6 * g + 2] = 0x7fffffff; bb[6 * g + 3] = bb[6 * g + 4] = bb[6 * g + 5] = -1; }
         rc = upload(h, h->inf_bbox, bb, st); if (rc) return rc;
         {
             WorkMap wm{};
-            wm.mode = 1; wm.hps = hist_per_spot; wm.n_sub = n_pilot; wm.cols = nullptr; wm.g0 = 0;
-            wm.n_items = (unsigned long long)ns * n_pilot;
+            wm.mode = 1; wm.hps = hist_per_spot; wm.n_sub = n_pilot; wm.cols = nullptr; wm.g0 = g_lo;
+            wm.n_items = (unsigned long long)(g_hi - g_lo) * n_pilot;
             ScoreArgs sa{};
             sa.cb.bbox = h->inf_bbox.as<int>();
             CU(h, cudaMemsetAsync(h->d_tal_scratch, 0, sizeof(DevTallies), st));
@@ -172,16 +182,17 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         CU(h, cudaStreamSynchronize(st));
         // ---- 2. boxes
         std::vector<HostBox> box(ns);
-        for (int g = 0; g < ns; ++g) {
-            if (bb[6 * g + 3] < 0) { for (int a = 0; a < 3; ++a) { box[g].lo[a] = 0; box[g].dim[a] = 1; } }   // pilot deposited nothing
-            else box[g] = grown_box(&bb[6 * g], h->G, h->box_grow, h->box_pad);
+        for (int g = g_lo; g < g_hi; ++g) {           // the pilot's columns are local: column c = spot g_lo + c
+            const int *pb = &bb[6 * (size_t)(g - g_lo)];
+            if (pb[3] < 0) { for (int a = 0; a < 3; ++a) { box[g].lo[a] = 0; box[g].dim[a] = 1; } }   // pilot deposited nothing
+            else box[g] = grown_box(pb, h->G, h->box_grow, h->box_pad);
         }
         // ---- 3./4. groups, with replay of the columns that outgrew their box
         std::vector<long long> row_nnz(ns, 0), row_src(ns, 0), row_ovf_off(ns, 0);
         std::vector<int> row_ovf_n(ns, 0);
         long long staged = 0, ostaged = 0;
-        std::vector<int> todo(ns);
-        std::iota(todo.begin(), todo.end(), 0);
+        std::vector<int> todo(g_hi - g_lo);
+        std::iota(todo.begin(), todo.end(), g_lo);
         bool replay = false;
         for (int round = 0; !todo.empty(); ++round) {
             if (round > 4) FAIL(h, VPMC_ERR_STATE, "influence: columns still outgrow their boxes after %d replays", round - 1);
@@ -203,6 +214,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     ++i0;
                 }
                 const int nc = (int)cols.size();
+                h->inf_stats.box_elements += (uint64_t)elems; h->inf_stats.groups += 1;
                 rc = ensure(h, h->inf_scratch, (size_t)elems * sizeof(float)); if (rc) return rc;
                 std::vector<int> obb((size_t)nc * 6);
                 for (int c = 0; c < nc; ++c) { obb[6 * c] = obb[6 * c + 1] = obb[6 * c + 2] = 0x7fffffff; obb[6 * c + 3] = obb[6 * c + 4] = obb[6 * c + 5] = -1; }
@@ -233,6 +245,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 CU(h, cudaMemcpyAsync(&n_ovf, h->ovf_ctr.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
                 CU(h, cudaStreamSynchronize(st));
                 n_ovf = std::min(n_ovf, ovf_cap);
+                h->inf_stats.ovf_deposits += n_ovf;
                 std::vector<int> skip(nc, 0);
                 for (int c = 0; c < nc; ++c)
                     if (obb[6 * c + 3] >= 0) {
@@ -242,6 +255,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                         for (int a = 0; a < 3; ++a) { u[a] = std::min(b.lo[a], obb[6 * c + a]); u[3 + a] = std::max(b.lo[a] + b.dim[a] - 1, obb[6 * c + 3 + a]); }
                         for (int a = 0; a < 3; ++a) { b.lo[a] = u[a]; b.dim[a] = u[3 + a] - u[a] + 1; }
                         next.push_back(cols[c]);
+                        h->inf_stats.columns_replayed += 1;
                     }
                 rc = upload(h, h->inf_skip, skip, st); if (rc) return rc;
                 CsrCols cc{};
@@ -299,6 +313,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     CU(h, cudaMemcpyAsync(h->ostage_val.as<float>() + ostaged, h->ovf_val2.p, (size_t)oadd * sizeof(float), cudaMemcpyDeviceToDevice, st));
                     h->launches += 1;
                     ostaged += oadd;
+                    h->inf_stats.ovf_kept += (uint64_t)oadd;
                 }
                 if (h->verbose) fprintf(stderr, "[vpmc]   group of %d columns: %u outside deposits, %lld kept entries of them, %lld box entries\n", nc, n_ovf, oadd, add);
                 if (add > 0) {
@@ -324,6 +339,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         const long long nnz = row_ptr[ns];
         vpmc_csr &o = out[s];
         o.n_rows = ns; o.nnz = nnz;
+        h->inf_stats.nnz += (uint64_t)nnz;
         o.row_ptr = (int64_t *)alloc((size_t)(ns + 1) * sizeof(int64_t), user);
         o.col = (int32_t *)alloc((size_t)std::max<long long>(nnz, 1) * sizeof(int32_t), user);
         o.val = (float *)alloc((size_t)std::max<long long>(nnz, 1) * sizeof(float), user);

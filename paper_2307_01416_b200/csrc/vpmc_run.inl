@@ -44,6 +44,8 @@ static double ct_min_w(const vpmc_t *h, const BeamHost &b, const float shift[3])
 static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
 {
     if (h->beams.empty()) FAIL(h, VPMC_ERR_STATE, "no beam");
+    join_setup(h, st);
+    h->launched = true;
     if (h->spots_dirty) {
         std::vector<float4> sp;
         std::vector<double> r0;
@@ -57,18 +59,14 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
             }
         h->n_spots = (int)sp.size();
         if (h->n_spots == 0) FAIL(h, VPMC_ERR_STATE, "no spots");
-        if (h->d_spots) cudaFree(h->d_spots);
-        if (h->d_spot_R0) cudaFree(h->d_spot_R0);
-        if (h->d_spot_beam) cudaFree(h->d_spot_beam);
-        if (h->d_beams) cudaFree(h->d_beams);
+        dev_release(h, h->d_spots); dev_release(h, h->d_spot_R0); dev_release(h, h->d_spot_beam); dev_release(h, h->d_beams);
         h->d_spots = nullptr; h->d_spot_R0 = nullptr; h->d_spot_beam = nullptr; h->d_beams = nullptr;
-        CU(h, cudaMalloc(&h->d_spots, sp.size() * sizeof(float4)));
-        CU(h, cudaMalloc(&h->d_spot_R0, r0.size() * sizeof(double)));
-        CU(h, cudaMalloc(&h->d_spot_beam, sp.size() * sizeof(int)));
-        CU(h, cudaMalloc(&h->d_beams, h->beams.size() * sizeof(DevBeam)));
-        CU(h, cudaMemcpy(h->d_spots, sp.data(), sp.size() * sizeof(float4), cudaMemcpyHostToDevice));
-        CU(h, cudaMemcpy(h->d_spot_R0, r0.data(), r0.size() * sizeof(double), cudaMemcpyHostToDevice));
-        CU(h, cudaMemcpy(h->d_spot_beam, h->spot_beam_h.data(), sp.size() * sizeof(int), cudaMemcpyHostToDevice));
+        int rc;
+        if ((rc = dev_alloc(h, (void **)&h->d_spots, sp.size() * sizeof(float4))) || (rc = dev_alloc(h, (void **)&h->d_spot_R0, r0.size() * sizeof(double))) ||
+            (rc = dev_alloc(h, (void **)&h->d_spot_beam, sp.size() * sizeof(int))) || (rc = dev_alloc(h, (void **)&h->d_beams, h->beams.size() * sizeof(DevBeam)))) return rc;
+        CU(h, cudaMemcpyAsync(h->d_spots, sp.data(), sp.size() * sizeof(float4), cudaMemcpyHostToDevice, st));
+        CU(h, cudaMemcpyAsync(h->d_spot_R0, r0.data(), r0.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        CU(h, cudaMemcpyAsync(h->d_spot_beam, h->spot_beam_h.data(), sp.size() * sizeof(int), cudaMemcpyHostToDevice, st));
         h->spots_dirty = false;
     }
     std::vector<DevBeam> db(h->beams.size());
@@ -153,17 +151,28 @@ static void enqueue_chunk(vpmc_t *h, const Ctx &c, const WorkMap &wm, unsigned l
     const unsigned int n = (unsigned int)wm.n_items;
     const int blocks = (int)((n + kBlock - 1) / kBlock);
     cudaMemsetAsync(h->d_qctr, 0, 8 * sizeof(unsigned int), st);
+    // timing classes: 4 = the one-thread-per-item stage kernels, 0 = the persistent beam-line kernels, 1 = the voxel kernel
     {
-        TimedScope ts(h, st, 0, timed);
+        TimedScope ts(h, st, 4, timed);
         source_kernel<<<blocks, kBlock, 0, st>>>(c, wm, i0, h->d_spots, h->d_spot_R0, h->d_spot_beam, cb.sb, cb.q_ap, cb.q_ct, tal);
-        if (h->any_rs) {
+    }
+    if (h->any_rs) {
+        {
+            TimedScope ts(h, st, 0, timed);
             beam_kernel<0><<<std::min(h->grid_beam[0], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_rs_out, cb.q_rs_out, cb.rs_head, tal);
-            ap_entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_rs_out, cb.q_ap, cb.q_ct, tal);
         }
-        if (h->any_ap) beam_kernel<1><<<std::min(h->grid_beam[1], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_ap, cb.q_ct, cb.ap_head, tal);
+        TimedScope ts(h, st, 4, timed);
+        ap_entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_rs_out, cb.q_ap, cb.q_ct, tal);
+    }
+    if (h->any_ap) {
+        TimedScope ts(h, st, 0, timed);
+        beam_kernel<1><<<std::min(h->grid_beam[1], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_ap, cb.q_ct, cb.ap_head, tal);
+    }
+    {
+        TimedScope ts(h, st, 4, timed);
+        entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_ct, tal);
     }
     TimedScope ts(h, st, 1, timed);
-    entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_ct, tal);
     if (h->smem_lut)
         voxel_kernel<MODE, true><<<std::min(h->grid[MODE][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, cb.q_ct, h->d_lut, sa, tal);
     else
@@ -206,8 +215,7 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     const int B = h->params.n_batches;
     const bool with_unc = B >= 2;
     if (with_unc && !h->d_s1) {
-        CU(h, cudaMalloc(&h->d_s1, h->nvox * sizeof(float)));
-        CU(h, cudaMalloc(&h->d_s2, h->nvox * sizeof(float)));
+        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->nvox * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->nvox * sizeof(float)))) return rc;
     }
     rc = ensure(h, h->edep, (size_t)B * h->nvox * sizeof(float)); if (rc) return rc;
     const size_t n_ent = (size_t)B * h->n_spots;
@@ -226,6 +234,12 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
             const unsigned __int128 n = cnt[g];
             unsigned long long lo = start[g] + (unsigned long long)((n * (unsigned)b) / (unsigned)B);
             unsigned long long hi = start[g] + (unsigned long long)((n * (unsigned)(b + 1)) / (unsigned)B);
+            if (h->shard_count > 1) {           // S:8e: shard k of K of every (spot, batch) id range
+                const unsigned __int128 len = hi - lo;
+                const unsigned long long a = lo + (unsigned long long)((len * (unsigned)h->shard_index) / (unsigned)h->shard_count);
+                hi = lo + (unsigned long long)((len * (unsigned)(h->shard_index + 1)) / (unsigned)h->shard_count);
+                lo = a;
+            }
             lo = std::max(lo, wlo); hi = std::min(hi, whi);
             const size_t e = (size_t)b * h->n_spots + g;
             first[e] = lo;
@@ -312,7 +326,7 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
         CU(h, cudaStreamCreateWithFlags(&h->seq_stream, cudaStreamNonBlocking));
         CU(h, cudaEventCreateWithFlags(&h->seq_ev_in, cudaEventDisableTiming));
         CU(h, cudaEventCreateWithFlags(&h->seq_ev_out, cudaEventDisableTiming));
-        CU(h, cudaMalloc(&h->d_seq, sizeof(SeqState)));
+        int rc0 = dev_alloc(h, (void **)&h->d_seq, sizeof(SeqState)); if (rc0) return rc0;
     }
     cudaStream_t st = h->seq_stream;
     CU(h, cudaStreamSynchronize(st));        // a previous graph of this handle must have drained before it is rebuilt
@@ -323,8 +337,7 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     h->last_stream = caller;
     h->unc_valid = false; h->seq_valid = false;
     if (!h->d_s1) {
-        CU(h, cudaMalloc(&h->d_s1, h->nvox * sizeof(float)));
-        CU(h, cudaMalloc(&h->d_s2, h->nvox * sizeof(float)));
+        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->nvox * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->nvox * sizeof(float)))) return rc;
     }
     ChunkBufs cb;
     if ((rc = ensure(h, h->edep, (size_t)h->nvox * sizeof(float))) ||
