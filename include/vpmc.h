@@ -225,6 +225,28 @@ int vpmc_get_influence_stats(vpmc_t *h, vpmc_influence_stats *out);
 int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, float rel_threshold,
                         int32_t *col_out_dev, float *val_out_dev, int64_t *nnz_out);
 
+/* ---- S:8f-1: one iteration of the robust optimiser on the influence matrices ("0.1-0.3 s per iteration", P:L160
+ * "13 uncertainty scenarios were included in the robust optimization").  The paper prints no objective; D:R16 takes
+ * the voxel-wise worst case over the scenarios of a weighted quadratic deviation.  A matrix is a vpmc_csr as vpmc_influence
+ * returns it (rows = spots, columns = voxels, [device]); vectors are fp32 [device]; everything is enqueued on cuda_stream.
+ *
+ * vpmc_spmv_dose:  dose[v] = sum_j D[j][v] w[j], v < n_cols; dose_dev (n_cols floats) is overwritten.  fp32 sums by
+ *                  atomic additions: equal up to their order.
+ * vpmc_spmv_grad:  grad[j] (+)= sum_v D[j][v] r[v] (accumulate != 0 adds to grad_dev); sums in a fixed order: bit-reproducible.
+ * vpmc_worst_case: doses_dev, resid_dev: [n_sc][n] row-major.  Per voxel v: e_s = d_s[v] - target[v], s* = the scenario with
+ *                  the largest e_s^2 (products rounded to fp32; the lowest index among equals), resid[s*][v] = 2 weight[v]
+ *                  e_s*, resid[s][v] = 0 otherwise; *objective_dev (one double, [device]) = sum_v weight[v] e_s*^2.
+ * vpmc_robust_iteration: all of it -- n_sc dose products into doses_ws_dev ([n_sc][n_cols]), the worst case into resid_ws_dev
+ *                  (same shape) and *objective_dev, then grad_dev[j] = sum_s sum_v D_s[j][v] resid_s[v], scenarios added in
+ *                  order.  All matrices must have the same number of rows. */
+int vpmc_spmv_dose(vpmc_t *h, const vpmc_csr *m, int64_t n_cols, const float *w_dev, float *dose_dev, void *cuda_stream);
+int vpmc_spmv_grad(vpmc_t *h, const vpmc_csr *m, const float *r_dev, float *grad_dev, int accumulate, void *cuda_stream);
+int vpmc_worst_case(vpmc_t *h, const float *doses_dev, int32_t n_sc, int64_t n, const float *target_dev, const float *weight_dev,
+                    float *resid_dev, double *objective_dev, void *cuda_stream);
+int vpmc_robust_iteration(vpmc_t *h, const vpmc_csr *mats, int32_t n_sc, int64_t n_cols, const float *w_dev, const float *target_dev,
+                          const float *weight_dev, float *doses_ws_dev, float *resid_ws_dev, float *grad_dev, double *objective_dev,
+                          void *cuda_stream);
+
 /* Upper bound in bytes on the per-group scratch of vpmc_influence (the dense per-column boxes of one group of spots);
  * 0 = automatic (a third of the free device memory, at most 24 GiB).  Smaller limits only mean more groups. */
 int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes);
@@ -302,8 +324,8 @@ int vpmc_set_knob(vpmc_t *h, int knob, double value);
  * stream.  vpmc_get_timing synchronises, returns accumulated milliseconds and launch counts per class
  * (0 beam_kernel: the persistent range-shifter / brass kernels S2-S3, 1 voxel_kernel S4-S7 incl. the influence pilot,
  * 2 dose conversion / uncertainty passes S6, 3 CSR writer passes S8, 4 the one-thread-per-item stage kernels: source +
- * opening phase S1/S3, aperture entry, CT entry) and resets. */
-#define VPMC_N_KERNEL_CLASSES 5
+ * opening phase S1/S3, aperture entry, CT entry, 5 the optimiser-iteration kernels S:8f-1) and resets. */
+#define VPMC_N_KERNEL_CLASSES 6
 int vpmc_set_timing(vpmc_t *h, int on);
 int vpmc_get_timing(vpmc_t *h, double *ms_out, uint64_t *launches_out);
 

@@ -307,10 +307,10 @@ class Engine:
     def timing(self):
         """{class: (milliseconds, launches)} accumulated since the last call; classes beamline (persistent beam kernels) /
         voxel / scoring / writer / stage (one-thread-per-item source, aperture-entry and CT-entry kernels)."""
-        ms = (C.c_double * 5)()
-        n = (C.c_uint64 * 5)()
+        ms = (C.c_double * 6)()
+        n = (C.c_uint64 * 6)()
         self._check(lib().vpmc_get_timing(self._h, ms, n))
-        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("beamline", "voxel", "scoring", "writer", "stage"))}
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("beamline", "voxel", "scoring", "writer", "stage", "optimiser"))}
 
     def trace(self, hids, n_or_hps: int, seed: int, sc: Scenario | None = None, mode: int = 0, max_steps: int = 1024):
         hids = np.ascontiguousarray(np.asarray(hids, dtype=np.uint64))

@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvpmc.so")
 SOURCES = ["vpmc_api.cu"]
 DEPS = ["vpmc_api.cu", "vpmc_run.inl", "vpmc_influence.inl", "vpmc_host.h", "vpmc_kernels.cuh", "vpmc_transport.cuh",
-        "vpmc_device.cuh", "vpmc_setup.cuh", "../../include/vpmc.h"]
+        "vpmc_device.cuh", "vpmc_setup.cuh", "vpmc_spmv.cuh", "vpmc_spmv.inl", "../../include/vpmc.h"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -18,7 +18,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
-           "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",
+           "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-ftz=true",
            "-Xptxas", "-v" if verbose else "-O3", "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)

@@ -197,10 +197,26 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
-                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n };
+                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part };
     for (DevBuf *b : bufs) if (b->p) { pool_give(b->p, b->bytes); b->p = nullptr; }
     delete h;
     return VPMC_OK;
+}
+
+// the persistent kernels by (stage | mode, table placement, fl): fl = 1 is the specialisation for flags == 7
+typedef void (*BeamFn)(const Ctx, const SourceBuf, const Queue, const Queue, unsigned int *, DevTallies *);
+typedef void (*VoxelFn)(const Ctx, const Queue, const float4 *, const ScoreArgs, DevTallies *);
+static BeamFn beam_fn(int stage, int fl)
+{
+    static const BeamFn t[2][2] = { { beam_kernel<0, -1>, beam_kernel<0, 7> }, { beam_kernel<1, -1>, beam_kernel<1, 7> } };
+    return t[stage][fl];
+}
+static VoxelFn voxel_fn(int mode, int smem, int fl)
+{
+    static const VoxelFn t[3][2][2] = { { { voxel_kernel<0, false, -1>, voxel_kernel<0, false, 7> }, { voxel_kernel<0, true, -1>, voxel_kernel<0, true, 7> } },
+                                        { { voxel_kernel<1, false, -1>, voxel_kernel<1, false, 7> }, { voxel_kernel<1, true, -1>, voxel_kernel<1, true, 7> } },
+                                        { { voxel_kernel<2, false, -1>, voxel_kernel<2, false, 7> }, { voxel_kernel<2, true, -1>, voxel_kernel<2, true, 7> } } };
+    return t[mode][smem][fl];
 }
 
 extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *cal, const vpmc_params *params)
@@ -272,7 +288,7 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     {
         h->tally_smem = (kWarps * sizeof(WarpTally) + 15) / 16 * 16;
         // occupancy queries are ~0.3 ms each: remember the answer per (device, table size, table placement)
-        struct GridCache { int device; size_t lut_bytes; bool smem; int grid_beam[2]; int grid[3][2]; };
+        struct GridCache { int device; size_t lut_bytes; bool smem; int grid_beam[2][2]; int grid[3][2][2]; };
         static std::mutex mu;
         static std::vector<GridCache> cache;
         bool hit = false;
@@ -283,27 +299,26 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
         }
         if (!hit) {
             int occ = 0;
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel<0>, kBlock, 0));
-            h->grid_beam[0] = std::max(occ, 1) * h->n_sm;
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_kernel<1>, kBlock, 0));
-            h->grid_beam[1] = std::max(occ, 1) * h->n_sm;
-            const void *fn[3][2] = { { (const void *)voxel_kernel<0, false>, (const void *)voxel_kernel<0, true> },
-                                     { (const void *)voxel_kernel<1, false>, (const void *)voxel_kernel<1, true> },
-                                     { (const void *)voxel_kernel<2, false>, (const void *)voxel_kernel<2, true> } };
-            for (int m = 0; m < 3; ++m)
-                for (int s = 0; s < 2; ++s) {
-                    if (s == 1 && !h->smem_lut) continue;
-                    const size_t sm = h->tally_smem + (s ? h->lut_bytes : 0);
-                    if (s) CUC(cudaFuncSetAttribute(fn[m][s], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxSmemLut + h->tally_smem)));
-                    CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn[m][s], kBlock, sm));
-                    h->grid[m][s] = std::max(occ, 1) * h->n_sm;
+            for (int st = 0; st < 2; ++st)
+                for (int f = 0; f < 2; ++f) {
+                    CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, beam_fn(st, f), kBlock, 0));
+                    h->grid_beam[st][f] = std::max(occ, 1) * h->n_sm;
                 }
+            for (int m = 0; m < 3; ++m)
+                for (int s = 0; s < 2; ++s)
+                    for (int f = 0; f < 2; ++f) {
+                        if (s == 1 && !h->smem_lut) continue;
+                        const size_t sm = h->tally_smem + (s ? h->lut_bytes : 0);
+                        if (s) CUC(cudaFuncSetAttribute(voxel_fn(m, s, f), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxSmemLut + h->tally_smem)));
+                        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, voxel_fn(m, s, f), kBlock, sm));
+                        h->grid[m][s][f] = std::max(occ, 1) * h->n_sm;
+                    }
             GridCache g; g.device = h->device; g.lut_bytes = h->lut_bytes; g.smem = h->smem_lut; memcpy(g.grid_beam, h->grid_beam, sizeof(g.grid_beam)); memcpy(g.grid, h->grid, sizeof(g.grid));
             std::lock_guard<std::mutex> lk(mu);
             cache.push_back(g);
         }
     }
-    CUC(cudaEventSynchronize(h->copy_ev));     // the caller's arrays are copied during the call (vpmc.h)
+    h->fl = (p.flags == (VPMC_FLAG_MCS | VPMC_FLAG_STRAGGLE | VPMC_FLAG_NUCLEAR)) ? 1 : 0;
 #undef CUC
 #undef CUA
     *out = h;

@@ -183,9 +183,13 @@ __device__ __forceinline__ float highland_dA(float t, float dt, float c_log, flo
 // R = alpha E^p every step; in fp32 that round trip loses 2^-24 of the FULL range per step, which the end of range
 // amplifies (dE/dR ~ 10 MeV/mm).  Here R is carried in fp64 and updated by differences:
 // R' = R - s rsp, and, after straggling, R_next = alpha E'^p = R' (E'/Ebar')^p = R' + R' ((1 + delta)^p - 1).
+// FL = the physics switches as a compile-time constant (the kernels are specialised for the default MCS | STRAGGLE | NUCLEAR),
+// or -1 = read them from the parameters.
+template <int FL>
 __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const Medium &m, float d,
                                             const PhiloxKey &K, StepOut &o)
 {
+    const int flags = (FL >= 0) ? FL : P.flags;
     o.removed = 0.0f; o.on_d = 0; o.theta = 0.0f; o.uphi = 0.5f;
     const float E = h.E;
     // 1
@@ -213,7 +217,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     // 4
     float Ep = Ebar, dep = dEm;
     double Rn = Rp;
-    if (P.flags & 2) {
+    if (flags & 2) {
         const float Emid = 0.5f * (E + Ebar);
         const float g = 1.0f + Emid * (1.0f / kMp);
         const float var = P.k_bohr * m.za_rho * s * 0.5f * fmaf(g, g, 1.0f);   // gamma^2 (1 - beta^2/2) = (gamma^2+1)/2
@@ -236,7 +240,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     o.dep = dep;
     o.s = s;
     // 6
-    if (P.flags & 4) {
+    if (flags & 4) {
         h.tau = fmaf(__fdividef(P.beta_nuc, fmaf(P.beta_nuc, R, 1.0f)) * m.rho_rel, s, h.tau);
         if (h.tau >= h.tau_star) {
             o.dep += P.gamma_loc * Ep;
@@ -246,7 +250,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
         }
     }
     // 7
-    if (P.flags & 1) {
+    if (flags & 1) {
         const float dt = s * m.inv_X0;
         const float dA = fmaxf(highland_dA(h.t_rad, dt, P.c_log, h.f_rad), 0.0f);
         const float Em = 0.5f * (E + Ep);

@@ -8,6 +8,7 @@
 
 #include "../../include/vpmc.h"
 #include "vpmc_kernels.cuh"
+#include "vpmc_spmv.cuh"
 
 struct BeamHost {
     vpmc_frame frame;
@@ -90,6 +91,7 @@ struct vpmc {
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
         ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
     vpmc_influence_stats inf_stats = {};
+    DevBuf spmv_part;                 // first / last partial sums per chunk of vpmc_spmv_grad
     size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
 
     // knobs (vpmc_set_knob)
@@ -100,8 +102,11 @@ struct vpmc {
     bool verbose = false;
 
     // launch configuration
-    int grid_beam[2] = { 0, 0 };      // resident CTAs of beam_kernel<STAGE>
-    int grid[3][2] = { { 0, 0 }, { 0, 0 }, { 0, 0 } };   // [mode][smem_lut] resident CTAs of voxel_kernel
+    // resident CTAs of beam_kernel<STAGE, FL> [stage][fl] and voxel_kernel<MODE, SMEM_LUT, FL> [mode][smem_lut][fl]; fl = 1: the
+    // kernels specialised for the default physics switches (flags == 7), 0: the switches read at run time
+    int grid_beam[2][2] = {};
+    int grid[3][2][2] = {};
+    int fl = 1;
     bool smem_lut = false;
     size_t lut_bytes = 0, tally_smem = 0;
 

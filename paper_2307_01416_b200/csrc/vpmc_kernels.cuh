@@ -318,7 +318,7 @@ ap_entry_kernel(const Ctx c, const Queue q_in, const Queue q_ap, const Queue q_c
 // range-shifter records), STAGE 1 the brass of the aperture region (input: the aperture queue).  A lane whose history ended
 // or left the device loads the next record (warp-aggregated claim on the input counter); histories that left the device
 // alive are pushed to `out` (STAGE 0: the aperture-entry queue, STAGE 1: the CT queue) with one atomic per warp and pass.
-template <int STAGE>
+template <int STAGE, int FL>
 __global__ void __launch_bounds__(kBlock, VPK_MIN_BLOCKS)
 beam_kernel(const Ctx c, const SourceBuf sb, const Queue in, const Queue out, unsigned int *head, DevTallies *tal)
 {
@@ -379,7 +379,7 @@ beam_kernel(const Ctx c, const SourceBuf sb, const Queue in, const Queue out, un
             continue;
         }
         if (alive) {
-            const int status = (STAGE == 0) ? rs_iter(c, h, dep, lc, tr) : ap_iter(c, h, dep, lc, tr, alive_mask);
+            const int status = (STAGE == 0) ? rs_iter<FL>(c, h, dep, lc, tr) : ap_iter<FL>(c, h, dep, lc, tr, alive_mask);
             if (status != BEAM_CONT) { alive = false; pend = status; }
         }
     }
@@ -426,7 +426,7 @@ entry_kernel(const Ctx c, const Queue q, DevTallies *tal)
 // S4-S7: persistent warps; free lanes load survivors from the queue (one atomic per warp and refill) and step through
 // the voxels with ct_step().  MODE 0 scores the dose grid(s), MODE 1 per-column boxes, MODE 2 only column bounding
 // boxes.  SMEM_LUT: material table staged in shared memory.
-template <int MODE, bool SMEM_LUT>
+template <int MODE, bool SMEM_LUT, int FL>
 __global__ void __launch_bounds__(kBlock, VPK_MIN_BLOCKS)
 voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const ScoreArgs sa, DevTallies *tal)
 {
@@ -495,8 +495,8 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         }
         if (alive) {
             int cause;
-            if (SMEM_LUT) cause = ct_step(c, LutShared{ lut_s }, h, hdep, lc, sc, tr);
-            else cause = ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
+            if (SMEM_LUT) cause = ct_step<FL>(c, LutShared{ lut_s }, h, hdep, lc, sc, tr);
+            else cause = ct_step<FL>(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
             if (cause != CONT) { alive = false; pend = cause; }
         }
     }
@@ -521,7 +521,7 @@ __device__ __forceinline__ float trace_history(const Ctx &c, unsigned long long 
     for (int it = 0; it < 1000000 && code == BEAM_CONT; ++it) code = beam_step(c, h, dep_rs, dep_ap, lc, tr);
     if (code == BEAM_EXIT && ct_entry(c, h, lc, sink, tr) == CONT) {
         for (int it = 0; it < 1000000; ++it)
-            if (ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr) != CONT) break;
+            if (ct_step<-1>(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr) != CONT) break;
     }
     return hdep;
 }
@@ -638,7 +638,7 @@ __global__ void step_state_kernel(const Ctx c, const StateIn *__restrict__ in, i
         h.rx = l[0]; h.ry = l[1]; h.rz = l[2];
         h.g0 = (uint32_t)q.ivox[0]; h.g1 = (uint32_t)q.ivox[1]; h.g2 = (uint32_t)q.ivox[2];
         h.g3 = (uint32_t)(q.ivox[0] + G.nx * (q.ivox[1] + G.ny * q.ivox[2]));
-        ct_step(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
+        ct_step<-1>(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
     }
     if (q.kind == STEP_CT_ENTRY || q.kind == STEP_CT) {
         o.ivox_after[0] = (int)h.g0; o.ivox_after[1] = (int)h.g1; o.ivox_after[2] = (int)h.g2;

@@ -159,24 +159,22 @@ static void enqueue_chunk(vpmc_t *h, const Ctx &c, const WorkMap &wm, unsigned l
     if (h->any_rs) {
         {
             TimedScope ts(h, st, 0, timed);
-            beam_kernel<0><<<std::min(h->grid_beam[0], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_rs_out, cb.q_rs_out, cb.rs_head, tal);
+            beam_fn(0, h->fl)<<<std::min(h->grid_beam[0][h->fl], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_rs_out, cb.q_rs_out, cb.rs_head, tal);
         }
         TimedScope ts(h, st, 4, timed);
         ap_entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_rs_out, cb.q_ap, cb.q_ct, tal);
     }
     if (h->any_ap) {
         TimedScope ts(h, st, 0, timed);
-        beam_kernel<1><<<std::min(h->grid_beam[1], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_ap, cb.q_ct, cb.ap_head, tal);
+        beam_fn(1, h->fl)<<<std::min(h->grid_beam[1][h->fl], blocks), kBlock, 0, st>>>(c, cb.sb, cb.q_ap, cb.q_ct, cb.ap_head, tal);
     }
     {
         TimedScope ts(h, st, 4, timed);
         entry_kernel<<<blocks, kBlock, 0, st>>>(c, cb.q_ct, tal);
     }
     TimedScope ts(h, st, 1, timed);
-    if (h->smem_lut)
-        voxel_kernel<MODE, true><<<std::min(h->grid[MODE][1], blocks), kBlock, h->tally_smem + h->lut_bytes, st>>>(c, cb.q_ct, h->d_lut, sa, tal);
-    else
-        voxel_kernel<MODE, false><<<std::min(h->grid[MODE][0], blocks), kBlock, h->tally_smem, st>>>(c, cb.q_ct, h->d_lut, sa, tal);
+    const int sl = h->smem_lut ? 1 : 0;
+    voxel_fn(MODE, sl, h->fl)<<<std::min(h->grid[MODE][sl][h->fl], blocks), kBlock, h->tally_smem + (sl ? h->lut_bytes : 0), st>>>(c, cb.q_ct, h->d_lut, sa, tal);
 }
 
 static unsigned int chunk_launches(const vpmc_t *h) { return 3u + (h->any_rs ? 2u : 0u) + (h->any_ap ? 1u : 0u); }
@@ -543,3 +541,4 @@ extern "C" int vpmc_step_from_state(vpmc_t *h, const vpmc_scenario *scp, uint64_
 }
 
 #include "vpmc_influence.inl"
+#include "vpmc_spmv.inl"

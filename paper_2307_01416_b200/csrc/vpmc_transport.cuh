@@ -288,21 +288,21 @@ __device__ __forceinline__ void slab_geometry(const DevParams &P, const DevBeam 
 }
 
 // one slab step (range shifter or brass): C4 items 1-8 and 10.  `out` = the history reached the exit plane of the device.
-template <class Tracer>
+template <int FL, class Tracer>
 __device__ __forceinline__ int slab_step(const Ctx &c, Hist &h, const Medium &m, const SlabGeom &g, int reg, float &dep,
                                          LaneCounters &lc, Tracer &tr, bool &out)
 {
     StepOut o;
     const float Eb = h.E; const uint32_t st = h.step;
     const float lat = fmaxf(fabsf(h.ux), fabsf(h.uy));        // direction of travel during the step
-    const int cause = step_physics(c.P, h, m, g.d, c.K, o);
+    const int cause = step_physics<FL>(c.P, h, m, g.d, c.K, o);
     h.rx = fmaf(-o.s, lat, h.rx);                              // brass budget (meaningless, and unused, in the range shifter)
     if (cause == CONT) {
         // C4-8: move along the OLD direction, then rotate
         pair_axpy(h.g0, h.g1, o.s, h.ux, h.lx);
         pair_axpy(h.g2, h.g3, o.s, h.uy, h.ly);
         h.rz = fmaf(o.s, h.uz, h.rz);
-        if (c.P.flags & 1) rotate(h, o.theta, o.uphi);
+        if (((FL >= 0) ? FL : c.P.flags) & 1) rotate(h, o.theta, o.uphi);
     }
     dep += o.dep;
     lc.n_slab += (cause != STOPPED);
@@ -332,7 +332,7 @@ __device__ __forceinline__ int rs_enter(const Ctx &c, Hist &h, Tracer &tr)
 }
 
 // one range-shifter step (S2; homogeneous, energy-only medium)
-template <class Tracer>
+template <int FL, class Tracer>
 __device__ __forceinline__ int rs_iter(const Ctx &c, Hist &h, float &dep_rs, LaneCounters &lc, Tracer &tr)
 {
     const DevParams &P = c.P;
@@ -342,7 +342,7 @@ __device__ __forceinline__ int rs_iter(const Ctx &c, Hist &h, float &dep_rs, Lan
     slab_geometry(P, bp, true, h, g);
     const Medium m = { P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
     bool out;
-    const int cause = slab_step(c, h, m, g, REG_RS, dep_rs, lc, tr, out);
+    const int cause = slab_step<FL>(c, h, m, g, REG_RS, dep_rs, lc, tr, out);
     if (cause != CONT) return (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
     if (!out) return BEAM_CONT;
     h.region = (__ldg(&bp->has_ap) ? REG_TO_AP : REG_TO_CT) | (h.region & ~0xff);
@@ -451,7 +451,7 @@ __device__ __forceinline__ int ap_enter(const Ctx &c, Hist &h, Tracer &tr)
 // brass, then at most ONE brass step.  `conv` = the lanes of the warp that called together: they re-converge before the
 // expensive slab step, whatever the opening phase did (0 = no forced re-convergence, for one-thread-per-history callers).
 // dep_ap = energy deposited so far in the brass.
-template <class Tracer>
+template <int FL, class Tracer>
 __device__ __forceinline__ int ap_iter(const Ctx &c, Hist &h, float &dep_ap, LaneCounters &lc, Tracer &tr, unsigned conv)
 {
     const DevParams &P = c.P;
@@ -469,7 +469,7 @@ __device__ __forceinline__ int ap_iter(const Ctx &c, Hist &h, float &dep_ap, Lan
     if (do_step) {
         const Medium m = { P.brass_rsp, P.brass_inv_rsp, P.brass_rho, P.brass_inv_X0, P.brass_za_rho };
         bool out;
-        const int cause = slab_step(c, h, m, g, REG_AP, dep_ap, lc, tr, out);
+        const int cause = slab_step<FL>(c, h, m, g, REG_AP, dep_ap, lc, tr, out);
         if (cause != CONT) status = (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
         else if (out) { h.region = REG_TO_CT | (h.region & ~0xff); status = BEAM_EXIT; }
     }
@@ -489,7 +489,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
         reg = REG_RS;
     }
     if (reg == REG_RS) {
-        const int st = rs_iter(c, h, dep_rs, lc, tr);
+        const int st = rs_iter<-1>(c, h, dep_rs, lc, tr);
         if (st != BEAM_EXIT) return st;
         return ((h.region & 0xff) == REG_TO_CT) ? BEAM_EXIT : BEAM_CONT;      // the aperture follows
     }
@@ -497,7 +497,7 @@ __device__ __forceinline__ int beam_step(const Ctx &c, Hist &h, float &dep_rs, f
         const int st = ap_enter(c, h, tr);
         if (st != BEAM_CONT) return st;
     }
-    return ap_iter(c, h, dep_ap, lc, tr, 0u);
+    return ap_iter<-1>(c, h, dep_ap, lc, tr, 0u);
 }
 
 // ---- once-per-history bookkeeping (tallies of S:8b), done in the kernels' event passes by ALL 32 lanes of the warp together:
@@ -549,7 +549,7 @@ __device__ __forceinline__ int ct_entry(const Ctx &c, Hist &h, LaneCounters &lc,
 
 // One voxel step of history h (S4, S5, S6/S7).  Returns CONT or the cause that ended the history; the once-per-history
 // tallies are booked by book_ct_end() in the kernel's refill pass.  hdep = energy deposited in the CT so far.
-template <class Lut, class Scorer, class Tracer>
+template <int FL, class Lut, class Scorer, class Tracer>
 __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, float &hdep, LaneCounters &lc,
                                        Scorer &sc, Tracer &tr)
 {
@@ -563,13 +563,13 @@ __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, fl
     const Medium m = { mv.x * c.rsp_scale, mv.w * c.inv_rsp_scale, mv.y, mv.z, P.za_w * mv.y };
     StepOut o;
     const float Eb = h.E; const uint32_t st = h.step;
-    int cause = step_physics(P, h, m, d, c.K, o);
+    int cause = step_physics<FL>(P, h, m, d, c.K, o);
     if (cause == CONT) {
         // C4-8: move along the OLD direction, then rotate
         h.rx = fmaf(o.s, h.lx, fmaf(o.s, h.ux, h.rx));
         h.ry = fmaf(o.s, h.ly, fmaf(o.s, h.uy, h.ry));
         h.rz = fmaf(o.s, h.lz, fmaf(o.s, h.uz, h.rz));
-        if (P.flags & 1) rotate(h, o.theta, o.uphi);
+        if (((FL >= 0) ? FL : P.flags) & 1) rotate(h, o.theta, o.uphi);
     }
     hdep += o.dep;
     if (o.dep != 0.0f) sc.deposit(h, o.dep);      // S6 / S7: the voxel at the START of the step
