@@ -523,6 +523,7 @@ def measure_influence(hps, steps, warmup):
     clocks = sampler.stop()
     tm = eng.timing()
     st = eng.influence_stats()
+    opt = measure_optimiser(eng, sc, hps, w, hbm_gbs, peak_kind)
     tl = eng.tallies()
     n_hist = len(sc) * eng.n_spots * hps
     wr_s = tm["writer"][0] * 1e-3 / steps
@@ -542,9 +543,43 @@ def measure_influence(hps, steps, warmup):
                       "bytes_as_implemented": impl, "achieved_as_implemented": impl / wr_s / 1e9 if wr_s > 0 else None,
                       "note": "algorithmic = 8 B x nnz written + 3 reads x 4 B of every box element (max, count, emit); the class also times the "
                               "library sort of the overflow list", "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"},
+           "optimiser_iteration": opt,
            "paper_context": "41.6 s for 13 influence matrices (P:L205-207): other data, other hardware"}
     eng.close()
     return out
+
+
+def measure_optimiser(eng, sc, hps, w, hbm_gbs, peak_kind, iters=5):
+    """SURVEY.md 8(f)-1 on the matrices just built: seconds per robust-optimiser iteration (13 dose products, the voxel-wise
+    worst case, 13 gradient products) with the 13 matrices resident in HBM; every entry streams through twice."""
+    import torch
+    mats = eng.influence(sc, hps, w["rel_threshold"], SEED)
+    nnz = sum(int(c.numel()) for (_, c, _) in mats)
+    n_sc, nvox = len(mats), eng.nvox
+    wts = torch.full((eng.n_spots,), 1.0e8, dtype=torch.float32, device="cuda")
+    d0 = eng.spmv_dose(mats[0], wts)
+    target = (0.95 * d0).contiguous()
+    weight = (d0 > 0.05 * d0.max()).float()
+    ws = (torch.empty((n_sc, nvox), dtype=torch.float32, device="cuda"), torch.empty((n_sc, nvox), dtype=torch.float32, device="cuda"))
+    obj, grad, _ = eng.robust_iteration(mats, wts, target, weight, ws=ws)          # warm-up
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(grad).all())
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    t_ms = 0.0
+    for _ in range(iters):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        obj, grad, _ = eng.robust_iteration(mats, wts, target, weight, ws=ws)
+        b.record(); torch.cuda.synchronize()
+        t_ms += a.elapsed_time(b)
+    sec = t_ms * 1e-3 / iters
+    alg = 16.0 * nnz + 4.0 * 4.0 * n_sc * nvox       # every entry (col + val) read twice; per scenario the dose and residual vectors written and read once each
+    del mats
+    return {"seconds_per_iteration": sec, "nnz": nnz, "scenarios": n_sc, "bound": "hbm", "algorithmic_bytes": alg, "achieved": alg / sec / 1e9,
+            "peak": hbm_gbs, "unit": "GB/s", "frac": alg / sec / 1e9 / hbm_gbs, "objective": float(obj), "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs",
+            "l2_flush_between_iterations": True,
+            "paper_context": "0.1-0.3 s per iteration on 4 x A100 (P:L95): other data, other hardware"}
 
 
 if __name__ == "__main__":

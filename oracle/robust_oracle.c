@@ -8,7 +8,9 @@
  *
  *   d_s[v]  = sum_j D_s[j][v] w_j                                   dose of scenario s (D_s: rows = spots j, CSR, C6)
  *   e_s[v]  = d_s[v] - t[v]
- *   s*(v)   = the scenario with the largest e_s[v]^2, the lowest index among equals
+ *   s*(v)   = the scenario with the largest e_s[v]^2, the lowest index among equals; this one comparison is taken in fp32
+ *             (difference and product each rounded to fp32), the precision the kernel takes it in, so that both sides
+ *             decide the integer s* alike on fp32 inputs; every value (f, r, g) is fp64
  *   f(w)    = sum_v p[v] e_{s*(v)}[v]^2
  *   r_s[v]  = 2 p[v] e_s[v] if s = s*(v), else 0
  *   g[j]    = sum_s sum_v D_s[j][v] r_s[v]                           gradient of f where s* is locally constant
@@ -48,9 +50,13 @@ double orb_worst_case(const double *doses, int32_t n_sc, int64_t n, const double
     for (int64_t v = 0; v < n; ++v) {
         int32_t best = 0;
         double e_best = doses[v] - target[v];
+        volatile float q_best = (float)doses[v] - (float)target[v];
+        q_best = q_best * q_best;
         for (int32_t s = 1; s < n_sc; ++s) {
             const double e = doses[(size_t)s * n + v] - target[v];
-            if (e * e > e_best * e_best) { e_best = e; best = s; }
+            volatile float q = (float)doses[(size_t)s * n + v] - (float)target[v];
+            q = q * q;
+            if (q > q_best) { e_best = e; best = s; q_best = q; }
         }
         for (int32_t s = 0; s < n_sc; ++s) resid[(size_t)s * n + v] = 0.0;
         resid[(size_t)best * n + v] = 2.0 * weight[v] * e_best;

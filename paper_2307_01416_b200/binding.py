@@ -22,7 +22,8 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_set_history_window", "vpmc_influence", "vpmc_csr_from_dense", "vpmc_get_tallies",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
-           "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats"]
+           "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats", "vpmc_spmv_dose", "vpmc_spmv_grad",
+           "vpmc_worst_case", "vpmc_robust_iteration"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
@@ -144,6 +145,11 @@ def lib():
         L.vpmc_get_aperture_tables.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]
         L.vpmc_set_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
         L.vpmc_get_influence_stats.argtypes = [C.c_void_p, C.POINTER(InfluenceStats)]
+        L.vpmc_spmv_dose.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.vpmc_spmv_grad.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.vpmc_worst_case.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.vpmc_robust_iteration.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -345,6 +351,72 @@ class Engine:
             val = keep[o.val][: 4 * o.nnz].view(torch.float32) if o.nnz else torch.empty(0, dtype=torch.float32, device="cuda")
             res.append((rp, col, val))
         return res
+
+    # -- optimiser iteration on the CSR matrices (marshalling only; the products run in vpmc_spmv.cuh)
+    @staticmethod
+    def _csr(m) -> _Csr:
+        import torch
+        rp, col, val = m
+        assert rp.is_cuda and rp.dtype == torch.int64 and col.dtype == torch.int32 and val.dtype == torch.float32
+        assert rp.is_contiguous() and col.is_contiguous() and val.is_contiguous()
+        c = _Csr()
+        c.row_ptr, c.col, c.val = rp.data_ptr(), col.data_ptr() if col.numel() else None, val.data_ptr() if val.numel() else None
+        c.nnz, c.n_rows = int(col.numel()), int(rp.numel()) - 1
+        return c
+
+    def spmv_dose(self, m, w, n_cols: int | None = None, out=None, stream=None):
+        """dose[v] = sum_j D[j][v] w[j] for a CSR matrix m = (row_ptr, col, val) of CUDA tensors (rows = spots)."""
+        import torch
+        n_cols = self.nvox if n_cols is None else int(n_cols)
+        if out is None:
+            out = torch.empty(n_cols, dtype=torch.float32, device="cuda")
+        assert w.is_cuda and w.dtype == torch.float32 and w.is_contiguous() and out.numel() == n_cols
+        st = torch.cuda.current_stream() if stream is None else stream
+        c = self._csr(m)
+        self._check(lib().vpmc_spmv_dose(self._h, C.byref(c), n_cols, w.data_ptr(), out.data_ptr(), st.cuda_stream))
+        return out
+
+    def spmv_grad(self, m, r, out=None, accumulate: bool = False, stream=None):
+        """grad[j] (+)= sum_v D[j][v] r[v]."""
+        import torch
+        c = self._csr(m)
+        if out is None:
+            assert not accumulate
+            out = torch.empty(c.n_rows, dtype=torch.float32, device="cuda")
+        assert r.is_cuda and r.dtype == torch.float32 and r.is_contiguous() and out.numel() == c.n_rows
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(lib().vpmc_spmv_grad(self._h, C.byref(c), r.data_ptr(), out.data_ptr(), 1 if accumulate else 0, st.cuda_stream))
+        return out
+
+    def worst_case(self, doses, target, weight, stream=None):
+        """(objective 0-d float64 CUDA tensor, resid [n_sc, n]) of the voxel-wise worst case over the rows of doses [n_sc, n]."""
+        import torch
+        assert doses.is_cuda and doses.dtype == torch.float32 and doses.is_contiguous() and doses.dim() == 2
+        n_sc, n = doses.shape
+        assert target.numel() == n and weight.numel() == n and target.dtype == torch.float32 and weight.dtype == torch.float32
+        resid = torch.empty_like(doses)
+        obj = torch.zeros((), dtype=torch.float64, device="cuda")
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(lib().vpmc_worst_case(self._h, doses.data_ptr(), n_sc, n, target.data_ptr(), weight.data_ptr(), resid.data_ptr(),
+                                          obj.data_ptr(), st.cuda_stream))
+        return obj, resid
+
+    def robust_iteration(self, mats, w, target, weight, ws=None, stream=None):
+        """One optimiser iteration on the scenario matrices `mats`: (objective 0-d float64 tensor, grad [n_spots], doses [n_sc, nvox]).
+        ws = (doses, resid) workspaces from an earlier call, reused."""
+        import torch
+        n_sc, n = len(mats), int(target.numel())
+        arr = (_Csr * n_sc)(*[self._csr(m) for m in mats])
+        if ws is None:
+            ws = (torch.empty((n_sc, n), dtype=torch.float32, device="cuda"), torch.empty((n_sc, n), dtype=torch.float32, device="cuda"))
+        doses, resid = ws
+        grad = torch.empty(arr[0].n_rows, dtype=torch.float32, device="cuda")
+        obj = torch.zeros((), dtype=torch.float64, device="cuda")
+        assert w.is_cuda and w.dtype == torch.float32 and w.numel() == arr[0].n_rows
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(lib().vpmc_robust_iteration(self._h, arr, n_sc, n, w.data_ptr(), target.data_ptr(), weight.data_ptr(), doses.data_ptr(),
+                                                resid.data_ptr(), grad.data_ptr(), obj.data_ptr(), st.cuda_stream))
+        return obj, grad, doses
 
     def influence_stats(self) -> dict:
         st = InfluenceStats()

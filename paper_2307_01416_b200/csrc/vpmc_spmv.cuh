@@ -129,10 +129,12 @@ worst_case_kernel(const float *__restrict__ doses, int n_sc, long long n, const 
     for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
         const float t = __ldg(target + v), p = __ldg(weight + v);
         int best = 0;
-        float e_best = doses[v] - t;
+        float e_best = __fsub_rn(doses[v], t);
+        float q_best = __fmul_rn(e_best, e_best);
         for (int s = 1; s < n_sc; ++s) {
-            const float e = doses[(size_t)s * n + v] - t;
-            if (e * e > e_best * e_best) { e_best = e; best = s; }
+            const float e = __fsub_rn(doses[(size_t)s * n + v], t);
+            const float q = __fmul_rn(e, e);
+            if (q > q_best) { e_best = e; best = s; q_best = q; }
         }
         for (int s = 0; s < n_sc; ++s) resid[(size_t)s * n + v] = (s == best) ? 2.0f * p * e_best : 0.0f;
         f += (double)p * (double)e_best * (double)e_best;
