@@ -88,6 +88,11 @@ typedef struct {
     const uint8_t *ap_open;     /* ny*nx, 1 = open */
     int32_t ap_nx, ap_ny;
     double ap_u0, ap_v0, ap_du, ap_dv;
+    /* the opening as the paper describes it ("the opening boundary ... polygon", crossing-number test,
+     * ref. 67).  ap_n_poly > 0: the opening is the closed polygon of these vertices (x0, y0, x1, y1, ...; beam frame, mm)
+     * and the bitmap is not used. */
+    int32_t ap_n_poly;
+    const double *ap_poly;
 } orc_beam;
 
 typedef struct {
@@ -408,6 +413,24 @@ static int drift_to_plane(ctx *c, hist *h, uint64_t hid, double wt)
     return ORC_CONT;
 }
 
+/* P:L87, ref. 67: crossing-number test -- a horizontal ray from (x, y) towards +x crosses the polygon's edges an odd number
+ * of times iff the point is inside.  Edge k joins vertex k to vertex k+1 (the last to the first); an edge counts when its
+ * end points lie on different sides of the ray's line (y1 > y differs from y2 > y) and it meets that line right of x. */
+static int point_in_polygon(const double *xy, int32_t n, double x, double y)
+{
+    int inside = 0;
+    for (int32_t k = 0; k < n; ++k) {
+        const double x1 = xy[2 * k], y1 = xy[2 * k + 1];
+        const double x2 = xy[2 * ((k + 1) % n)], y2 = xy[2 * ((k + 1) % n) + 1];
+        if ((y1 > y) != (y2 > y)) {
+            const double xi = x1 + (y - y1) * (x2 - x1) / (y2 - y1);
+            if (x < xi) inside = !inside;
+        }
+    }
+    return inside;
+}
+int orc_point_in_polygon(const double *xy, int32_t n, double x, double y) { return point_in_polygon(xy, n, x, y); }
+
 static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
 {
     const orc_problem *pb = c->pb;
@@ -471,7 +494,8 @@ static void run_history(ctx *c, uint64_t hid, const orc_beam *b, int32_t j)
             if (d < 0.0) d = 0.0;
             /* per-step test of the medium under the current (u,v) */
             int open = 0;
-            {
+            if (b->ap_n_poly > 0) open = point_in_polygon(b->ap_poly, b->ap_n_poly, h.r[0], h.r[1]);
+            else {
                 double fx = floor((h.r[0] - b->ap_u0) / b->ap_du), fy = floor((h.r[1] - b->ap_v0) / b->ap_dv);
                 if (fx >= 0.0 && fx < (double)b->ap_nx && fy >= 0.0 && fy < (double)b->ap_ny)
                     open = b->ap_open[(int64_t)fy * b->ap_nx + (int64_t)fx] != 0;

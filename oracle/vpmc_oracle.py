@@ -82,7 +82,8 @@ class _Beam(C.Structure):
                 ("rs_wet", C.c_double), ("rs_face", C.c_double), ("ap_present", C.c_int32),
                 ("ap_T", C.c_double), ("ap_face", C.c_double), ("ap_open", C.c_void_p),
                 ("ap_nx", C.c_int32), ("ap_ny", C.c_int32),
-                ("ap_u0", C.c_double), ("ap_v0", C.c_double), ("ap_du", C.c_double), ("ap_dv", C.c_double)]
+                ("ap_u0", C.c_double), ("ap_v0", C.c_double), ("ap_du", C.c_double), ("ap_dv", C.c_double),
+                ("ap_n_poly", C.c_int32), ("ap_poly", C.c_void_p)]
 
 
 class _Problem(C.Structure):
@@ -194,7 +195,12 @@ class Problem:
             arr[i].rs_face = float(b.get("rs_face", 190.0))
             ap = b.get("aperture")
             arr[i].ap_present = 0 if ap is None else 1
-            if ap is not None:
+            if ap is not None and ap.get("polygon") is not None:      # polygon opening, no bitmap
+                poly = _f64(ap["polygon"]).reshape(-1, 2)
+                keep.append(poly)
+                arr[i].ap_T, arr[i].ap_face = float(ap["T"]), float(ap.get("face", 150.0))
+                arr[i].ap_n_poly, arr[i].ap_poly = poly.shape[0], poly.ctypes.data
+            elif ap is not None:
                 op = np.ascontiguousarray(np.asarray(ap["open"], dtype=np.uint8))
                 keep.append(op)
                 arr[i].ap_T, arr[i].ap_face = float(ap["T"]), float(ap.get("face", 150.0))
@@ -257,6 +263,13 @@ def calib_eval(calib: dict, hu: float):
     out = (C.c_double * 3)()
     lib().orc_calib_eval(C.byref(cal), C.c_double(float(hu)), out)
     return tuple(out)
+
+
+def point_in_polygon(poly, x: float, y: float) -> bool:
+    """The oracle's crossing-number test (ref. 67) of point (x, y) against the closed polygon poly [n, 2]."""
+    p = _f64(poly).reshape(-1, 2)
+    lib().orc_point_in_polygon.restype = C.c_int
+    return bool(lib().orc_point_in_polygon(C.c_void_p(p.ctypes.data), C.c_int32(p.shape[0]), C.c_double(float(x)), C.c_double(float(y))))
 
 
 def spot_counts(pb: Problem, N: int) -> np.ndarray:

@@ -11,7 +11,8 @@ Problem format (dict):
   calib  = {hu, rsp, rho: fp32 node arrays ascending in hu, xsp: None}
   beams  = [{iso: (3,), rot: (3,3) with r_ct = iso + rot @ r_beam, spots: fp32 [n,5] = x, y, E, weight, sigma,
              rs_wet: mm (0 = none), rs_face: mm upstream of isocentre, aperture: None or
-             {T, face, open: uint8 [ny,nx], u0, v0, du, dv}}]
+             {T, face, open: uint8 [ny,nx], u0, v0, du, dv} (opening bitmap) or
+             {T, face, polygon: fp32 [n,2]} (the opening's boundary polygon, tested on the device: SURVEY.md 8(f)-2)}]
 """
 from __future__ import annotations
 
@@ -77,6 +78,11 @@ def beam(spots, iso, rot=None, rs_wet=0.0, rs_face=190.0, aperture=None):
 def aperture(open_u8, u0, v0, du, dv, T=30.0, face=150.0):
     return {"T": F(T), "face": F(face), "open": np.ascontiguousarray(open_u8, dtype=np.uint8),
             "u0": F(u0), "v0": F(v0), "du": F(du), "dv": F(dv)}
+
+
+def polygon_aperture(poly_xy, T=30.0, face=150.0):
+    """Aperture whose opening is the closed polygon poly_xy [n, 2] (beam frame, mm), exact fp32 vertices."""
+    return {"T": F(T), "face": F(face), "polygon": np.ascontiguousarray(np.asarray(poly_xy, dtype=F).reshape(-1, 2))}
 
 
 # ------------------------------------------------------------------------------------------ configs
@@ -271,9 +277,17 @@ def config4(hist_per_spot: int = 10_000, lo: int = 1800, hi: int = 2200, max_see
     raise RuntimeError("no seed gives %d..%d spots" % (lo, hi))
 
 
-def config5(seed: int = 5, n_histories: int = 100_000_000):
+def star_polygon(a, ph, n_vertices: int = 720):
+    """Config 5's irregular opening: r(phi) = 15 mm (1 + sum_{k=2..6} a_k cos(k phi + phi_k)); fp32 vertices."""
+    phi = np.linspace(0.0, 2 * np.pi, n_vertices, endpoint=False)
+    r = 15.0 * (1.0 + sum(a[i] * np.cos((i + 2) * phi + ph[i]) for i in range(5)))
+    return np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1).astype(F)
+
+
+def config5(seed: int = 5, n_histories: int = 100_000_000, polygon: bool = False):
     """BASELINE.json configs[4]: 512x512x200 voxels of 1 mm, random z-slabs (-1000..+1500 HU), 45 mm WET range shifter,
-    30 mm brass with a star-shaped opening (bitmap 1024^2 @ 0.1 mm), 65 layers 70..230 MeV, 5 mm lattice."""
+    30 mm brass with a star-shaped opening (bitmap 1024^2 @ 0.1 mm), 65 layers 70..230 MeV, 5 mm lattice.
+    polygon=True: the same opening handed over as its boundary polygon instead of the rasterised bitmap."""
     rng = np.random.default_rng(seed)
     n, h = (512, 512, 200), (1.0, 1.0, 1.0)
     hu = np.empty((n[2], n[1], n[0]), dtype=np.int16)
@@ -283,14 +297,15 @@ def config5(seed: int = 5, n_histories: int = 100_000_000):
         hu[z:z + t] = np.int16(rng.integers(-1000, 1501))
         z += t
     ct = {"n": n, "h": tuple(F(v) for v in h), "origin": (F(-256.0), F(-256.0), F(0.0)), "hu": hu}
-    a = rng.uniform(0.0, 0.12, size=5); ph = rng.uniform(0.0, 2 * np.pi, size=5)
-    phi = np.linspace(0.0, 2 * np.pi, 720, endpoint=False)
-    r = 15.0 * (1.0 + sum(a[i] * np.cos((i + 2) * phi + ph[i]) for i in range(5)))
-    poly = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=1)
-    op, u0, v0, du, dv = polygon_bitmap(1024, 0.1, poly)
-    half = np.ceil(np.abs(poly).max() / 5.0) * 5.0 + 5.0
+    poly = star_polygon(rng.uniform(0.0, 0.12, size=5), rng.uniform(0.0, 2 * np.pi, size=5))      # a_k in U[0, 0.12]
+    if polygon:
+        ap = polygon_aperture(poly, 30.0, 150.0)
+    else:
+        op, u0, v0, du, dv = polygon_bitmap(1024, 0.1, poly)
+        ap = aperture(op, u0, v0, du, dv, 30.0, 150.0)
+    half = np.ceil(np.abs(poly.astype(np.float64)).max() / 5.0) * 5.0 + 5.0
     g = np.arange(-half, half + 1e-9, 5.0)
     energies = 70.0 + 2.5 * np.arange(65)
     spots = [(x, y, E, 1.0, float(spot_sigma(E))) for E in energies for y in g for x in g]
-    b = beam(spots, iso=(0.0, 0.0, 100.0), rs_wet=45.0, rs_face=190.0, aperture=aperture(op, u0, v0, du, dv, 30.0, 150.0))
-    return {"name": "config5", "ct": ct, "calib": calibration(), "beams": [b], "n_histories": n_histories, "seed": seed}
+    b = beam(spots, iso=(0.0, 0.0, 100.0), rs_wet=45.0, rs_face=190.0, aperture=ap)
+    return {"name": "config5" + ("_polygon" if polygon else ""), "ct": ct, "calib": calibration(), "beams": [b], "n_histories": n_histories, "seed": seed}
