@@ -111,7 +111,10 @@ def pin_problem(w):
     for b in w["beams"]:
         b = dict(b); b["spots"] = pinned(b["spots"])
         if b.get("aperture") is not None:
-            b["aperture"] = dict(b["aperture"]); b["aperture"]["open"] = pinned(b["aperture"]["open"])
+            b["aperture"] = dict(b["aperture"])
+            for k in ("open", "polygon"):
+                if b["aperture"].get(k) is not None:
+                    b["aperture"][k] = pinned(b["aperture"][k])
         beams.append(b)
     w["beams"] = beams
     return w
@@ -135,6 +138,9 @@ def workload_plans(name, plans_arg=""):
     if name == "config5":
         return [("stress", "config5", {})], 100_000_000, \
             "BASELINE.json configs[4]: 512x512x200 @ 1 mm random-slab phantom, RS 45 mm + star-shaped aperture, 70-230 MeV"
+    if name == "config5_polygon":
+        return [("stress_polygon", "config5", {"polygon": True})], 100_000_000, \
+            "BASELINE.json configs[4] with the star-shaped opening given as its 720-vertex boundary polygon (crossing-number test on the device, SURVEY.md 8(f)-2)"
     raise SystemExit("unknown --workload %s" % name)
 
 
@@ -311,7 +317,7 @@ def measure_dose(workload, args, rank, local_rank, world, dev, steps, warmup, wi
     t_ms = dist.max_over_ranks(t_ms, world, dev)
     launches = sum(e.launch_count() for e in engines) - launches0
     hist_per_step = N * len(plans) * world
-    tm = {k: [0.0, 0] for k in ("beamline", "voxel", "scoring", "writer", "stage")}
+    tm = {k: [0.0, 0] for k in ("beamline", "voxel", "scoring", "writer", "stage", "optimiser")}
     steps_ct = steps_slab = 0
     finite = True
     for e, d in zip(engines, doses):
@@ -436,6 +442,10 @@ def run_b200(args):
             sub["config2"] = {k: r2[k] for k in ("workload", "value", "ms_per_step", "histories_per_plan", "plans_per_step", "e2e", "timing_ms_per_step", "gpu_launches")}
             sub["config2"]["e2e_over_value"] = r2["e2e"]["value"] / r2["value"]
             sub["config2"]["roofline"] = k2
+        if args.workload != "config5_polygon":
+            rp = measure_dose("config5_polygon", args, 0, local_rank, 1, dev, 2, 2, with_e2e=False)
+            sub["config5_polygon"] = {k: rp[k] for k in ("workload", "value", "ms_per_step", "histories_per_plan", "timing_ms_per_step", "gpu_launches")}
+            sub["config5_polygon"]["relative_to_bitmap"] = rp["value"] / rec["value"] if args.workload == "config5" else None
         sub["config3"] = measure_to_uncertainty(CONFIG3_SEEDS)
         sub["config4"] = measure_influence(10_000, 1, 1)
         sub["config4"]["roofline_voxel_box"] = None

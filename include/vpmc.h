@@ -183,6 +183,16 @@ int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *sc, uint64_t batch_
 /* Result of the last vpmc_dose_to_uncertainty: batches run, the estimate after the last one, whether the target stopped it. */
 int vpmc_get_run_info(vpmc_t *h, int32_t *batches_out, float *rel_unc_out, int32_t *reached_target_out);
 
+/* S:8f-2: aperture block whose opening is given as its boundary polygon, as the paper describes it (the medium is
+ * decided at every MC step by the crossing-number test of the proton's lateral position against the opening's polygon,
+ * ref. 67; P:L61 on why a voxelised opening is too coarse for small apertures).  vertices_xy: [host], n_vertices pairs
+ * (x, y) in the beam frame, mm; edge k joins vertex k to vertex k + 1, the last to the first; either orientation; a point is
+ * in the opening iff a ray towards +x crosses an odd number of edges.  Everything outside the polygon is brass.  Replaces
+ * any opening set before on this beam.  The test runs on the device for every aperture step (tests whose answer is known
+ * from the distance to the nearest edge are skipped, D:5.2). */
+int vpmc_set_aperture_polygon(vpmc_t *h, int beam, float thickness_mm, int material, const float *vertices_xy, int32_t n_vertices,
+                              float downstream_face_mm);
+
 /* Test-only: the device tables S0 builds from an opening bitmap (D:5.2).  dims_out[4] = {words per row, rows, tiles in u,
  * tiles in v}; bits_out_host: rows x words packed bitmap (bit ix & 31 of word ix >> 5); dist_out_host: 2 maps of tiles_v x
  * tiles_u bytes -- Chebyshev distance in tiles (capped at 255) to the nearest tile that is not fully open, with everything

@@ -23,7 +23,7 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
            "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats", "vpmc_spmv_dose", "vpmc_spmv_grad",
-           "vpmc_worst_case", "vpmc_robust_iteration"]
+           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
@@ -150,6 +150,7 @@ def lib():
         L.vpmc_worst_case.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vpmc_robust_iteration.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.vpmc_set_aperture_polygon.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_int, C.c_void_p, C.c_int32, C.c_float]
         L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -237,7 +238,12 @@ class Engine:
         if float(b.get("rs_wet", 0.0)) > 0:
             self._check(L.vpmc_set_range_shifter(self._h, bid.value, float(b["rs_wet"]), float(b.get("rs_face", 190.0))))
         ap = b.get("aperture")
-        if ap is not None:
+        if ap is not None and ap.get("polygon") is not None:
+            poly = _f32(ap["polygon"]).reshape(-1, 2)
+            self._check(L.vpmc_set_aperture_polygon(self._h, bid.value, float(ap["T"]), BRASS, poly.ctypes.data, poly.shape[0],
+                                                    float(ap.get("face", 150.0))))
+            self.h2d_bytes += poly.nbytes
+        elif ap is not None:
             op = np.ascontiguousarray(np.asarray(ap["open"], dtype=np.uint8))
             self._check(L.vpmc_set_aperture(self._h, bid.value, float(ap["T"]), BRASS, op.ctypes.data, op.shape[1],
                                             op.shape[0], float(ap["u0"]), float(ap["v0"]), float(ap["du"]),

@@ -172,8 +172,8 @@ static double pl_eval(const vpmc_calib *c, const float *y, double hu)
 
 static void free_beam(vpmc_t *h, BeamHost &b)
 {
-    dev_release(h, b.d_bits); dev_release(h, b.d_dist); dev_release(h, b.d_ap_tmp);
-    b.d_bits = nullptr; b.d_dist = nullptr; b.d_ap_tmp = nullptr;
+    dev_release(h, b.d_bits); dev_release(h, b.d_dist); dev_release(h, b.d_ap_tmp); dev_release(h, b.d_poly); dev_release(h, b.d_pgrid); dev_release(h, b.d_prows);
+    b.d_bits = nullptr; b.d_dist = nullptr; b.d_ap_tmp = nullptr; b.d_poly = nullptr; b.d_pgrid = nullptr; b.d_prows = nullptr; b.ap_n_poly = 0;
 }
 
 extern "C" int vpmc_destroy(vpmc_t *h)
@@ -413,11 +413,65 @@ extern "C" int vpmc_set_aperture(vpmc_t *h, int beam, float thickness_mm, int ma
     return VPMC_OK;
 }
 
+extern "C" int vpmc_set_aperture_polygon(vpmc_t *h, int beam, float thickness_mm, int material, const float *vertices_xy, int32_t n_vertices,
+                                         float downstream_face_mm)
+{
+    int rc = check_beam(h, beam); if (rc) return rc;
+    BeamHost &b = h->beams[beam];
+    if (!(thickness_mm > 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "thickness must be positive (use vpmc_set_aperture with 0 to remove the block)");
+    if (material != VPMC_BRASS) FAIL(h, VPMC_ERR_INVALID_ARG, "only VPMC_BRASS is supported");
+    if (!vertices_xy || n_vertices < 3 || n_vertices > (1 << 20)) FAIL(h, VPMC_ERR_INVALID_ARG, "a polygon needs 3 .. 2^20 vertices");
+    float lo[2] = { vertices_xy[0], vertices_xy[1] }, hi[2] = { vertices_xy[0], vertices_xy[1] };
+    for (int k = 0; k < n_vertices; ++k)
+        for (int a = 0; a < 2; ++a) {
+            const float v = vertices_xy[2 * k + a];
+            if (!std::isfinite(v)) FAIL(h, VPMC_ERR_INVALID_ARG, "vertex %d is not finite", k);
+            lo[a] = std::min(lo[a], v); hi[a] = std::max(hi[a], v);
+        }
+    const float ext = std::max(hi[0] - lo[0], hi[1] - lo[1]);
+    if (!(ext > 0)) FAIL(h, VPMC_ERR_INVALID_ARG, "degenerate polygon");
+    // coarse grid: ~96 cells across the larger extent, one cell of margin all round
+    const float cell = ext / 96.0f;
+    const int nx = (int)std::ceil((hi[0] - lo[0]) / cell) + 2, ny = (int)std::ceil((hi[1] - lo[1]) / cell) + 2;
+    // per grid row: the edges whose y-range meets the row, widened by a margin that covers the rounding of the row lookup
+    const float x0 = lo[0] - cell, y0 = lo[1] - cell, margin = 1e-3f * cell + 1e-4f;
+    std::vector<int> rows((size_t)ny + 1, 0), edges;
+    {
+        std::vector<std::vector<int>> lists((size_t)ny);
+        for (int k = 0; k < n_vertices; ++k) {
+            const float ya = vertices_xy[2 * k + 1], yb = vertices_xy[2 * ((k + 1) % n_vertices) + 1];
+            const int r0 = std::max((int)std::floor((std::min(ya, yb) - margin - y0) / cell), 0);
+            const int r1 = std::min((int)std::floor((std::max(ya, yb) + margin - y0) / cell), ny - 1);
+            for (int r = r0; r <= r1; ++r) lists[r].push_back(k);
+        }
+        for (int r = 0; r < ny; ++r) { rows[r + 1] = rows[r] + (int)lists[r].size(); edges.insert(edges.end(), lists[r].begin(), lists[r].end()); }
+    }
+    rows.insert(rows.end(), edges.begin(), edges.end());
+    free_beam(h, b);
+    if ((rc = dev_alloc(h, (void **)&b.d_poly, (size_t)n_vertices * sizeof(float2))) || (rc = dev_alloc(h, (void **)&b.d_pgrid, (size_t)nx * ny * sizeof(float))) ||
+        (rc = dev_alloc(h, (void **)&b.d_prows, rows.size() * sizeof(int)))) return rc;
+    cudaStream_t ss = h->setup_stream;
+    CU(h, cudaMemcpyAsync(b.d_poly, vertices_xy, (size_t)n_vertices * sizeof(float2), cudaMemcpyHostToDevice, ss));
+    CU(h, cudaMemcpyAsync(b.d_prows, rows.data(), rows.size() * sizeof(int), cudaMemcpyHostToDevice, ss));
+    CU(h, cudaEventRecord(h->copy_ev, ss));
+    b.pg_nx = nx; b.pg_ny = ny; b.pg_cell = cell; b.pg_x0 = x0; b.pg_y0 = y0;
+    polygon_grid_kernel<<<(nx * ny + 127) / 128, 128, 0, ss>>>(b.d_poly, n_vertices, nx, ny, b.pg_x0, b.pg_y0, cell, b.d_pgrid);
+    CU(h, cudaGetLastError());
+    h->launches += 1;
+    h->setup_pending = true;
+    b.ap_n_poly = n_vertices;
+    b.has_ap = true; b.ap_T = thickness_mm; b.ap_face = downstream_face_mm > 0 ? downstream_face_mm : 150.0f;
+    b.ap_nx = b.ap_ny = 0; b.ap_row_words = 0; b.ap_ntx = b.ap_nty = 0;
+    h->spots_dirty = true;
+    CU(h, cudaEventSynchronize(h->copy_ev));       // the caller's vertices are copied during the call
+    return VPMC_OK;
+}
+
 extern "C" int vpmc_get_aperture_tables(vpmc_t *h, int beam, uint32_t *bits_out_host, uint8_t *dist_out_host, int32_t *dims_out)
 {
     int rc = check_beam(h, beam); if (rc) return rc;
     const BeamHost &b = h->beams[beam];
-    if (!b.has_ap) FAIL(h, VPMC_ERR_STATE, "beam %d has no aperture", beam);
+    if (!b.has_ap || b.ap_n_poly > 0) FAIL(h, VPMC_ERR_STATE, "beam %d has no bitmap aperture", beam);
     if (dims_out) { dims_out[0] = b.ap_row_words; dims_out[1] = b.ap_ny; dims_out[2] = b.ap_ntx; dims_out[3] = b.ap_nty; }
     CU(h, cudaStreamSynchronize(h->setup_stream));
     if (bits_out_host) CU(h, cudaMemcpy(bits_out_host, b.d_bits, (size_t)b.ap_row_words * b.ap_ny * sizeof(uint32_t), cudaMemcpyDeviceToHost));

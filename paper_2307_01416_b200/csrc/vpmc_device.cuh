@@ -60,6 +60,18 @@ struct DevBeam {
     const unsigned char *ap_dist_open;
     int ap_ntx;
     float ap_tile_u, ap_tile_v;   // tile size in mm
+    // S:8f-2: polygon opening (ap_n_poly > 0; no bitmap then).  Vertices (x, y), and a coarse grid over the polygon's bounding
+    // box: per cell 0 = the boundary may pass through it (exact test needed), > 0 = wholly inside the opening, < 0 = wholly
+    // in brass, |value| = a radius in the L-infinity norm (mm) around ANY point of the cell in which the answer cannot change
+    const float2 *ap_poly;
+    int ap_n_poly;
+    const float *ap_pgrid;
+    int ap_pg_nx, ap_pg_ny;
+    float ap_pg_x0, ap_pg_y0, ap_pg_inv_cell;
+    // per grid row, the edges whose y-range meets the row (+ a rounding margin): the only ones a ray along +x from a point of
+    // that row can cross.  ap_prow_ptr [ny + 1], ap_pedges = edge indices (edge k = vertex k -> vertex k + 1)
+    const int *ap_prow_ptr;
+    const int *ap_pedges;
 };
 
 #ifndef VPK_AP_TILE_SHIFT

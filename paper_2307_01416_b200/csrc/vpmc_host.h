@@ -22,6 +22,13 @@ struct BeamHost {
     unsigned char *d_dist = nullptr;  // safe-distance maps of the opening, one byte per tile of 2^kApTileShift pixels: to brass, then to the opening
     unsigned char *d_ap_tmp = nullptr;    // set-up scratch: the caller's uint8 bitmap, tile flags, column distances
     int ap_ntx = 0, ap_nty = 0;
+    // polygon opening (vpmc_set_aperture_polygon)
+    int ap_n_poly = 0;
+    float2 *d_poly = nullptr;
+    float *d_pgrid = nullptr;
+    int *d_prows = nullptr;           // row_ptr [pg_ny + 1] followed by the edge lists
+    int pg_nx = 0, pg_ny = 0;
+    float pg_x0 = 0, pg_y0 = 0, pg_cell = 1;
 };
 
 // a device buffer that only grows

@@ -503,6 +503,24 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
     flush_warp_tallies(wt_all + warp, lc, tal, lane);
 }
 
+// S0 for polygon openings (S:8f-2): classify the cells of the coarse grid over the polygon's bounding box.  Every point of a
+// cell lies within half a diagonal of its centre, so when the centre is farther than that from the boundary the whole cell
+// is on the centre's side, and around ANY point of the cell the answer holds within d - half_diag (Euclidean), i.e. within
+// (d - half_diag) / sqrt(2) in the L-infinity norm the step loop measures its lateral travel in.
+__global__ void polygon_grid_kernel(const float2 *__restrict__ poly, int n, int nx, int ny, float x0, float y0, float cell, float *__restrict__ grid)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nx * ny) return;
+    const int iy = t / nx, ix = t - iy * nx;
+    float d2;
+    const bool in = polygon_query(poly, n, fmaf((float)ix + 0.5f, cell, x0), fmaf((float)iy + 0.5f, cell, y0), d2);
+    const float d = sqrtf(d2);
+    const float half_diag = 0.70711f * cell * 1.01f + 1e-4f;        // + the rounding of the cell lookup
+    float v = 0.0f;
+    if (d > half_diag) { const float r = fmaxf(0.7f * (d - half_diag), 1e-6f); v = in ? r : -r; }
+    grid[t] = v;
+}
+
 // ------------------------------------------------------------------------------------------- trace (test-only)
 // one thread per selected history, from the source to its end through the SAME step functions as the production kernels;
 // records (RecTracer) or a digest (DigestTracer) per history

@@ -86,6 +86,9 @@ static int prepare_beams(vpmc_t *h, const vpmc_scenario &sc, cudaStream_t st)
         d.ap_u0 = b.ap_u0; d.ap_v0 = b.ap_v0; d.ap_inv_du = (float)(1.0 / (double)b.ap_du); d.ap_inv_dv = (float)(1.0 / (double)b.ap_dv);
         d.ap_dist = b.d_dist; d.ap_dist_open = b.d_dist ? b.d_dist + (size_t)b.ap_ntx * b.ap_nty : nullptr; d.ap_ntx = b.ap_ntx;
         d.ap_tile_u = (float)(1 << kApTileShift) * b.ap_du; d.ap_tile_v = (float)(1 << kApTileShift) * b.ap_dv;
+        d.ap_poly = b.d_poly; d.ap_n_poly = b.ap_n_poly; d.ap_pgrid = b.d_pgrid; d.ap_pg_nx = b.pg_nx; d.ap_pg_ny = b.pg_ny;
+        d.ap_pg_x0 = b.pg_x0; d.ap_pg_y0 = b.pg_y0; d.ap_pg_inv_cell = (float)(1.0 / (double)b.pg_cell);
+        d.ap_prow_ptr = b.d_prows; d.ap_pedges = b.d_prows ? b.d_prows + b.pg_ny + 1 : nullptr;
         const double wct = ct_min_w(h, b, sc.shift);
         if (d.has_rs && d.has_ap && d.w_rs_out > d.w_ap_in) FAIL(h, VPMC_ERR_GEOMETRY, "beam %zu: range shifter is not upstream of the aperture", i);
         const double w_last = d.has_ap ? d.w_ap_out : (d.has_rs ? d.w_rs_out : -std::numeric_limits<double>::infinity());

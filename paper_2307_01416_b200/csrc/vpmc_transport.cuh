@@ -154,6 +154,100 @@ __device__ __forceinline__ bool aperture_open(const DevBeam *b, float x, float y
     return (wv >> (ix & 31)) & 1u;
 }
 
+// S:8f-2 (ref. 67): crossing-number test of (x, y) against the closed polygon, edge k = vertex k -> vertex k + 1 --
+// an edge counts when its end points lie on different sides of the line through y and it meets that line right of x -- and,
+// in the same pass, the squared distance to the nearest edge.  Kept out of line: it is called once or twice per history and
+// must not cost the step loops their registers.
+__device__ __noinline__ bool polygon_query(const float2 *__restrict__ poly, int n, float x, float y, float &dist2)
+{
+    bool inside = false;
+    float d2 = 1e30f;
+    float2 a = __ldg(poly + n - 1);
+    for (int k = 0; k < n; ++k) {
+        const float2 b = __ldg(poly + k);
+        const float ex = b.x - a.x, ey = b.y - a.y, px = x - a.x, py = y - a.y;
+        if ((a.y > y) != (b.y > y)) {
+            const float xi = a.x + __fdiv_rn(py * ex, ey);
+            if (x < xi) inside = !inside;
+        }
+        const float l2 = fmaf(ex, ex, ey * ey);
+        const float t = (l2 > 0.0f) ? fminf(fmaxf(__fdiv_rn(fmaf(px, ex, py * ey), l2), 0.0f), 1.0f) : 0.0f;
+        const float dx = fmaf(-t, ex, px), dy = fmaf(-t, ey, py);
+        d2 = fminf(d2, fmaf(dx, dx, dy * dy));
+        a = b;
+    }
+    dist2 = d2;
+    return inside;
+}
+
+// The same test for a point of grid row `row`, over the edges that can matter there: the crossing count over the row's own
+// edge list (an edge outside it has both end points on one side of the ray's line: the full loop would skip it too, so the
+// answer is the full loop's), the distance over the lists of the rows row - 1 .. row + 1 -- any other edge is at least one
+// cell away, so the distance is capped at one cell.
+__device__ __noinline__ bool polygon_query_row(const DevBeam *bp, int row, float x, float y, float &dist2)
+{
+    const float2 *__restrict__ poly = bp->ap_poly;
+    const int *__restrict__ rp = bp->ap_prow_ptr, *__restrict__ ed = bp->ap_pedges;
+    const int n = __ldg(&bp->ap_n_poly), ny = __ldg(&bp->ap_pg_ny);
+    const float cell = __frcp_rn(__ldg(&bp->ap_pg_inv_cell));
+    bool inside = false;
+    float d2 = cell * cell;
+    for (int r = max(row - 1, 0); r <= min(row + 1, ny - 1); ++r)
+        for (int i = __ldg(rp + r); i < __ldg(rp + r + 1); ++i) {
+            const int k = __ldg(ed + i);
+            const float2 a = __ldg(poly + k), b = __ldg(poly + (k + 1 == n ? 0 : k + 1));
+            const float ex = b.x - a.x, ey = b.y - a.y, px = x - a.x, py = y - a.y;
+            if (r == row && (a.y > y) != (b.y > y)) {
+                const float xi = a.x + __fdiv_rn(py * ex, ey);
+                if (x < xi) inside = !inside;
+            }
+            const float l2 = fmaf(ex, ex, ey * ey);
+            const float t = (l2 > 0.0f) ? fminf(fmaxf(__fdividef(fmaf(px, ex, py * ey), l2), 0.0f), 1.0f) : 0.0f;
+            const float dx = fmaf(-t, ex, px), dy = fmaf(-t, ey, py);
+            d2 = fminf(d2, fmaf(dx, dx, dy * dy));
+        }
+    dist2 = d2;
+    return inside;
+}
+
+// The medium under (x, y) of either kind of opening, with the lateral travel (L-infinity norm, mm, per axis) over which the
+// answer is KNOWN not to change -- 0 when nothing is known (the per-step test of P:L87 is kept in outcome,
+// tests whose answer is known are not executed).
+__device__ __forceinline__ bool aperture_query(const DevBeam *bp, float x, float y, float &safe_u, float &safe_v)
+{
+    if (__ldg(&bp->ap_n_poly) > 0) {
+        const float gx = (x - __ldg(&bp->ap_pg_x0)) * __ldg(&bp->ap_pg_inv_cell), gy = (y - __ldg(&bp->ap_pg_y0)) * __ldg(&bp->ap_pg_inv_cell);
+        const int nx = __ldg(&bp->ap_pg_nx), ny = __ldg(&bp->ap_pg_ny);
+        if (!(gx >= 0.0f && gx < (float)nx && gy >= 0.0f && gy < (float)ny)) {
+            // outside the grid (which covers the polygon's bounding box): brass at least up to the grid's rectangle
+            const float cell = __frcp_rn(__ldg(&bp->ap_pg_inv_cell));
+            const float d = fmaxf(fmaxf(-gx, gx - (float)nx), fmaxf(-gy, gy - (float)ny)) * cell;
+            safe_u = safe_v = 0.99f * fmaxf(d, 0.0f);
+            return false;
+        }
+        const float cv = __ldg(bp->ap_pgrid + (size_t)(int)gy * nx + (int)gx);
+        if (cv != 0.0f) { safe_u = safe_v = fabsf(cv); return cv > 0.0f; }
+        float d2;
+        const bool in = polygon_query_row(bp, (int)gy, x, y, d2);
+        safe_u = safe_v = 0.7f * sqrt_fast(d2);          // Euclidean radius d -> L-infinity radius d / sqrt(2), rounded down
+        return in;
+    }
+    int ix, iy;
+    const bool open = aperture_open(bp, x, y, ix, iy);
+    if (ix < 0) {        // outside the bitmap: brass up to its rectangle
+        const float u0 = __ldg(&bp->ap_u0), v0 = __ldg(&bp->ap_v0);
+        const float u1 = u0 + (float)__ldg(&bp->ap_nx) * __frcp_rn(__ldg(&bp->ap_inv_du)), v1 = v0 + (float)__ldg(&bp->ap_ny) * __frcp_rn(__ldg(&bp->ap_inv_dv));
+        safe_u = safe_v = 0.99f * fmaxf(fmaxf(u0 - x, x - u1), fmaxf(v0 - y, y - v1));
+        return false;
+    }
+    // k tiles to the nearest tile of the other kind -> (k - 1) tiles of lateral travel are safe
+    const unsigned char *map = open ? bp->ap_dist : bp->ap_dist_open;
+    const int k = (int)__ldg(map + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
+    const float safe = (k >= 2) ? 0.99f * (float)(k - 1) : 0.0f;
+    safe_u = safe * __ldg(&bp->ap_tile_u); safe_v = safe * __ldg(&bp->ap_tile_v);
+    return open;
+}
+
 // Beam frame -> CT frame (setup shift moves the patient), ray-box entry, entry voxel (C3).  Done in fp64: it runs
 // once per history and fixes the entry point that every later face crossing inherits.  On return the geometry
 // slots hold ix, iy, iz, v and rx, ry, rz are LOCAL offsets inside that voxel.
@@ -361,19 +455,9 @@ __device__ __forceinline__ int ap_open_phase(const Ctx &c, const DevBeam *bp, Hi
     const DevParams &P = c.P;
     const float T = g.T, w_in = g.w_in;
     for (;;) {
-        int ix, iy;
-        if (!aperture_open(bp, beam_xh(h), beam_yh(h), ix, iy)) {
-            // brass: how far is the opening?  (k tiles away -> at least (k - 1) tiles of lateral travel are brass)
-            float budget;
-            if (ix >= 0) {
-                const int k = (int)__ldg(bp->ap_dist_open + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
-                budget = 0.99f * (float)(k - 1) * fminf(__ldg(&bp->ap_tile_u), __ldg(&bp->ap_tile_v));
-            } else {      // outside the bitmap: distance to its rectangle
-                const float x = beam_xh(h), y = beam_yh(h), u0 = __ldg(&bp->ap_u0), v0 = __ldg(&bp->ap_v0);
-                const float u1 = u0 + (float)__ldg(&bp->ap_nx) * __frcp_rn(__ldg(&bp->ap_inv_du)), v1 = v0 + (float)__ldg(&bp->ap_ny) * __frcp_rn(__ldg(&bp->ap_inv_dv));
-                budget = 0.99f * fmaxf(fmaxf(u0 - x, x - u1), fmaxf(v0 - y, y - v1));
-            }
-            h.rx = fmaxf(budget, 1e-30f);          // > 0: the step that follows this test IS a brass step
+        float safe_u, safe_v;
+        if (!aperture_query(bp, beam_xh(h), beam_yh(h), safe_u, safe_v)) {
+            h.rx = fmaxf(fminf(safe_u, safe_v), 1e-30f);          // > 0: the step that follows this test IS a brass step
             return BEAM_CONT;
         }
         // nf = full steps left before the exit step; if all of their tests are known, go straight to the exit plane, else
@@ -387,14 +471,10 @@ __device__ __forceinline__ int ap_open_phase(const Ctx &c, const DevBeam *bp, Hi
             else if (nf > 0 && fmaf(-(float)(nf - 1), duz, rem) <= duz) nf -= 1;
         }
         float n_safe = 0.0f;
-        if (nf > 0) {
-            const int k = (int)__ldg(bp->ap_dist + (size_t)(iy >> kApTileShift) * __ldg(&bp->ap_ntx) + (ix >> kApTileShift));
-            if (k >= 2) {
-                const float safe = 0.99f * (float)(k - 1);
-                const float nu = __fdividef(safe * __ldg(&bp->ap_tile_u), fmaxf(fabsf(P.s_ap * h.ux), 1e-12f));
-                const float nv = __fdividef(safe * __ldg(&bp->ap_tile_v), fmaxf(fabsf(P.s_ap * h.uy), 1e-12f));
-                n_safe = floorf(fminf(fminf(nu, nv), 65536.0f));
-            }
+        if (nf > 0 && safe_u > 0.0f && safe_v > 0.0f) {
+            const float nu = __fdividef(safe_u, fmaxf(fabsf(P.s_ap * h.ux), 1e-12f));
+            const float nv = __fdividef(safe_v, fmaxf(fabsf(P.s_ap * h.uy), 1e-12f));
+            n_safe = floorf(fminf(fminf(nu, nv), 65536.0f));
         }
         const bool whole = n_safe >= (float)nf;            // includes the plain exit step (nf = 0)
         const int n = whole ? nf : max((int)n_safe, 1);    // full steps taken now

@@ -94,6 +94,17 @@ def oracle_columns_parallel(fn, kw, nvox, spots, hps, seed, sc=None):
     return [_merge(res[j * per:(j + 1) * per], nvox)[0] for j in range(len(spots))]
 
 
+def polygon_edge_distance(poly, x, y):
+    """Euclidean distance of (x, y) to the boundary of the closed polygon poly [n, 2] (numpy, fp64)."""
+    p = np.asarray(poly, dtype=np.float64).reshape(-1, 2)
+    q = np.roll(p, -1, axis=0)
+    e = q - p
+    l2 = np.maximum((e * e).sum(axis=1), 1e-300)
+    t = np.clip(((np.array([x, y]) - p) * e).sum(axis=1) / l2, 0.0, 1.0)
+    d = p + t[:, None] * e - np.array([x, y])
+    return float(np.sqrt((d * d).sum(axis=1).min()))
+
+
 def deciding_gap(O, w, P, kind, beam, E, E0, r, u, ivox, tau_after, tau_star, extent):
     """the smallest relative gap of the discrete decisions of one step (kind 'ct' | 'rs' | 'ap'),
     evaluated in the ORACLE's pre-step state: how far, relative to the fixed scales (grid extent, R0, 1), the state is
@@ -128,7 +139,9 @@ def deciding_gap(O, w, P, kind, beam, E, E0, r, u, ivox, tau_after, tau_star, ex
         gaps += [abs(dist - d0) * abs(u[2]) / extent, abs(u[2])]
         rsp = P.rs_rsp if rs else P.brass_rsp
         gaps.append(abs(min(d0, dist) - max(P.f_R * R, P.R_cut) / rsp) * rsp / P.f_R / R0)
-        if not rs:
+        if not rs and b["aperture"].get("polygon") is not None:      # polygon opening: distance to the nearest edge
+            gaps.append(polygon_edge_distance(b["aperture"]["polygon"], r[0], r[1]) / extent)
+        elif not rs:
             ap = b["aperture"]
             for x, x0, dx in ((r[0], float(ap["u0"]), float(ap["du"])), (r[1], float(ap["v0"]), float(ap["dv"]))):
                 f = (x - x0) / dx

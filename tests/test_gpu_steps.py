@@ -50,11 +50,19 @@ def star_case():
     return w
 
 
+def star_polygon_case():
+    """The same with the opening handed over as its boundary polygon: crossing-number test on the device."""
+    w = star_case()
+    w["beams"][0]["aperture"] = wl.config5(polygon=True)["beams"][0]["aperture"]
+    w["name"] = "star_polygon"
+    return w
+
+
 def config3_case():
     return wl.config3(3)
 
 
-STEP_CASES = dict(CASES, star=star_case, config3=config3_case)
+STEP_CASES = dict(CASES, star=star_case, star_polygon=star_polygon_case, config3=config3_case)
 
 
 def spot_beams(w):
