@@ -257,6 +257,15 @@ int vpmc_robust_iteration(vpmc_t *h, const vpmc_csr *mats, int32_t n_sc, int64_t
                           const float *weight_dev, float *doses_ws_dev, float *resid_ws_dev, float *grad_dev, double *objective_dev,
                           void *cuda_stream);
 
+/* S:8f-3: 3-D gamma index of two dose grids on this engine's CT grid ("3D Gamma passing rate", Table 2; ref. 80),
+ * computed on the device.  S:8c-C6: global normalisation -- dose criterion dd_rel x max(ref); voxels with ref >= threshold_rel
+ * x max(ref) are evaluated; a voxel passes if |eval - ref| <= criterion at zero distance, else if min over the lattice points
+ * of spacing h / sub within dta_mm of (distance / dta)^2 + ((eval interpolated trilinearly, edge values beyond the grid) - ref)^2
+ * / criterion^2 is <= 1.  ref_dev, eval_dev: [device] nx*ny*nz floats.  *n_eval_out, *n_fail_out [host]: voxels evaluated, voxels
+ * failing; pass rate = 1 - n_fail / n_eval.  Synchronises cuda_stream. */
+int vpmc_gamma(vpmc_t *h, const float *ref_dev, const float *eval_dev, float dd_rel, float dta_mm, float threshold_rel, int32_t sub,
+               uint64_t *n_eval_out, uint64_t *n_fail_out, void *cuda_stream);
+
 /* Upper bound in bytes on the per-group scratch of vpmc_influence (the dense per-column boxes of one group of spots);
  * 0 = automatic (a third of the free device memory, at most 24 GiB).  Smaller limits only mean more groups. */
 int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes);

@@ -428,11 +428,10 @@ def dose_to_uncertainty(pb: Problem, batch_histories: int, target: float, seed: 
     return np.mean(np.array(batches), axis=0), len(batches), history
 
 
-def gamma_pass_rate(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: float = 1.0, thr: float = 0.1,
-                    sub: int = 10) -> float:
+def gamma_counts(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: float = 1.0, thr: float = 0.1, sub: int = 10):
     """C6 / P:L107: global 3D gamma.  ref, ev: [nz, ny, nx]; h = (hx, hy, hz) mm; dd relative to the reference
     maximum; voxels with ref >= thr*max evaluated; pass iff gamma <= 1.  Zero-distance test first, full search
-    with trilinear sub-sampling at h/sub only for voxels failing it."""
+    with trilinear sub-sampling at h/sub only for voxels failing it.  Returns (voxels evaluated, voxels failing)."""
     from scipy.ndimage import map_coordinates
     ref = np.asarray(ref, dtype=np.float64)
     ev = np.asarray(ev, dtype=np.float64)
@@ -441,11 +440,11 @@ def gamma_pass_rate(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: f
     sel = ref >= thr * mx
     n_eval = int(sel.sum())
     if n_eval == 0:
-        return 1.0
+        return 0, 0
     fail = sel & (np.abs(ev - ref) > dcrit)
     idx = np.argwhere(fail)
     if idx.size == 0:
-        return 1.0
+        return n_eval, 0
     hz, hy, hx = float(h[2]), float(h[1]), float(h[0])
     rng = [np.arange(-int(np.ceil(dta / s * sub)), int(np.ceil(dta / s * sub)) + 1) / sub for s in (hz, hy, hx)]
     oz, oy, ox = np.meshgrid(*rng, indexing="ij")
@@ -458,4 +457,11 @@ def gamma_pass_rate(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: f
         g2 = dist2 + ((vals - ref[z, y, x]) / dcrit) ** 2
         if g2.min() > 1.0:
             n_fail += 1
-    return 1.0 - n_fail / n_eval
+    return n_eval, n_fail
+
+
+def gamma_pass_rate(ref: np.ndarray, ev: np.ndarray, h, dd: float = 0.01, dta: float = 1.0, thr: float = 0.1,
+                    sub: int = 10) -> float:
+    """Pass rate 1 - failing / evaluated of gamma_counts (1.0 when no voxel is evaluated)."""
+    n_eval, n_fail = gamma_counts(ref, ev, h, dd, dta, thr, sub)
+    return 1.0 if n_eval == 0 else 1.0 - n_fail / n_eval

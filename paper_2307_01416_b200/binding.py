@@ -23,7 +23,7 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
            "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats", "vpmc_spmv_dose", "vpmc_spmv_grad",
-           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon"]
+           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon", "vpmc_gamma"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
@@ -151,6 +151,8 @@ def lib():
         L.vpmc_robust_iteration.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vpmc_set_aperture_polygon.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_int, C.c_void_p, C.c_int32, C.c_float]
+        L.vpmc_gamma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int32, C.POINTER(C.c_uint64),
+                                 C.POINTER(C.c_uint64), C.c_void_p]
         L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -423,6 +425,17 @@ class Engine:
         self._check(lib().vpmc_robust_iteration(self._h, arr, n_sc, n, w.data_ptr(), target.data_ptr(), weight.data_ptr(), doses.data_ptr(),
                                                 resid.data_ptr(), grad.data_ptr(), obj.data_ptr(), st.cuda_stream))
         return obj, grad, doses
+
+    def gamma(self, ref, ev, dd: float = 0.01, dta: float = 1.0, thr: float = 0.1, sub: int = 10, stream=None):
+        """3-D gamma of two dose tensors on this engine's grid (vpmc_gamma): (pass rate, voxels evaluated, voxels failing)."""
+        import torch
+        for t in (ref, ev):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.nvox
+        st = torch.cuda.current_stream() if stream is None else stream
+        ne, nf = C.c_uint64(), C.c_uint64()
+        self._check(lib().vpmc_gamma(self._h, ref.data_ptr(), ev.data_ptr(), float(dd), float(dta), float(thr), int(sub), C.byref(ne),
+                                     C.byref(nf), st.cuda_stream))
+        return (1.0 - nf.value / ne.value) if ne.value else 1.0, int(ne.value), int(nf.value)
 
     def influence_stats(self) -> dict:
         st = InfluenceStats()

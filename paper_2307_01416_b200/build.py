@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvpmc.so")
 SOURCES = ["vpmc_api.cu"]
 DEPS = ["vpmc_api.cu", "vpmc_run.inl", "vpmc_influence.inl", "vpmc_host.h", "vpmc_kernels.cuh", "vpmc_transport.cuh",
-        "vpmc_device.cuh", "vpmc_setup.cuh", "vpmc_spmv.cuh", "vpmc_spmv.inl", "../../include/vpmc.h"]
+        "vpmc_device.cuh", "vpmc_setup.cuh", "vpmc_spmv.cuh", "vpmc_spmv.inl", "vpmc_gamma.cuh", "../../include/vpmc.h"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -197,7 +197,7 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
-                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part };
+                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part, &h->gamma_buf };
     for (DevBuf *b : bufs) if (b->p) { pool_give(b->p, b->bytes); b->p = nullptr; }
     delete h;
     return VPMC_OK;

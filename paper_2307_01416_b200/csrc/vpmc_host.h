@@ -9,6 +9,7 @@
 #include "../../include/vpmc.h"
 #include "vpmc_kernels.cuh"
 #include "vpmc_spmv.cuh"
+#include "vpmc_gamma.cuh"
 
 struct BeamHost {
     vpmc_frame frame;
@@ -98,6 +99,7 @@ struct vpmc {
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
         ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
     vpmc_influence_stats inf_stats = {};
+    DevBuf gamma_buf;                 // counters + list of the voxels that fail the zero-distance test (vpmc_gamma)
     DevBuf spmv_part;                 // first / last partial sums per chunk of vpmc_spmv_grad
     size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
 

@@ -98,3 +98,32 @@ extern "C" int vpmc_robust_iteration(vpmc_t *h, const vpmc_csr *mats, int32_t n_
         if ((rc = spmv_grad_launch(h, mats + s, resid_ws_dev + (size_t)s * n_cols, grad_dev, s > 0, st))) return rc;
     return VPMC_OK;
 }
+
+// ---- S:8f-3: 3-D gamma index of two dose grids of this engine's CT (vpmc_gamma.cuh)
+extern "C" int vpmc_gamma(vpmc_t *h, const float *ref_dev, const float *eval_dev, float dd_rel, float dta_mm, float threshold_rel, int32_t sub,
+                          uint64_t *n_eval_out, uint64_t *n_fail_out, void *cuda_stream)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (!ref_dev || !eval_dev || !(dd_rel > 0) || !(dta_mm > 0) || !(threshold_rel >= 0) || sub < 1 || sub > 64 || !n_eval_out || !n_fail_out)
+        FAIL(h, VPMC_ERR_INVALID_ARG, "bad gamma arguments");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->last_stream = st; h->launched = true;
+    int rc;
+    const unsigned int cap = (unsigned int)std::min<long long>(h->nvox, 0x7fffffffLL);
+    if ((rc = ensure(h, h->gamma_buf, sizeof(GammaCounts) + (size_t)cap * sizeof(unsigned int)))) return rc;
+    GammaCounts *c = h->gamma_buf.as<GammaCounts>();
+    unsigned int *list = reinterpret_cast<unsigned int *>(c + 1);
+    GammaArgs a = { h->G.nx, h->G.ny, h->G.nz, h->G.hx, h->G.hy, h->G.hz, dd_rel, dta_mm, threshold_rel, (int)sub };
+    CU(h, cudaMemsetAsync(c, 0, sizeof(GammaCounts), st));
+    const int g = grid_for(h->nvox, h->n_sm);
+    gamma_max_kernel<<<g, 256, 0, st>>>(ref_dev, h->nvox, c);
+    gamma_select_kernel<<<g, 256, 0, st>>>(ref_dev, eval_dev, h->nvox, a, c, list, cap);
+    gamma_search_kernel<<<h->n_sm * 8, 256, 0, st>>>(ref_dev, eval_dev, a, c, list, cap);
+    CU(h, cudaGetLastError());
+    h->launches += 3;
+    GammaCounts out;
+    CU(h, cudaMemcpyAsync(&out, c, sizeof(out), cudaMemcpyDeviceToHost, st));
+    CU(h, cudaStreamSynchronize(st));
+    *n_eval_out = out.n_eval; *n_fail_out = out.n_fail;
+    return VPMC_OK;
+}
