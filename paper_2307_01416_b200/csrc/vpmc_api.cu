@@ -153,7 +153,7 @@ static DevParams make_dev_params(const vpmc_params &p)
     d.brass_za_rho = (float)((double)p.brass_za * (double)p.brass_rho);
     d.rs_rsp = p.rs_rsp; d.rs_inv_rsp = (float)(1.0 / (double)p.rs_rsp); d.rs_rho = p.rs_rho; d.rs_inv_X0 = (float)(1.0 / (double)p.rs_X0);
     d.rs_za_rho = (float)((double)p.za_w * (double)p.rs_rho);
-    d.rho_min = p.rho_min; d.delta_E = p.delta_E; d.flags = p.flags;
+    d.rho_min = p.rho_min; d.delta_E = p.delta_E; d.flags = p.flags; d.R_cut_d = (double)p.R_cut;
     const double pp = (double)p.p;
     d.pc2 = (float)(pp * (pp - 1) / 2); d.pc3 = (float)(pp * (pp - 1) * (pp - 2) / 6);
     d.pc4 = (float)(pp * (pp - 1) * (pp - 2) * (pp - 3) / 24); d.pc5 = (float)(pp * (pp - 1) * (pp - 2) * (pp - 3) * (pp - 4) / 120);
@@ -195,7 +195,7 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     for (auto &o : h->owned) pool_give(o.p, o.bytes);
     h->owned.clear();
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
-                       &h->inf_tile0, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
+                       &h->inf_tile0, &h->inf_tilecol, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
                        &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part, &h->gamma_buf };
     for (DevBuf *b : bufs) if (b->p) { pool_give(b->p, b->bytes); b->p = nullptr; }

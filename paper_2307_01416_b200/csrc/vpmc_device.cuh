@@ -35,6 +35,7 @@ struct DevParams {
     float rho_min, delta_E;
     float pc2, pc3, pc4, pc5;     // binomial coefficients of (1+d)^p - 1 = d (p + d (pc2 + d (pc3 + ...)))
     int flags;
+    double R_cut_d;               // R_cut as fp64: the stop test compares the fp64 range with it every step
 };
 
 struct DevGrid {
@@ -116,6 +117,12 @@ __device__ __forceinline__ void pair_axpy(uint32_t &ghi, uint32_t &glo, float s,
 }
 
 struct StepOut { float s, dep, removed, theta, uphi; int on_d; };
+
+// fp32 -> fp64 without the flush-to-zero canonicalisation -ftz=true attaches to the plain cast (one FMUL per conversion)
+__device__ __forceinline__ double f2d(float x)
+{
+    double d; asm("cvt.f64.f32 %0, %1;" : "=d"(d) : "f"(x)); return d;
+}
 
 // ---------------------------------------------------------------------------------------------- C1
 // the ten round keys (k + r * Weyl increment) are the same for every thread: they are computed once on the host and
@@ -206,15 +213,18 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     const float E = h.E;
     // 1
     const float R = (float)h.R;
-    if (h.R <= (double)P.R_cut) { o.dep = E; o.s = 0.0f; h.E = 0.0f; h.R = 0.0; return STOPPED; }
+    if (h.R <= P.R_cut_d) { o.dep = E; o.s = 0.0f; h.E = 0.0f; h.R = 0.0; return STOPPED; }
     // 2
     float s = d; int face = 1;
     const float lim = fmaxf(P.f_R * R, P.R_cut) * m.inv_rsp;
     if (lim < s) { s = lim; face = 0; }
     if (P.s_max < s) { s = P.s_max; face = 0; }
-    // R' >= 0 by construction (C4-2), but inv_rsp is a rounded reciprocal: when the step is the R_cut limit and R is within
-    // an ulp of R_cut, s * rsp can exceed R by 1e-7.  Clamped, so that the logarithm below never sees a negative range.
-    const double Rp = fmax(fma(-(double)s, (double)m.rsp, h.R), 0.0);
+    // R' > 0 by construction (C4-2), but inv_rsp is a rounded reciprocal: when the step is the R_cut limit and R is within
+    // an ulp of R_cut, s * rsp can exceed R by 1e-7.  R' is kept above 1e-12 mm, so that the logarithm below never sees a
+    // non-positive range and the update R_next = R' (E'/Ebar)^p stays what it is everywhere else (R_next <= R_cut then: the
+    // history stops at its next step).
+    double Rp = fma(-f2d(s), f2d(m.rsp), h.R);
+    Rp = (Rp > 1e-12) ? Rp : 1e-12;
     // E is re-derived from the fp64 range every step, so a 3e-7 relative MUFU error does not accumulate
     const float Ebar = exp2f(P.inv_p * __log2f((float)Rp * P.inv_alpha));
     // mean energy lost in the step.  E - Ebar cancels when the step is thin in water-equivalent terms (1 mm of air
@@ -244,8 +254,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
             if (fabsf(dl) < 0.05f) g1 = dl * fmaf(dl, fmaf(dl, fmaf(dl, fmaf(dl, P.pc5, P.pc4), P.pc3), P.pc2), P.p);
             else g1 = exp2f(P.p * __log2f(1.0f + dl)) - 1.0f;   // end of range only (sigma_E / E > 5 %): nothing cancels, and a
                                                                 // 3e-7 relative error of a residual range of a few mm is 1e-6 mm
-            Rn = fma(Rp, (double)g1, Rp);
-            if (!(Rp > 0.0)) Rn = (double)(P.alpha * exp2f(P.p * __log2f(Ep)));      // R' clamped to 0 (Ebar = 0): alpha E'^p directly
+            Rn = fma(Rp, f2d(g1), Rp);
         }
     }
     // 5

@@ -95,7 +95,7 @@ struct vpmc {
     bool seq_valid = false;
 
     // influence workspace (grown on demand)
-    DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_skip, inf_tilecnt, inf_colmax,
+    DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_tilecol, inf_skip, inf_tilecnt, inf_colmax,
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
         ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
     vpmc_influence_stats inf_stats = {};

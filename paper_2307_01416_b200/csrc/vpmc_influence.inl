@@ -261,6 +261,13 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 CsrCols cc{};
                 cc.lo = cb.lo; cc.dim = cb.dim; cc.offset = cb.offset; cc.tile0 = h->inf_tile0.as<int>(); cc.skip = h->inf_skip.as<int>();
                 cc.n_cols = nc; cc.n_tiles = tile0.back(); cc.nx = h->G.nx; cc.ny = h->G.ny;
+                cc.tile_col = nullptr;
+                if (cc.n_tiles > 0) {
+                    rc = ensure(h, h->inf_tilecol, (size_t)cc.n_tiles * sizeof(int)); if (rc) return rc;
+                    csr_tile_cols_kernel<<<(cc.n_tiles + 255) / 256, 256, 0, st>>>(cc, h->inf_tilecol.as<int>());
+                    cc.tile_col = h->inf_tilecol.as<int>();
+                    h->launches += 1;
+                }
                 rc = csr_max_pass(h, cc, cb.scratch, true, coef, st); if (rc) return rc;
                 std::vector<unsigned int> ocnt(nc, 0u);
                 int n_sel = 0;

@@ -828,15 +828,27 @@ struct CsrCols {
     const unsigned long long *offset;   // element offset of each column in `data`
     const int *tile0;                   // [n_cols + 1] prefix of tiles per column
     const int *skip;                    // [n_cols] or NULL: non-zero = column not written in this round
+    const int *tile_col;                // [n_tiles] or NULL: column of every tile (the passes would otherwise each spend a
+                                        // dependent 11-load binary search per 8 KB tile: measured 2.4 TB/s instead of HBM speed)
     int n_cols, n_tiles;
     int nx, ny;                         // of the CT grid (voxel index of box element)
 };
 
 __device__ __forceinline__ int tile_column(const CsrCols &cc, int tile)
 {
+    if (cc.tile_col) return __ldg(cc.tile_col + tile);       // looked up once per group by csr_tile_cols_kernel
     int lo = 0, hi = cc.n_cols;
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(cc.tile0 + mid) <= tile) lo = mid; else hi = mid; }
     return lo;
+}
+
+// column of every tile, once per group
+__global__ void csr_tile_cols_kernel(CsrCols cc, int *__restrict__ tile_col)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= cc.n_tiles) return;
+    cc.tile_col = nullptr;
+    tile_col[t] = tile_column(cc, t);
 }
 
 // first element of this thread in its tile (a box has < 2^31 elements) and the number of elements it owns (0..kPerThread)
