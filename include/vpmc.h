@@ -199,6 +199,15 @@ int vpmc_set_aperture_polygon(vpmc_t *h, int beam, float thickness_mm, int mater
  * outside the bitmap brass, then to the nearest tile holding any open pixel.  Any output pointer may be NULL. */
 int vpmc_get_aperture_tables(vpmc_t *h, int beam, uint32_t *bits_out_host, uint8_t *dist_out_host, int32_t *dims_out);
 
+/* S:8f-4, coarse-grid scoring ("memory usage was further reduced by using dynamic voxel spacing"): score on a grid whose
+ * cells are div_x x div_y x div_z CT voxels (the last cell of an axis may be smaller); transport is unchanged.  Afterwards
+ * every dose grid this handle takes or returns (vpmc_dose*, vpmc_dose_to_uncertainty, vpmc_gamma) has sn_x*sn_y*sn_z elements,
+ * sn = ceil(n / div) (vpmc_get_scoring_dims), cell c = cx + sn_x (cy + sn_y cz), and the influence matrices' columns are cells.
+ * Dose of a cell = its energy / its mass: (W/N) E_dep[c] / (V_vox sum_{v in c} max(rho_v, rho_min)) x 1.602176634e-10 Gy,
+ * which is C6 for (1, 1, 1), the default.  One factor for the whole grid; spacing per organ would need contours (not built). */
+int vpmc_set_scoring_grid(vpmc_t *h, int32_t div_x, int32_t div_y, int32_t div_z);
+int vpmc_get_scoring_dims(vpmc_t *h, int32_t *dims_out /* [3] */);
+
 /* Restrict the next dose / trace calls to history ids [hid_begin, hid_end) of the N-history run (prefix
  * parity, S:8d).  hid_end = 0 -> no restriction. */
 int vpmc_set_history_window(vpmc_t *h, uint64_t hid_begin, uint64_t hid_end);

@@ -303,6 +303,30 @@ def dose_from_edep(pb: Problem, edep: np.ndarray, scale: float) -> np.ndarray:
     return out
 
 
+def coarse_cells(pb: Problem, div):
+    """SURVEY 8(f)-4 / include/vpmc.h vpmc_set_scoring_grid: cell index of every voxel (flat, v = ix + nx (iy + ny iz)) for cells of
+    div voxels per axis, and the scoring grid's dimensions sn = ceil(n / div); cell c = cx + sn_x (cy + sn_y cz)."""
+    n = [int(x) for x in pb.ct["n"]]
+    sn = [(n[a] + int(div[a]) - 1) // int(div[a]) for a in range(3)]
+    iz, iy, ix = np.meshgrid(np.arange(n[2]) // int(div[2]), np.arange(n[1]) // int(div[1]), np.arange(n[0]) // int(div[0]), indexing="ij")
+    return (ix + sn[0] * (iy + sn[1] * iz)).reshape(-1), sn
+
+
+def dose_from_edep_coarse(pb: Problem, edep: np.ndarray, scale: float, div) -> np.ndarray:
+    """Dose of the scoring cells: energy of a cell / mass of a cell, the density floored per voxel as in C6:
+    dose[c] = scale * sum_{v in c} E_dep[v] / (V_vox * sum_{v in c} max(rho_v, rho_min)) * 1.602176634e-10 Gy."""
+    cell, sn = coarse_cells(pb, div)
+    ncell = sn[0] * sn[1] * sn[2]
+    hu = np.asarray(pb.ct["hu"], dtype=np.float64).reshape(-1)
+    rho = np.interp(hu, _f64(pb.calib["hu"]), _f64(pb.calib["rho"]))          # piecewise linear, clamped at the end nodes (C5)
+    rho = np.maximum(rho, float(pb.params.rho_min))
+    h = [float(x) for x in pb.ct["h"]]
+    V = h[0] * h[1] * h[2] * 1e-3
+    e_c = np.bincount(cell, weights=_f64(edep), minlength=ncell)
+    m_c = np.bincount(cell, weights=rho, minlength=ncell) * V
+    return float(scale) * e_c / m_c * 1.602176634e-10
+
+
 def dose(pb: Problem, N: int, seed: int, sc: Scenario | None = None):
     """Full dose-mode result: dose [Gy] (fp64, flat), tallies.  scale = W/N (C6)."""
     e, tal = dose_edep(pb, N, seed, sc)

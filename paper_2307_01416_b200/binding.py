@@ -23,7 +23,8 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
            "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats", "vpmc_spmv_dose", "vpmc_spmv_grad",
-           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon", "vpmc_gamma"]
+           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon", "vpmc_gamma", "vpmc_set_scoring_grid",
+           "vpmc_get_scoring_dims"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE = range(6)
@@ -153,6 +154,8 @@ def lib():
         L.vpmc_set_aperture_polygon.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_int, C.c_void_p, C.c_int32, C.c_float]
         L.vpmc_gamma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int32, C.POINTER(C.c_uint64),
                                  C.POINTER(C.c_uint64), C.c_void_p]
+        L.vpmc_set_scoring_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32]
+        L.vpmc_get_scoring_dims.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
         L.vpmc_digests.argtypes = [C.c_void_p, C.POINTER(Scenario), C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -204,6 +207,7 @@ class Engine:
             raise VpmcError(rc, L.vpmc_last_error(None).decode())
         self.n = tuple(int(x) for x in ct["n"])
         self.nvox = self.n[0] * self.n[1] * self.n[2]
+        self.ncell = self.nvox              # elements of a dose grid (vpmc_set_scoring_grid changes it)
         self.h2d_bytes = hu.nbytes + sum(a.nbytes for a in arrs.values() if a is not None)
         self.n_spots = 0
         for b in problem["beams"]:
@@ -256,6 +260,14 @@ class Engine:
     def set_history_window(self, begin: int, end: int):
         self._check(lib().vpmc_set_history_window(self._h, int(begin), int(end)))
 
+    def set_scoring_grid(self, div=(1, 1, 1)):
+        """Score on cells of div voxels per axis (vpmc_set_scoring_grid); returns the scoring grid's dimensions."""
+        self._check(lib().vpmc_set_scoring_grid(self._h, int(div[0]), int(div[1]), int(div[2])))
+        d = (C.c_int32 * 3)()
+        self._check(lib().vpmc_get_scoring_dims(self._h, d))
+        self.ncell = int(d[0]) * int(d[1]) * int(d[2])
+        return int(d[0]), int(d[1]), int(d[2])
+
     def set_shard(self, index: int, count: int):
         """This handle computes shard `index` of `count` (vpmc_set_shard)."""
         self._check(lib().vpmc_set_shard(self._h, int(index), int(count)))
@@ -265,8 +277,8 @@ class Engine:
         """Dose [Gy] as a torch.float32 CUDA tensor of nvox elements (v = ix + nx*(iy + ny*iz))."""
         import torch
         if out is None:
-            out = torch.empty(self.nvox, dtype=torch.float32, device="cuda")
-        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.nvox and out.is_contiguous()
+            out = torch.empty(self.ncell, dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.ncell and out.is_contiguous()
         st = torch.cuda.current_stream() if stream is None else stream
         if sc is None:
             self._check(lib().vpmc_dose(self._h, int(n_histories), int(seed), out.data_ptr(), st.cuda_stream))
@@ -281,8 +293,8 @@ class Engine:
         (vpmc_dose_to_uncertainty).  Returns the dose tensor; run_info() gives (batches, estimate, reached)."""
         import torch
         if out is None:
-            out = torch.empty(self.nvox, dtype=torch.float32, device="cuda")
-        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.nvox and out.is_contiguous()
+            out = torch.empty(self.ncell, dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.numel() == self.ncell and out.is_contiguous()
         st = torch.cuda.current_stream() if stream is None else stream
         self._check(lib().vpmc_dose_to_uncertainty(self._h, C.byref(sc) if sc is not None else None, int(batch_histories),
                                                    int(min_batches), int(max_batches), float(target), int(seed),
@@ -296,7 +308,8 @@ class Engine:
 
     def dose_host(self, n_histories: int, seed: int, out: np.ndarray | None = None) -> np.ndarray:
         if out is None:
-            out = np.empty(self.nvox, dtype=np.float32)
+            out = np.empty(self.ncell, dtype=np.float32)
+        assert out.size == self.ncell
         self._check(lib().vpmc_dose_host(self._h, int(n_histories), int(seed), out.ctypes.data))
         return out
 
@@ -375,7 +388,7 @@ class Engine:
     def spmv_dose(self, m, w, n_cols: int | None = None, out=None, stream=None):
         """dose[v] = sum_j D[j][v] w[j] for a CSR matrix m = (row_ptr, col, val) of CUDA tensors (rows = spots)."""
         import torch
-        n_cols = self.nvox if n_cols is None else int(n_cols)
+        n_cols = self.ncell if n_cols is None else int(n_cols)
         if out is None:
             out = torch.empty(n_cols, dtype=torch.float32, device="cuda")
         assert w.is_cuda and w.dtype == torch.float32 and w.is_contiguous() and out.numel() == n_cols
@@ -430,7 +443,7 @@ class Engine:
         """3-D gamma of two dose tensors on this engine's grid (vpmc_gamma): (pass rate, voxels evaluated, voxels failing)."""
         import torch
         for t in (ref, ev):
-            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.nvox
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.ncell
         st = torch.cuda.current_stream() if stream is None else stream
         ne, nf = C.c_uint64(), C.c_uint64()
         self._check(lib().vpmc_gamma(self._h, ref.data_ptr(), ev.data_ptr(), float(dd), float(dta), float(thr), int(sub), C.byref(ne),

@@ -243,7 +243,8 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     vpmc_t *h = new vpmc();
     h->params = p;
     h->P = make_dev_params(p);
-    h->nvox = nvox;
+    h->nvox = nvox; h->ncell = nvox;
+    h->sn[0] = ct->n[0]; h->sn[1] = ct->n[1]; h->sn[2] = ct->n[2];
     cudaGetDevice(&h->device);
     cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
     DevGrid &G = h->G;
@@ -476,6 +477,42 @@ extern "C" int vpmc_get_aperture_tables(vpmc_t *h, int beam, uint32_t *bits_out_
     CU(h, cudaStreamSynchronize(h->setup_stream));
     if (bits_out_host) CU(h, cudaMemcpy(bits_out_host, b.d_bits, (size_t)b.ap_row_words * b.ap_ny * sizeof(uint32_t), cudaMemcpyDeviceToHost));
     if (dist_out_host) CU(h, cudaMemcpy(dist_out_host, b.d_dist, (size_t)2 * b.ap_ntx * b.ap_nty, cudaMemcpyDeviceToHost));
+    return VPMC_OK;
+}
+
+static ScoreGeom score_geom(const vpmc_t *h)
+{
+    ScoreGeom g;
+    g.on = h->d_cell_rho ? 1 : 0;
+    g.dx = h->sdiv[0]; g.dy = h->sdiv[1]; g.dz = h->sdiv[2]; g.snx = h->sn[0]; g.sny = h->sn[1];
+    return g;
+}
+
+extern "C" int vpmc_set_scoring_grid(vpmc_t *h, int32_t div_x, int32_t div_y, int32_t div_z)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    if (div_x < 1 || div_y < 1 || div_z < 1 || div_x > h->G.nx || div_y > h->G.ny || div_z > h->G.nz) FAIL(h, VPMC_ERR_INVALID_ARG, "scoring divisors must be in [1, n] per axis");
+    dev_release(h, h->d_cell_rho); dev_release(h, h->d_s1); dev_release(h, h->d_s2);       // sized by the scoring grid
+    h->d_cell_rho = nullptr; h->d_s1 = nullptr; h->d_s2 = nullptr;
+    h->sdiv[0] = div_x; h->sdiv[1] = div_y; h->sdiv[2] = div_z;
+    const int n[3] = { h->G.nx, h->G.ny, h->G.nz };
+    for (int a = 0; a < 3; ++a) h->sn[a] = (n[a] + h->sdiv[a] - 1) / h->sdiv[a];
+    h->ncell = (long long)h->sn[0] * h->sn[1] * h->sn[2];
+    h->unc_valid = false;
+    if (div_x == 1 && div_y == 1 && div_z == 1) return VPMC_OK;
+    int rc = dev_alloc(h, (void **)&h->d_cell_rho, (size_t)h->ncell * sizeof(float)); if (rc) return rc;
+    // the per-voxel buffers of the uncertainty estimate keep their (larger) size
+    cell_rho_kernel<<<(unsigned)((h->ncell + 127) / 128), 128, 0, h->setup_stream>>>(h->d_hu, h->d_lut, h->G, h->params.rho_min, score_geom(h), h->sn[2], h->d_cell_rho);
+    CU(h, cudaGetLastError());
+    h->launches += 1;
+    h->setup_pending = true;
+    return VPMC_OK;
+}
+
+extern "C" int vpmc_get_scoring_dims(vpmc_t *h, int32_t *dims_out)
+{
+    if (!h || !dims_out) return VPMC_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a) dims_out[a] = h->sn[a];
     return VPMC_OK;
 }
 

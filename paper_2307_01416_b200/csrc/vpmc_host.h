@@ -45,6 +45,10 @@ struct vpmc {
     vpk::DevGrid G;
     long long nvox = 0;
     int device = 0, n_sm = 0;
+    // scoring grid (S:8f-4, vpmc_set_scoring_grid): cells of sdiv voxels per axis; ncell = nvox and d_cell_rho = NULL by default
+    int sdiv[3] = { 1, 1, 1 }, sn[3] = { 0, 0, 0 };
+    long long ncell = 0;
+    float *d_cell_rho = nullptr;      // per cell: sum over its voxels of max(rho, rho_min)
 
     // Device memory of the fixed-size members below comes from the process-wide buffer cache (vpmc_api.cu) and goes back to
     // it in vpmc_destroy.  Set-up work (uploads, S0 kernels) is enqueued on setup_stream; the next compute call makes its

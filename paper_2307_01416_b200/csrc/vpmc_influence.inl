@@ -47,9 +47,9 @@ static int csr_max_pass(vpmc_t *h, const CsrCols &cc, float *data, bool convert,
         const int grid = std::max(1, std::min(cc.n_tiles, h->n_sm * 8));
         TimedScope ts(h, st, 3);
         if (convert)
-            csr_max_kernel<true><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
+            csr_max_kernel<true><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>(), h->d_cell_rho);
         else
-            csr_max_kernel<false><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
+            csr_max_kernel<false><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>(), nullptr);
         CU(h, cudaGetLastError());
         h->launches += 1;
     }
@@ -120,10 +120,9 @@ extern "C" int vpmc_set_workspace_limit(vpmc_t *h, uint64_t bytes)
     return VPMC_OK;
 }
 
-static HostBox grown_box(const int bb[6], const DevGrid &G, float grow, int pad_vox)
+static HostBox grown_box(const int bb[6], const int n[3], float grow, int pad_vox)
 {
     HostBox b;
-    const int n[3] = { G.nx, G.ny, G.nz };
     for (int a = 0; a < 3; ++a) {
         const int ext = bb[3 + a] - bb[a] + 1;
         const int pad = (int)std::ceil(grow * (float)ext) + pad_vox;
@@ -174,7 +173,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
             wm.mode = 1; wm.hps = hist_per_spot; wm.n_sub = n_pilot; wm.cols = nullptr; wm.g0 = g_lo;
             wm.n_items = (unsigned long long)(g_hi - g_lo) * n_pilot;
             ScoreArgs sa{};
-            sa.cb.bbox = h->inf_bbox.as<int>();
+            sa.cb.bbox = h->inf_bbox.as<int>(); sa.sg = score_geom(h);
             CU(h, cudaMemsetAsync(h->d_tal_scratch, 0, sizeof(DevTallies), st));
             rc = launch_transport<2>(h, ctx, wm, sa, h->d_tal_scratch, st); if (rc) return rc;
         }
@@ -185,7 +184,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
         for (int g = g_lo; g < g_hi; ++g) {           // the pilot's columns are local: column c = spot g_lo + c
             const int *pb = &bb[6 * (size_t)(g - g_lo)];
             if (pb[3] < 0) { for (int a = 0; a < 3; ++a) { box[g].lo[a] = 0; box[g].dim[a] = 1; } }   // pilot deposited nothing
-            else box[g] = grown_box(pb, h->G, h->box_grow, h->box_pad);
+            else box[g] = grown_box(pb, h->sn, h->box_grow, h->box_pad);
         }
         // ---- 3./4. groups, with replay of the columns that outgrew their box
         std::vector<long long> row_nnz(ns, 0), row_src(ns, 0), row_ovf_off(ns, 0);
@@ -235,7 +234,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     wm.mode = 1; wm.hps = hist_per_spot; wm.n_sub = hist_per_spot; wm.cols = h->inf_cols.as<int>(); wm.g0 = 0;
                     wm.n_items = (unsigned long long)nc * hist_per_spot;
                     ScoreArgs sa{};
-                    sa.cb = cb;
+                    sa.cb = cb; sa.sg = score_geom(h);
                     if (replay) CU(h, cudaMemsetAsync(h->d_tal_scratch, 0, sizeof(DevTallies), st));
                     rc = launch_transport<1>(h, ctx, wm, sa, replay ? h->d_tal_scratch : h->d_tal, st); if (rc) return rc;
                 }
@@ -260,7 +259,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 rc = upload(h, h->inf_skip, skip, st); if (rc) return rc;
                 CsrCols cc{};
                 cc.lo = cb.lo; cc.dim = cb.dim; cc.offset = cb.offset; cc.tile0 = h->inf_tile0.as<int>(); cc.skip = h->inf_skip.as<int>();
-                cc.n_cols = nc; cc.n_tiles = tile0.back(); cc.nx = h->G.nx; cc.ny = h->G.ny;
+                cc.n_cols = nc; cc.n_tiles = tile0.back(); cc.nx = h->sn[0]; cc.ny = h->sn[1];
                 cc.tile_col = nullptr;
                 if (cc.n_tiles > 0) {
                     rc = ensure(h, h->inf_tilecol, (size_t)cc.n_tiles * sizeof(int)); if (rc) return rc;
@@ -288,7 +287,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     CU(h, cub::DeviceRadixSort::SortPairs(h->cub_temp.p, tb, k1, k2, v1, v2, (int)n_ovf, 0, 56, st));
                     CU(h, cub::DeviceReduce::ReduceByKey(h->cub_temp.p, tb, k2, k1, v2, v1, ctr + 1, cub::Sum(), (int)n_ovf, st));
                     const int g1 = std::max(1, std::min((int)((n_ovf + 255) / 256), h->n_sm * 8));
-                    ovf_convert_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>());
+                    ovf_convert_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>(), h->d_cell_rho);
                     CU(h, cudaMemsetAsync(h->ovf_colcnt.p, 0, (size_t)nc * 4, st));
                     CU(h, cudaMemsetAsync(h->ovf_flag.p, 0, (size_t)n_ovf, st));
                     ovf_flag_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->inf_colmax.as<unsigned int>(), h->inf_skip.as<int>(), rel_threshold,

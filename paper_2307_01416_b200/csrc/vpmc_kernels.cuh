@@ -75,10 +75,25 @@ __device__ __forceinline__ void map_item(const WorkMap &wm, unsigned long long k
 }
 
 // ------------------------------------------------------------------------------------------- scorers (S6, S7)
+// S:8f-4, coarse-grid scoring: deposits can be scored on a grid whose cells are div[0] x div[1] x div[2] CT voxels
+// (vpmc_set_scoring_grid); on = 0 is the plain case, scoring cell = CT voxel.
+struct ScoreGeom { int on; int dx, dy, dz; int snx, sny; };
+
+__device__ __forceinline__ void score_coords(const ScoreGeom &sg, const Hist &h, int &x, int &y, int &z)
+{
+    x = (int)h.g0; y = (int)h.g1; z = (int)h.g2;
+    if (sg.on) { x /= sg.dx; y /= sg.dy; z /= sg.dz; }
+}
+
 struct DoseScorer {            // MODE 0: E_dep[batch][v] += dE, fp32 RED into L2-resident grids
-    float *edep; unsigned long long nvox;
+    float *edep; unsigned long long nvox; ScoreGeom sg;
     __device__ __forceinline__ void begin(const Hist &) {}
-    __device__ __forceinline__ void deposit(const Hist &h, float dep) { atomicAdd(edep + (size_t)h.col * nvox + h.g3, dep); }
+    __device__ __forceinline__ void deposit(const Hist &h, float dep)
+    {
+        unsigned int v = h.g3;
+        if (sg.on) { int x, y, z; score_coords(sg, h, x, y, z); v = (unsigned)(x + sg.snx * (y + sg.sny * z)); }
+        atomicAdd(edep + (size_t)h.col * nvox + v, dep);
+    }
     __device__ __forceinline__ void end(const Hist &) {}
 };
 
@@ -89,32 +104,37 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
 }
 
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
-    ColumnBoxes cb;
+    ColumnBoxes cb; ScoreGeom sg;
     __device__ __forceinline__ void begin(const Hist &) {}
     __device__ __forceinline__ void deposit(const Hist &h, float dep)
     {
         const int c = h.col;
         const int4 lo = __ldg(cb.lo + c), dm = __ldg(cb.dim + c);
-        const int bx = (int)h.g0 - lo.x, by = (int)h.g1 - lo.y, bz = (int)h.g2 - lo.z;
+        int sx, sy, sz;
+        score_coords(sg, h, sx, sy, sz);
+        const int bx = sx - lo.x, by = sy - lo.y, bz = sz - lo.z;
         if ((unsigned)bx < (unsigned)dm.x && (unsigned)by < (unsigned)dm.y && (unsigned)bz < (unsigned)dm.z)
             atomicAdd(cb.scratch + __ldg(cb.offset + c) + (bx + (unsigned long long)dm.x * (by + (unsigned long long)dm.y * bz)), dep);
         else {
             const unsigned slot = atomicAdd(cb.ovf_count, 1u);
-            if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | h.g3; cb.ovf_val[slot] = dep; }
-            else bbox_merge(cb.bbox + 6 * c, (int)h.g0, (int)h.g1, (int)h.g2, (int)h.g0, (int)h.g1, (int)h.g2);
+            const unsigned int v = sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3;
+            if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | v; cb.ovf_val[slot] = dep; }
+            else bbox_merge(cb.bbox + 6 * c, sx, sy, sz, sx, sy, sz);
         }
     }
     __device__ __forceinline__ void end(const Hist &) {}
 };
 
 struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits of each column
-    int *bbox;
+    int *bbox; ScoreGeom sg;
     int x0, y0, z0, x1, y1, z1;
     __device__ __forceinline__ void begin(const Hist &) { x0 = y0 = z0 = 0x7fffffff; x1 = y1 = z1 = -1; }
     __device__ __forceinline__ void deposit(const Hist &h, float)
     {
-        x0 = min(x0, (int)h.g0); y0 = min(y0, (int)h.g1); z0 = min(z0, (int)h.g2);
-        x1 = max(x1, (int)h.g0); y1 = max(y1, (int)h.g1); z1 = max(z1, (int)h.g2);
+        int sx, sy, sz;
+        score_coords(sg, h, sx, sy, sz);
+        x0 = min(x0, sx); y0 = min(y0, sy); z0 = min(z0, sz);
+        x1 = max(x1, sx); y1 = max(y1, sy); z1 = max(z1, sz);
     }
     __device__ __forceinline__ void end(const Hist &h) { if (x1 >= 0) bbox_merge(bbox + 6 * h.col, x0, y0, z0, x1, y1, z1); }
 };
@@ -124,12 +144,12 @@ template <> struct ScorerOf<0> { typedef DoseScorer type; };
 template <> struct ScorerOf<1> { typedef BoxScorer type; };
 template <> struct ScorerOf<2> { typedef BoundsScorer type; };
 
-struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; };
+struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; ScoreGeom sg; };
 
 template <int MODE> __device__ __forceinline__ typename ScorerOf<MODE>::type make_scorer(const ScoreArgs &a);
-template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox }; }
-template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { return BoxScorer{ a.cb }; }
-template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; return s; }
+template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox, a.sg }; }
+template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { return BoxScorer{ a.cb, a.sg }; }
+template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; s.sg = a.sg; return s; }
 
 // ------------------------------------------------------------------------------------------- S1-S7
 // Pipeline of one chunk of work items:
@@ -683,12 +703,37 @@ __global__ void step_state_kernel(const Ctx c, const StateIn *__restrict__ in, i
 }
 
 // ------------------------------------------------------------------------------------------- S6 / C6
+// Density in the dose conversion: max(rho_v, rho_min) of the voxel, or, with coarse-grid scoring, the sum of that over the
+// cell's voxels (cell_rho, built by cell_rho_kernel): dose of a cell = its energy / its mass.
+__device__ __forceinline__ float score_density(const float *__restrict__ cell_rho, const short *__restrict__ hu, const float4 *__restrict__ lut,
+                                               int hu_min, int n_lut, float rho_min, long long v)
+{
+    if (cell_rho) return __ldg(cell_rho + v);
+    int t = (int)__ldg(hu + v) - hu_min;
+    t = min(max(t, 0), n_lut - 1);
+    return fmaxf(__ldg(lut + t).y, rho_min);
+}
+
+__global__ void cell_rho_kernel(const short *__restrict__ hu, const float4 *__restrict__ lut, DevGrid G, float rho_min, ScoreGeom sg, int snz,
+                                float *__restrict__ cell_rho)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= (long long)sg.snx * sg.sny * snz) return;
+    const int cz = (int)(c / ((long long)sg.snx * sg.sny)), rem = (int)(c - (long long)cz * sg.snx * sg.sny), cy = rem / sg.snx, cx = rem - cy * sg.snx;
+    float sum = 0.0f;
+    for (int z = cz * sg.dz; z < min((cz + 1) * sg.dz, G.nz); ++z)
+        for (int y = cy * sg.dy; y < min((cy + 1) * sg.dy, G.ny); ++y)
+            for (int x = cx * sg.dx; x < min((cx + 1) * sg.dx, G.nx); ++x)
+                sum += score_density(nullptr, hu, lut, G.hu_min, G.n_lut, rho_min, x + (long long)G.nx * (y + (long long)G.ny * z));
+    cell_rho[c] = sum;
+}
+
 // One pass over the B batch grids: dose[v] = coef * sum_b E_b[v] / max(rho_v, rho_min); with B >= 2 also the batch
 // sums s1 = sum_b f_b E_b, s2 = sum_b (f_b E_b)^2 (f_b = N / N_b scales a batch to full weight) for C6.
 __global__ void dose_finalize_kernel(const float *__restrict__ edep, int B, const float *__restrict__ fb,
                                      const short *__restrict__ hu, const float4 *__restrict__ lut, DevGrid G, float rho_min,
                                      float coef, float *__restrict__ dose, float *__restrict__ s1, float *__restrict__ s2,
-                                     long long n, unsigned int *max_bits)
+                                     long long n, unsigned int *max_bits, const float *__restrict__ cell_rho)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     float mx = 0.0f;
@@ -700,9 +745,7 @@ __global__ void dose_finalize_kernel(const float *__restrict__ edep, int B, cons
             const float y = __ldg(fb + b) * x;
             a1 += y; a2 = fmaf(y, y, a2);
         }
-        int t = (int)__ldg(hu + v) - G.hu_min;
-        t = min(max(t, 0), G.n_lut - 1);
-        const float rho = fmaxf(__ldg(lut + t).y, rho_min);
+        const float rho = score_density(cell_rho, hu, lut, G.hu_min, G.n_lut, rho_min, v);
         const float dv = __fdiv_rn(coef * sum, rho);
         dose[v] = dv;
         if (s1) { s1[v] = a1; s2[v] = a2; }
@@ -801,15 +844,13 @@ __global__ void seq_decide_kernel(cudaGraphConditionalHandle handle, SeqState *s
 
 // dose[v] = coef_batch / B * s1[v] / max(rho_v, rho_min), coef_batch = (W / N_b) / V * 1.602e-10 (C6 with N = B N_b)
 __global__ void seq_finalize_kernel(const float *__restrict__ s1, const short *__restrict__ hu, const float4 *__restrict__ lut, DevGrid G,
-                                    float rho_min, float coef_batch, const SeqState *st, float *__restrict__ dose, long long n)
+                                    float rho_min, float coef_batch, const SeqState *st, float *__restrict__ dose, long long n,
+                                    const float *__restrict__ cell_rho)
 {
     const float coef = coef_batch / (float)max(st->batch, 1u);
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
-        int t = (int)__ldg(hu + v) - G.hu_min;
-        t = min(max(t, 0), G.n_lut - 1);
-        dose[v] = __fdiv_rn(coef * s1[v], fmaxf(__ldg(lut + t).y, rho_min));
-    }
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride)
+        dose[v] = __fdiv_rn(coef * s1[v], score_density(cell_rho, hu, lut, G.hu_min, G.n_lut, rho_min, v));
 }
 
 // ------------------------------------------------------------------------------------------- S8: CSR writer
@@ -889,7 +930,7 @@ __device__ __forceinline__ void load8(const float *p, int cnt, float x[kPerThrea
 template <bool CONVERT>
 __global__ void __launch_bounds__(kBlock)
 csr_max_kernel(const CsrCols cc, float *__restrict__ data, const short *__restrict__ hu, const float4 *__restrict__ lut,
-               int hu_min, int n_lut, float rho_min, float coef, unsigned int *__restrict__ colmax_bits)
+               int hu_min, int n_lut, float rho_min, float coef, unsigned int *__restrict__ colmax_bits, const float *__restrict__ cell_rho)
 {
     for (int tile = blockIdx.x; tile < cc.n_tiles; tile += gridDim.x) {
         const int c = tile_column(cc, tile);
@@ -911,9 +952,7 @@ csr_max_kernel(const CsrCols cc, float *__restrict__ data, const short *__restri
             for (int i = 0; i < kPerThread; ++i) {
                 if (x[i] != 0.0f) {
                     const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
-                    int t = (int)__ldg(hu + v) - hu_min;
-                    t = min(max(t, 0), n_lut - 1);
-                    x[i] = __fdiv_rn(coef * x[i], fmaxf(__ldg(lut + t).y, rho_min));
+                    x[i] = __fdiv_rn(coef * x[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, v));
                 }
                 box_next(dm, bx, by, bz);
             }
@@ -1039,14 +1078,12 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
 // E_dep -> dose value, in place; the column maximum takes these entries into account
 __global__ void ovf_convert_kernel(const unsigned long long *__restrict__ key, float *__restrict__ val, const int *__restrict__ n_ptr,
                                    const short *__restrict__ hu, const float4 *__restrict__ lut, int hu_min, int n_lut,
-                                   float rho_min, float coef, unsigned int *__restrict__ colmax_bits)
+                                   float rho_min, float coef, unsigned int *__restrict__ colmax_bits, const float *__restrict__ cell_rho)
 {
     const int n = *n_ptr;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const unsigned long long k = key[i];
-        int t = (int)__ldg(hu + (unsigned)k) - hu_min;
-        t = min(max(t, 0), n_lut - 1);
-        const float x = __fdiv_rn(coef * val[i], fmaxf(__ldg(lut + t).y, rho_min));
+        const float x = __fdiv_rn(coef * val[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, (long long)(unsigned)k));
         val[i] = x;
         if (x > 0.0f) atomicMax(colmax_bits + (unsigned)(k >> 32), __float_as_uint(x));
     }

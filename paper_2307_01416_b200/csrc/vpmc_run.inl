@@ -216,9 +216,9 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     const int B = h->params.n_batches;
     const bool with_unc = B >= 2;
     if (with_unc && !h->d_s1) {
-        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->nvox * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->nvox * sizeof(float)))) return rc;
+        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->ncell * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->ncell * sizeof(float)))) return rc;
     }
-    rc = ensure(h, h->edep, (size_t)B * h->nvox * sizeof(float)); if (rc) return rc;
+    rc = ensure(h, h->edep, (size_t)B * h->ncell * sizeof(float)); if (rc) return rc;
     const size_t n_ent = (size_t)B * h->n_spots;
     rc = ensure(h, h->cum, (n_ent + 1) * sizeof(unsigned long long)); if (rc) return rc;
     rc = ensure(h, h->first, (n_ent + 1) * sizeof(unsigned long long)); if (rc) return rc;
@@ -251,7 +251,7 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     const unsigned long long n_total = cum[n_ent];
     for (int b = 0; b < B; ++b) fb[b] = nb[b] ? (float)((double)n_total / (double)nb[b]) : 0.0f;
 
-    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)B * h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)B * h->ncell * sizeof(float), st));
     CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
     CU(h, cudaMemsetAsync(h->d_max_bits, 0, sizeof(unsigned int), st));
     CU(h, cudaMemsetAsync(h->d_unc, 0, 2 * sizeof(double), st));
@@ -263,7 +263,7 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     wm.mode = 0; wm.n_items = n_total; wm.cum = h->cum.as<unsigned long long>(); wm.first = h->first.as<unsigned long long>();
     wm.n_entries = (int)n_ent; wm.n_spots = h->n_spots;
     ScoreArgs sa{};
-    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->nvox;
+    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->ncell; sa.sg = score_geom(h);
     rc = launch_transport<0>(h, make_ctx(h, sc, seed), wm, sa, h->d_tal, st); if (rc) return rc;
     // C6
     double W = 0.0;
@@ -271,12 +271,12 @@ extern "C" int vpmc_dose_scenario(vpmc_t *h, const vpmc_scenario *scp, uint64_t 
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef = (float)((n_histories ? W / (double)n_histories : 0.0) / V * 1.602176634e-10);
     TimedScope ts(h, st, 2);
-    dose_finalize_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(h->edep.as<float>(), B, h->d_fb, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef,
-                                                                   dose_out_dev, with_unc ? h->d_s1 : nullptr, with_unc ? h->d_s2 : nullptr, h->nvox, h->d_max_bits);
+    dose_finalize_kernel<<<grid_for(h->ncell, h->n_sm), 256, 0, st>>>(h->edep.as<float>(), B, h->d_fb, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef,
+                                                                   dose_out_dev, with_unc ? h->d_s1 : nullptr, with_unc ? h->d_s2 : nullptr, h->ncell, h->d_max_bits, h->d_cell_rho);
     CU(h, cudaGetLastError());
     h->launches += 1;
     if (with_unc) {
-        uncertainty_kernel<<<grid_for(h->nvox, h->n_sm), 256, 0, st>>>(dose_out_dev, h->d_s1, h->d_s2, h->nvox, B, h->d_max_bits, h->d_unc);
+        uncertainty_kernel<<<grid_for(h->ncell, h->n_sm), 256, 0, st>>>(dose_out_dev, h->d_s1, h->d_s2, h->ncell, B, h->d_max_bits, h->d_unc);
         CU(h, cudaGetLastError());
         h->launches += 1;
         h->unc_valid = true;
@@ -295,11 +295,11 @@ extern "C" int vpmc_dose_host(vpmc_t *h, uint64_t n_histories, uint64_t seed, fl
     if (!h) return VPMC_ERR_INVALID_ARG;
     if (!dose_out_host) FAIL(h, VPMC_ERR_INVALID_ARG, "NULL argument");
     DevBuf tmp;
-    int rc = ensure(h, tmp, h->nvox * sizeof(float)); if (rc) return rc;
+    int rc = ensure(h, tmp, h->ncell * sizeof(float)); if (rc) return rc;
     float *d = tmp.as<float>();
     rc = vpmc_dose(h, n_histories, seed, d, nullptr);
     if (rc == VPMC_OK) {
-        cudaError_t e = cudaMemcpy(dose_out_host, d, h->nvox * sizeof(float), cudaMemcpyDeviceToHost);
+        cudaError_t e = cudaMemcpy(dose_out_host, d, h->ncell * sizeof(float), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { h->err = cudaGetErrorString(e); rc = VPMC_ERR_CUDA; }
     }
     pool_give(tmp.p, tmp.bytes);
@@ -338,10 +338,10 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     h->last_stream = caller;
     h->unc_valid = false; h->seq_valid = false;
     if (!h->d_s1) {
-        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->nvox * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->nvox * sizeof(float)))) return rc;
+        if ((rc = dev_alloc(h, (void **)&h->d_s1, h->ncell * sizeof(float))) || (rc = dev_alloc(h, (void **)&h->d_s2, h->ncell * sizeof(float)))) return rc;
     }
     ChunkBufs cb;
-    if ((rc = ensure(h, h->edep, (size_t)h->nvox * sizeof(float))) ||
+    if ((rc = ensure(h, h->edep, (size_t)h->ncell * sizeof(float))) ||
         (rc = ensure(h, h->cum, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) || (rc = ensure(h, h->first, ((size_t)h->n_spots + 1) * sizeof(unsigned long long))) ||
         (rc = chunk_buffers(h, batch_histories, cb))) return rc;
     // C2 for one batch: ids i in [0, N_b) contiguous per spot in spot order (the batch index goes into the id's high word)
@@ -351,9 +351,9 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     CU(h, cudaMemcpyAsync(h->cum.p, cum.data(), cum.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
     CU(h, cudaMemcpyAsync(h->first.p, first.data(), first.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
     CU(h, cudaStreamSynchronize(st));        // cum / first are stack vectors
-    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)h->nvox * sizeof(float), st));
-    CU(h, cudaMemsetAsync(h->d_s1, 0, (size_t)h->nvox * sizeof(float), st));
-    CU(h, cudaMemsetAsync(h->d_s2, 0, (size_t)h->nvox * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->edep.p, 0, (size_t)h->ncell * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_s1, 0, (size_t)h->ncell * sizeof(float), st));
+    CU(h, cudaMemsetAsync(h->d_s2, 0, (size_t)h->ncell * sizeof(float), st));
     CU(h, cudaMemsetAsync(h->d_tal, 0, sizeof(DevTallies), st));
     CU(h, cudaMemsetAsync(h->d_seq, 0, sizeof(SeqState), st));
 
@@ -362,8 +362,8 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     wm.mode = 0; wm.n_items = batch_histories; wm.cum = h->cum.as<unsigned long long>(); wm.first = h->first.as<unsigned long long>();
     wm.n_entries = h->n_spots; wm.n_spots = h->n_spots; wm.batch_hi = &h->d_seq->batch;
     ScoreArgs sa{};
-    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->nvox;
-    const int gv = grid_for(h->nvox, h->n_sm);
+    sa.edep = h->edep.as<float>(); sa.nvox = (unsigned long long)h->ncell; sa.sg = score_geom(h);
+    const int gv = grid_for(h->ncell, h->n_sm);
 
     // the graph: one WHILE node whose body is the batch pass
     CU(h, cudaGraphCreate(&h->seq_graph, 0));
@@ -378,8 +378,8 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     cudaGraph_t body = np.conditional.phGraph_out[0];
     CU(h, cudaStreamBeginCaptureToGraph(st, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
     enqueue_chunk<0>(h, c, wm, 0ull, cb, sa, h->d_tal, st, false);
-    seq_accumulate_kernel<<<gv, 256, 0, st>>>(h->edep.as<float>(), h->d_s1, h->d_s2, h->nvox, h->d_seq);
-    seq_uncertainty_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_s2, h->nvox, h->d_seq);
+    seq_accumulate_kernel<<<gv, 256, 0, st>>>(h->edep.as<float>(), h->d_s1, h->d_s2, h->ncell, h->d_seq);
+    seq_uncertainty_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_s2, h->ncell, h->d_seq);
     seq_decide_kernel<<<1, 1, 0, st>>>(handle, h->d_seq, (int)min_batches, (int)max_batches, target_rel_unc);
     cudaError_t ce = cudaStreamEndCapture(st, nullptr);
     if (ce != cudaSuccess) { cudaGetLastError(); seq_release(h); FAIL(h, VPMC_ERR_CUDA, "graph capture of the batch pass: %s", cudaGetErrorString(ce)); }
@@ -389,7 +389,7 @@ extern "C" int vpmc_dose_to_uncertainty(vpmc_t *h, const vpmc_scenario *scp, uin
     for (double x : h->spot_w) W += x;
     const double V = (double)h->G.hx * h->G.hy * h->G.hz * 1e-3;
     const float coef_batch = (float)(W / (double)batch_histories / V * 1.602176634e-10);
-    seq_finalize_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef_batch, h->d_seq, dose_out_dev, h->nvox);
+    seq_finalize_kernel<<<gv, 256, 0, st>>>(h->d_s1, h->d_hu, h->d_lut, h->G, h->params.rho_min, coef_batch, h->d_seq, dose_out_dev, h->ncell, h->d_cell_rho);
     CU(h, cudaGetLastError());
     CU(h, cudaEventRecord(h->seq_ev_out, st));
     CU(h, cudaStreamWaitEvent(caller, h->seq_ev_out, 0));

@@ -109,15 +109,17 @@ extern "C" int vpmc_gamma(vpmc_t *h, const float *ref_dev, const float *eval_dev
     cudaStream_t st = (cudaStream_t)cuda_stream;
     h->last_stream = st; h->launched = true;
     int rc;
-    const unsigned int cap = (unsigned int)std::min<long long>(h->nvox, 0x7fffffffLL);
+    const unsigned int cap = (unsigned int)std::min<long long>(h->ncell, 0x7fffffffLL);
     if ((rc = ensure(h, h->gamma_buf, sizeof(GammaCounts) + (size_t)cap * sizeof(unsigned int)))) return rc;
     GammaCounts *c = h->gamma_buf.as<GammaCounts>();
     unsigned int *list = reinterpret_cast<unsigned int *>(c + 1);
-    GammaArgs a = { h->G.nx, h->G.ny, h->G.nz, h->G.hx, h->G.hy, h->G.hz, dd_rel, dta_mm, threshold_rel, (int)sub };
+    // the grids are on the scoring grid: cells of sdiv voxels per axis
+    GammaArgs a = { h->sn[0], h->sn[1], h->sn[2], h->G.hx * (float)h->sdiv[0], h->G.hy * (float)h->sdiv[1], h->G.hz * (float)h->sdiv[2], dd_rel, dta_mm,
+                    threshold_rel, (int)sub };
     CU(h, cudaMemsetAsync(c, 0, sizeof(GammaCounts), st));
-    const int g = grid_for(h->nvox, h->n_sm);
-    gamma_max_kernel<<<g, 256, 0, st>>>(ref_dev, h->nvox, c);
-    gamma_select_kernel<<<g, 256, 0, st>>>(ref_dev, eval_dev, h->nvox, a, c, list, cap);
+    const int g = grid_for(h->ncell, h->n_sm);
+    gamma_max_kernel<<<g, 256, 0, st>>>(ref_dev, h->ncell, c);
+    gamma_select_kernel<<<g, 256, 0, st>>>(ref_dev, eval_dev, h->ncell, a, c, list, cap);
     gamma_search_kernel<<<h->n_sm * 8, 256, 0, st>>>(ref_dev, eval_dev, a, c, list, cap);
     CU(h, cudaGetLastError());
     h->launches += 3;
