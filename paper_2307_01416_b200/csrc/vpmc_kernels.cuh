@@ -105,17 +105,25 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
 
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
     ColumnBoxes cb; ScoreGeom sg;
-    __device__ __forceinline__ void begin(const Hist &) {}
+    // the history's column box, read once when the lane takes the history (three dependent loads per deposit otherwise:
+    // ncu long_scoreboard 2.2 against 0.5 in dose mode): low corner, extent, element offset of the box
+    int lx, ly, lz, dx, dy, dz;
+    unsigned long long off;
+    __device__ __forceinline__ void begin(const Hist &h)
+    {
+        const int4 lo = __ldg(cb.lo + h.col), dm = __ldg(cb.dim + h.col);
+        lx = lo.x; ly = lo.y; lz = lo.z; dx = dm.x; dy = dm.y; dz = dm.z;
+        off = __ldg(cb.offset + h.col);
+    }
     __device__ __forceinline__ void deposit(const Hist &h, float dep)
     {
-        const int c = h.col;
-        const int4 lo = __ldg(cb.lo + c), dm = __ldg(cb.dim + c);
         int sx, sy, sz;
         score_coords(sg, h, sx, sy, sz);
-        const int bx = sx - lo.x, by = sy - lo.y, bz = sz - lo.z;
-        if ((unsigned)bx < (unsigned)dm.x && (unsigned)by < (unsigned)dm.y && (unsigned)bz < (unsigned)dm.z)
-            atomicAdd(cb.scratch + __ldg(cb.offset + c) + (bx + (unsigned long long)dm.x * (by + (unsigned long long)dm.y * bz)), dep);
+        const int bx = sx - lx, by = sy - ly, bz = sz - lz;
+        if ((unsigned)bx < (unsigned)dx && (unsigned)by < (unsigned)dy && (unsigned)bz < (unsigned)dz)
+            atomicAdd(cb.scratch + off + (bx + (unsigned long long)dx * (by + (unsigned long long)dy * bz)), dep);
         else {
+            const int c = h.col;
             const unsigned slot = atomicAdd(cb.ovf_count, 1u);
             const unsigned int v = sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3;
             if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | v; cb.ovf_val[slot] = dep; }
@@ -148,7 +156,7 @@ struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; ScoreGe
 
 template <int MODE> __device__ __forceinline__ typename ScorerOf<MODE>::type make_scorer(const ScoreArgs &a);
 template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox, a.sg }; }
-template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { return BoxScorer{ a.cb, a.sg }; }
+template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { BoxScorer s; s.cb = a.cb; s.sg = a.sg; s.lx = s.ly = s.lz = 0; s.dx = s.dy = s.dz = 0; s.off = 0ull; return s; }
 template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; s.sg = a.sg; return s; }
 
 // ------------------------------------------------------------------------------------------- S1-S7
