@@ -213,7 +213,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     const float E = h.E;
     // 1
     const float R = (float)h.R;
-    if (h.R <= P.R_cut_d) { o.dep = E; o.s = 0.0f; h.E = 0.0f; h.R = 0.0; return STOPPED; }
+    if (__builtin_expect(h.R <= P.R_cut_d, 0)) { o.dep = E; o.s = 0.0f; h.E = 0.0f; h.R = 0.0; return STOPPED; }
     // 2
     float s = d; int face = 1;
     const float lim = fmaxf(P.f_R * R, P.R_cut) * m.inv_rsp;
@@ -224,7 +224,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     // non-positive range and the update R_next = R' (E'/Ebar)^p stays what it is everywhere else (R_next <= R_cut then: the
     // history stops at its next step).
     double Rp = fma(-f2d(s), f2d(m.rsp), h.R);
-    Rp = (Rp > 1e-12) ? Rp : 1e-12;
+    if (__builtin_expect(__double2hiint(Rp) < 0x3d719799, 0)) Rp = 1e-12;      // Rp < ~1e-12 (or negative): high word below that of 1e-12
     // E is re-derived from the fp64 range every step, so a 3e-7 relative MUFU error does not accumulate
     const float Ebar = exp2f(P.inv_p * __log2f((float)Rp * P.inv_alpha));
     // mean energy lost in the step.  E - Ebar cancels when the step is thin in water-equivalent terms (1 mm of air
@@ -263,7 +263,7 @@ __device__ __forceinline__ int step_physics(const DevParams &P, Hist &h, const M
     // 6
     if (flags & 4) {
         h.tau = fmaf(__fdividef(P.beta_nuc, fmaf(P.beta_nuc, R, 1.0f)) * m.rho_rel, s, h.tau);
-        if (h.tau >= h.tau_star) {
+        if (__builtin_expect(h.tau >= h.tau_star, 0)) {
             o.dep += P.gamma_loc * Ep;
             o.removed = (1.0f - P.gamma_loc) * Ep;
             h.E = Ep; h.R = Rn;

@@ -437,8 +437,8 @@ __device__ __forceinline__ int rs_iter(const Ctx &c, Hist &h, float &dep_rs, Lan
     const Medium m = { P.rs_rsp, P.rs_inv_rsp, P.rs_rho, P.rs_inv_X0, P.rs_za_rho };
     bool out;
     const int cause = slab_step<FL>(c, h, m, g, REG_RS, dep_rs, lc, tr, out);
-    if (cause != CONT) return (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
-    if (!out) return BEAM_CONT;
+    if (__builtin_expect(cause != CONT, 0)) return (cause == NUCLEAR) ? BEAM_NUCLEAR : BEAM_STOPPED;
+    if (__builtin_expect(!out, 1)) return BEAM_CONT;
     h.region = (__ldg(&bp->has_ap) ? REG_TO_AP : REG_TO_CT) | (h.region & ~0xff);
     return BEAM_EXIT;
 }
