@@ -346,6 +346,8 @@ int vpmc_digests(vpmc_t *h, const vpmc_scenario *sc, uint64_t n_histories, uint6
 #define VPMC_KNOB_OVF_CAP 3      /* influence: capacity of the overflow list (default 2^25; 0 forces the replay path) */
 #define VPMC_KNOB_LUT_GLOBAL 4   /* 1 = never stage the material table in shared memory */
 #define VPMC_KNOB_VERBOSE 5      /* 1 = progress lines of the influence path on stderr */
+#define VPMC_KNOB_OVF_SORT_CAP 6 /* influence: overflow entries of ONE column a CTA sorts (default and maximum 16384); a column with more
+                                    is replayed with a larger box */
 int vpmc_set_knob(vpmc_t *h, int knob, double value);
 
 /* Per-kernel-class device timing (bench.py's roofline): when on, every launch is bracketed by CUDA events on its

@@ -9,8 +9,6 @@
 #include <mutex>
 #include <numeric>
 
-#include <cub/cub.cuh>
-
 #include "vpmc_host.h"
 #include "vpmc_setup.cuh"
 
@@ -197,7 +195,7 @@ extern "C" int vpmc_destroy(vpmc_t *h)
     DevBuf *bufs[] = { &h->cum, &h->first, &h->edep, &h->s0, &h->s1, &h->s2, &h->a0, &h->a1, &h->a2, &h->a3, &h->a4, &h->b0, &h->b1, &h->b2, &h->b3, &h->b4, &h->b5, &h->q0, &h->q1, &h->q2, &h->q3, &h->q4, &h->inf_scratch, &h->inf_lo, &h->inf_dim, &h->inf_off, &h->inf_bbox, &h->inf_cols,
                        &h->inf_tile0, &h->inf_tilecol, &h->inf_skip, &h->inf_tilecnt, &h->inf_colmax, &h->inf_colnnz, &h->inf_colbase,
                        &h->inf_stage_idx, &h->inf_stage_val, &h->inf_rowsrc, &h->ovf_key, &h->ovf_val, &h->ovf_key2, &h->ovf_val2, &h->ovf_flag,
-                       &h->ovf_colcnt, &h->ovf_ctr, &h->cub_temp, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part, &h->gamma_buf };
+                       &h->ovf_colcnt, &h->ovf_coloff, &h->ovf_kept, &h->ovf_ctr, &h->ostage_idx, &h->ostage_val, &h->row_ovf_off, &h->row_ovf_n, &h->spmv_part, &h->gamma_buf };
     for (DevBuf *b : bufs) if (b->p) { pool_give(b->p, b->bytes); b->p = nullptr; }
     delete h;
     return VPMC_OK;
@@ -617,6 +615,9 @@ extern "C" int vpmc_set_knob(vpmc_t *h, int knob, double value)
     case VPMC_KNOB_OVF_CAP:
         if (!(value >= 0.0 && value <= 268435456.0)) FAIL(h, VPMC_ERR_INVALID_ARG, "overflow capacity must be in [0, 2^28]");
         h->ovf_cap = (unsigned int)value; break;
+    case VPMC_KNOB_OVF_SORT_CAP:
+        if (!(value >= 1.0 && value <= (double)kOvfSortCap)) FAIL(h, VPMC_ERR_INVALID_ARG, "overflow sort capacity must be in [1, %d]", kOvfSortCap);
+        h->ovf_sort_cap = (unsigned int)value; break;
     case VPMC_KNOB_LUT_GLOBAL:
         h->smem_lut = (value == 0.0) && h->lut_bytes <= kMaxSmemLut; break;
     case VPMC_KNOB_VERBOSE:

@@ -101,7 +101,7 @@ struct vpmc {
     // influence workspace (grown on demand)
     DevBuf inf_scratch, inf_lo, inf_dim, inf_off, inf_bbox, inf_cols, inf_tile0, inf_tilecol, inf_skip, inf_tilecnt, inf_colmax,
         inf_colnnz, inf_colbase, inf_stage_idx, inf_stage_val, inf_rowsrc,
-        ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_ctr, cub_temp, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
+        ovf_key, ovf_val, ovf_key2, ovf_val2, ovf_flag, ovf_colcnt, ovf_coloff, ovf_kept, ovf_ctr, ostage_idx, ostage_val, row_ovf_off, row_ovf_n;
     vpmc_influence_stats inf_stats = {};
     DevBuf gamma_buf;                 // counters + list of the voxels that fail the zero-distance test (vpmc_gamma)
     DevBuf spmv_part;                 // first / last partial sums per chunk of vpmc_spmv_grad
@@ -112,6 +112,7 @@ struct vpmc {
     float box_grow = 0.05f;           // influence: growth of the pilot box, fraction of its extent
     int box_pad = 1;                  // influence: extra voxels per side
     unsigned int ovf_cap = 1u << 25;  // influence: entries of the overflow list (12 B each)
+    unsigned int ovf_sort_cap = vpk::kOvfSortCap;   // influence: overflow entries of one column beyond which the column is replayed
     bool verbose = false;
 
     // launch configuration

@@ -6,9 +6,9 @@
 //      (tight on purpose: the overflow list of step 4 takes the halo, and every box element is zeroed and scanned);
 //   3. columns are packed into groups whose boxes fit the workspace; per group: zero the boxes, transport all
 //      hist_per_spot histories of the group's spots in MODE 1, then max / count / scan / emit into a staging area;
-//   4. deposits outside a column's box go to an overflow list of (column, voxel, MeV) entries, which is sorted, summed
-//      per voxel, thresholded with the column and merged into the row at the end.  Only when that list is full is a
-//      column NOT written: its box is replaced by the union with the bounding box of the lost deposits and the column is
+//   4. deposits outside a column's box go to an overflow list of (column, voxel, MeV) entries, which is bucketed by column,
+//      sorted by voxel and summed per voxel by one CTA per column, thresholded with the column and merged into the row at
+//      the end.  Only when that list is full (or a column's bucket exceeds what a CTA sorts) is a column NOT written: its box is replaced by the union with the bounding box of the lost deposits and the column is
 //      replayed in a later group -- streams are keyed by history id, so the replay reproduces the same histories and
 //      now fits by construction;
 //   5. row_ptr = exclusive scan of the row counts; the caller's allocator provides row_ptr / col / val and the rows are
@@ -223,7 +223,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 ColumnBoxes cb{};
                 cb.lo = h->inf_lo.as<int4>(); cb.dim = h->inf_dim.as<int4>(); cb.offset = h->inf_off.as<unsigned long long>();
                 cb.scratch = h->inf_scratch.as<float>(); cb.bbox = h->inf_bbox.as<int>();
-                // overflow list: deposits outside the boxes (ovf_ctr: [0] entries appended, [1] unique entries, [2] kept entries)
+                // overflow list: deposits outside the boxes (ovf_ctr[0]: entries appended)
                 if ((rc = ensure(h, h->ovf_key, (size_t)ovf_cap * 8 + 8)) || (rc = ensure(h, h->ovf_val, (size_t)ovf_cap * 4 + 4)) ||
                     (rc = ensure(h, h->ovf_ctr, 4 * sizeof(int)))) return rc;
                 CU(h, cudaMemsetAsync(h->ovf_ctr.p, 0, 4 * sizeof(int), st));
@@ -245,6 +245,28 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 CU(h, cudaStreamSynchronize(st));
                 n_ovf = std::min(n_ovf, ovf_cap);
                 h->inf_stats.ovf_deposits += n_ovf;
+                // overflow entries per column; a column with more than a CTA sorts is treated like one that lost deposits
+                std::vector<unsigned int> ovf_cnt(nc, 0u), ovf_off(nc, 0u);
+                if (n_ovf > 0) {
+                    if ((rc = ensure(h, h->ovf_colcnt, (size_t)nc * 4)) || (rc = ensure(h, h->ovf_flag, (size_t)nc * 4)) || (rc = ensure(h, h->ovf_kept, (size_t)nc * 4))) return rc;
+                    const int g1 = std::max(1, std::min((int)((n_ovf + 255) / 256), h->n_sm * 8));
+                    CU(h, cudaMemsetAsync(h->ovf_colcnt.p, 0, (size_t)nc * 4, st));
+                    ovf_hist_kernel<<<g1, 256, 0, st>>>(h->ovf_key.as<unsigned long long>(), n_ovf, h->ovf_colcnt.as<unsigned int>());
+                    h->launches += 1;
+                    CU(h, cudaMemcpyAsync(ovf_cnt.data(), h->ovf_colcnt.p, (size_t)nc * 4, cudaMemcpyDeviceToHost, st));
+                    CU(h, cudaStreamSynchronize(st));
+                    std::vector<int> big(nc, 0);
+                    bool any_big = false;
+                    unsigned int run = 0;
+                    for (int c = 0; c < nc; ++c) { ovf_off[c] = run; run += ovf_cnt[c]; if (ovf_cnt[c] > h->ovf_sort_cap) { big[c] = 1; any_big = true; } }
+                    if (any_big) {
+                        rc = upload(h, h->inf_skip, big, st); if (rc) return rc;
+                        ovf_bbox_kernel<<<g1, 256, 0, st>>>(h->ovf_key.as<unsigned long long>(), n_ovf, h->inf_skip.as<int>(), h->sn[0], h->sn[1], h->inf_bbox.as<int>());
+                        h->launches += 1;
+                        CU(h, cudaMemcpyAsync(obb.data(), h->inf_bbox.p, obb.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
+                        CU(h, cudaStreamSynchronize(st));
+                    }
+                }
                 std::vector<int> skip(nc, 0);
                 for (int c = 0; c < nc; ++c)
                     if (obb[6 * c + 3] >= 0) {
@@ -269,35 +291,27 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 }
                 rc = csr_max_pass(h, cc, cb.scratch, true, coef, st); if (rc) return rc;
                 std::vector<unsigned int> ocnt(nc, 0u);
-                int n_sel = 0;
                 if (n_ovf > 0) {
-                    // sort by (column, voxel), sum duplicates, convert, threshold against the column maximum, compact
-                    if ((rc = ensure(h, h->ovf_key2, (size_t)n_ovf * 8)) || (rc = ensure(h, h->ovf_val2, (size_t)n_ovf * 4)) ||
-                        (rc = ensure(h, h->ovf_flag, (size_t)n_ovf)) || (rc = ensure(h, h->ovf_colcnt, (size_t)nc * 4))) return rc;
-                    unsigned long long *k1 = h->ovf_key.as<unsigned long long>(), *k2 = h->ovf_key2.as<unsigned long long>();
-                    float *v1 = h->ovf_val.as<float>(), *v2 = h->ovf_val2.as<float>();
-                    int *ctr = h->ovf_ctr.as<int>();
-                    size_t t1 = 0, t2 = 0, t3 = 0;
-                    cub::DeviceRadixSort::SortPairs(nullptr, t1, k1, k2, v1, v2, (int)n_ovf, 0, 56, st);
-                    cub::DeviceReduce::ReduceByKey(nullptr, t2, k2, k1, v2, v1, ctr + 1, cub::Sum(), (int)n_ovf, st);
-                    cub::DeviceSelect::Flagged(nullptr, t3, k1, h->ovf_flag.as<unsigned char>(), k2, ctr + 2, (int)n_ovf, st);
-                    size_t tb = std::max(t1, std::max(t2, t3));
-                    rc = ensure(h, h->cub_temp, tb); if (rc) return rc;
+                    // bucket by column, then one CTA per column: sort by cell, sum per cell, convert, column maximum, threshold,
+                    // kept pairs written at the start of the column's stretch of the overflow staging (vpmc_kernels.cuh)
+                    if ((rc = ensure(h, h->ovf_key2, (size_t)n_ovf * 4)) || (rc = ensure(h, h->ovf_val2, (size_t)n_ovf * 4)) ||
+                        (rc = grow_keep(h, h->ostage_idx, (size_t)(ostaged + n_ovf) * sizeof(int), (size_t)ostaged * sizeof(int), st)) ||
+                        (rc = grow_keep(h, h->ostage_val, (size_t)(ostaged + n_ovf) * sizeof(float), (size_t)ostaged * sizeof(float), st)) ||
+                        (rc = upload(h, h->ovf_coloff, ovf_off, st))) return rc;
+                    static bool smem_set = false;
+                    if (!smem_set) { CU(h, cudaFuncSetAttribute(ovf_columns_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kOvfSortCap * 8)); smem_set = true; }
                     TimedScope ts(h, st, 3);
-                    CU(h, cub::DeviceRadixSort::SortPairs(h->cub_temp.p, tb, k1, k2, v1, v2, (int)n_ovf, 0, 56, st));
-                    CU(h, cub::DeviceReduce::ReduceByKey(h->cub_temp.p, tb, k2, k1, v2, v1, ctr + 1, cub::Sum(), (int)n_ovf, st));
                     const int g1 = std::max(1, std::min((int)((n_ovf + 255) / 256), h->n_sm * 8));
-                    ovf_convert_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>(), h->d_cell_rho);
-                    CU(h, cudaMemsetAsync(h->ovf_colcnt.p, 0, (size_t)nc * 4, st));
-                    CU(h, cudaMemsetAsync(h->ovf_flag.p, 0, (size_t)n_ovf, st));
-                    ovf_flag_kernel<<<g1, 256, 0, st>>>(k1, v1, ctr + 1, h->inf_colmax.as<unsigned int>(), h->inf_skip.as<int>(), rel_threshold,
-                                                       h->ovf_flag.as<unsigned char>(), h->ovf_colcnt.as<unsigned int>());
-                    CU(h, cub::DeviceSelect::Flagged(h->cub_temp.p, tb, k1, h->ovf_flag.as<unsigned char>(), k2, ctr + 2, (int)n_ovf, st));
-                    CU(h, cub::DeviceSelect::Flagged(h->cub_temp.p, tb, v1, h->ovf_flag.as<unsigned char>(), v2, ctr + 3, (int)n_ovf, st));
+                    CU(h, cudaMemsetAsync(h->ovf_flag.p, 0, (size_t)nc * 4, st));                // cursors
+                    ovf_scatter_kernel<<<g1, 256, 0, st>>>(h->ovf_key.as<unsigned long long>(), h->ovf_val.as<float>(), n_ovf, h->ovf_coloff.as<unsigned int>(),
+                                                          h->ovf_flag.as<unsigned int>(), h->ovf_key2.as<unsigned int>(), h->ovf_val2.as<float>());
+                    ovf_columns_kernel<<<nc, kOvfBlock, kOvfSortCap * 8, st>>>(h->ovf_key2.as<unsigned int>(), h->ovf_val2.as<float>(), h->ovf_coloff.as<unsigned int>(),
+                                                                           h->ovf_colcnt.as<unsigned int>(), h->inf_skip.as<int>(), h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut,
+                                                                           h->params.rho_min, coef, h->d_cell_rho, rel_threshold, h->inf_colmax.as<unsigned int>(),
+                                                                           h->ostage_idx.as<int>() + ostaged, h->ostage_val.as<float>() + ostaged, h->ovf_kept.as<unsigned int>(), h->ovf_sort_cap);
                     CU(h, cudaGetLastError());
-                    h->launches += 8;
-                    CU(h, cudaMemcpyAsync(ocnt.data(), h->ovf_colcnt.p, (size_t)nc * 4, cudaMemcpyDeviceToHost, st));
-                    CU(h, cudaMemcpyAsync(&n_sel, ctr + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
+                    h->launches += 2;
+                    CU(h, cudaMemcpyAsync(ocnt.data(), h->ovf_kept.p, (size_t)nc * 4, cudaMemcpyDeviceToHost, st));
                 }
                 rc = csr_count_pass(h, cc, cb.scratch, rel_threshold, st); if (rc) return rc;
                 std::vector<long long> nnz(nc), base(nc);
@@ -308,19 +322,11 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     base[c] = staged + add;
                     if (!skip[c]) {
                         row_nnz[cols[c]] = nnz[c] + ocnt[c]; row_src[cols[c]] = base[c]; add += nnz[c];
-                        row_ovf_off[cols[c]] = ostaged + oadd; row_ovf_n[cols[c]] = (int)ocnt[c]; oadd += ocnt[c];
+                        row_ovf_off[cols[c]] = ostaged + (long long)(n_ovf > 0 ? ovf_off[c] : 0u); row_ovf_n[cols[c]] = (int)ocnt[c]; oadd += ocnt[c];
                     }
                 }
-                if (oadd != n_sel) FAIL(h, VPMC_ERR_STATE, "influence: overflow bookkeeping mismatch (%lld vs %d)", oadd, n_sel);
-                if (oadd > 0) {       // the kept overflow entries, sorted by (column, voxel), join the persistent overflow staging
-                    if ((rc = grow_keep(h, h->ostage_idx, (size_t)(ostaged + oadd) * sizeof(int), (size_t)ostaged * sizeof(int), st)) ||
-                        (rc = grow_keep(h, h->ostage_val, (size_t)(ostaged + oadd) * sizeof(float), (size_t)ostaged * sizeof(float), st))) return rc;
-                    ovf_split_keys_kernel<<<std::max(1, std::min((int)((oadd + 255) / 256), h->n_sm * 8)), 256, 0, st>>>(h->ovf_key2.as<unsigned long long>(), (int)oadd, h->ostage_idx.as<int>() + ostaged);
-                    CU(h, cudaMemcpyAsync(h->ostage_val.as<float>() + ostaged, h->ovf_val2.p, (size_t)oadd * sizeof(float), cudaMemcpyDeviceToDevice, st));
-                    h->launches += 1;
-                    ostaged += oadd;
-                    h->inf_stats.ovf_kept += (uint64_t)oadd;
-                }
+                if (n_ovf > 0) ostaged += n_ovf;          // a column's kept pairs sit at the start of its bucket's stretch
+                h->inf_stats.ovf_kept += (uint64_t)oadd;
                 if (h->verbose) fprintf(stderr, "[vpmc]   group of %d columns: %u outside deposits, %lld kept entries of them, %lld box entries\n", nc, n_ovf, oadd, add);
                 if (add > 0) {
                     if ((rc = grow_keep(h, h->inf_stage_idx, (size_t)(staged + add) * sizeof(int), (size_t)staged * sizeof(int), st)) ||

@@ -1082,38 +1082,113 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
     }
 }
 
-// ---- overflow list (deposits outside a column's box), after sort + reduce-by-key: unique (column << 32 | voxel, MeV)
-// E_dep -> dose value, in place; the column maximum takes these entries into account
-__global__ void ovf_convert_kernel(const unsigned long long *__restrict__ key, float *__restrict__ val, const int *__restrict__ n_ptr,
-                                   const short *__restrict__ hu, const float4 *__restrict__ lut, int hu_min, int n_lut,
-                                   float rho_min, float coef, unsigned int *__restrict__ colmax_bits, const float *__restrict__ cell_rho)
+// ---- overflow list (deposits outside a column's box): (column << 32 | cell, MeV) entries in arrival order.  They are
+// bucketed by column (count -> offsets on the host -> scatter through a cursor per column), and then ONE CTA per column sorts
+// its bucket by cell in shared memory, sums the deposits of a cell, converts to dose, folds the values into the column
+// maximum, thresholds and writes the kept (cell, value) pairs, ascending, at the start of the column's own stretch of the
+// staging arrays -- all hand-written; a bucket larger than kOvfSortCap is not handled here: the column is replayed with a
+// larger box (the host sees the counts).
+constexpr int kOvfSortCap = 16384;        // entries a CTA sorts in shared memory (128 KB)
+constexpr int kOvfBlock = 1024;
+
+__global__ void ovf_hist_kernel(const unsigned long long *__restrict__ key, unsigned int n, unsigned int *__restrict__ col_cnt)
 {
-    const int n = *n_ptr;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) atomicAdd(col_cnt + (unsigned)(key[i] >> 32), 1u);
+}
+
+// bounding box (scoring-grid coordinates) of the overflow entries of the columns flagged in `lost`
+__global__ void ovf_bbox_kernel(const unsigned long long *__restrict__ key, unsigned int n, const int *__restrict__ lost, int snx, int sny, int *__restrict__ bbox)
+{
+    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const unsigned c = (unsigned)(key[i] >> 32), v = (unsigned)key[i];
+        if (!__ldg(lost + c)) continue;
+        const int z = (int)(v / (unsigned)(snx * sny)), rem = (int)(v - (unsigned)z * (unsigned)(snx * sny)), y = rem / snx, x = rem - y * snx;
+        bbox_merge(bbox + 6 * c, x, y, z, x, y, z);
+    }
+}
+
+__global__ void ovf_scatter_kernel(const unsigned long long *__restrict__ key, const float *__restrict__ val, unsigned int n,
+                                   const unsigned int *__restrict__ col_off, unsigned int *__restrict__ cursor, unsigned int *__restrict__ b_cell,
+                                   float *__restrict__ b_val)
+{
+    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const unsigned long long k = key[i];
-        const float x = __fdiv_rn(coef * val[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, (long long)(unsigned)k));
-        val[i] = x;
-        if (x > 0.0f) atomicMax(colmax_bits + (unsigned)(k >> 32), __float_as_uint(x));
+        const unsigned c = (unsigned)(k >> 32);
+        const unsigned pos = __ldg(col_off + c) + atomicAdd(cursor + c, 1u);
+        b_cell[pos] = (unsigned)k; b_val[pos] = val[i];
     }
 }
 
-// keep flags of the unique overflow entries and kept entries per column
-__global__ void ovf_flag_kernel(const unsigned long long *__restrict__ key, const float *__restrict__ val, const int *__restrict__ n_ptr,
-                                const unsigned int *__restrict__ colmax_bits, const int *__restrict__ skip, float rel_thr,
-                                unsigned char *__restrict__ flag, unsigned int *__restrict__ col_cnt)
+// one CTA per column
+__global__ void __launch_bounds__(kOvfBlock)
+ovf_columns_kernel(const unsigned int *__restrict__ b_cell, const float *__restrict__ b_val, const unsigned int *__restrict__ col_off,
+                   const unsigned int *__restrict__ col_cnt, const int *__restrict__ skip, const short *__restrict__ hu, const float4 *__restrict__ lut,
+                   int hu_min, int n_lut, float rho_min, float coef, const float *__restrict__ cell_rho, float rel_thr,
+                   unsigned int *__restrict__ colmax_bits, int *__restrict__ out_idx, float *__restrict__ out_val, unsigned int *__restrict__ kept_cnt,
+                   unsigned int sort_cap)
 {
-    const int n = *n_ptr;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const unsigned c = (unsigned)(key[i] >> 32);
-        const bool keep = !__ldg(skip + c) && csr_keep(val[i], rel_thr * __uint_as_float(__ldg(colmax_bits + c)));
-        flag[i] = keep ? 1 : 0;
-        if (keep) atomicAdd(col_cnt + c, 1u);
+    extern __shared__ unsigned int ovf_smem[];
+    unsigned int *key = ovf_smem;
+    float *val = reinterpret_cast<float *>(ovf_smem + kOvfSortCap);
+    __shared__ unsigned int s_warp[kOvfBlock / 32];
+    __shared__ unsigned int s_max, s_carry;
+    const int c = blockIdx.x;
+    const unsigned int n = __ldg(col_cnt + c), off = __ldg(col_off + c);
+    if (threadIdx.x == 0) kept_cnt[c] = 0u;
+    if (n == 0u || n > sort_cap || __ldg(skip + c)) return;
+    unsigned int P = 1u;
+    while (P < n) P <<= 1;
+    for (unsigned int i = threadIdx.x; i < P; i += kOvfBlock) { key[i] = (i < n) ? b_cell[off + i] : 0xffffffffu; val[i] = (i < n) ? b_val[off + i] : 0.0f; }
+    __syncthreads();
+    // bitonic sort by cell
+    for (unsigned int k = 2; k <= P; k <<= 1)
+        for (unsigned int j = k >> 1; j > 0; j >>= 1) {
+            for (unsigned int i = threadIdx.x; i < P; i += kOvfBlock) {
+                const unsigned int l = i ^ j;
+                if (l > i) {
+                    const unsigned int a = key[i], b = key[l];
+                    if ((a > b) == ((i & k) == 0u)) { key[i] = b; key[l] = a; const float t = val[i]; val[i] = val[l]; val[l] = t; }
+                }
+            }
+            __syncthreads();
+        }
+    // the first entry of every cell sums the cell's deposits and converts them to dose; the others are marked
+    if (threadIdx.x == 0) { s_max = __ldg(colmax_bits + c); s_carry = 0u; }
+    __syncthreads();
+    float mx = 0.0f;
+    for (unsigned int i = threadIdx.x; i < n; i += kOvfBlock) {
+        const unsigned int v = key[i];
+        if (i > 0 && key[i - 1] == v) continue;
+        float sum = val[i];
+        for (unsigned int l = i + 1; l < n && key[l] == v; ++l) sum += val[l];
+        const float x = __fdiv_rn(coef * sum, score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, (long long)v));
+        mx = fmaxf(mx, x);
+        val[i] = x;                                       // (heads only read their own run: no other thread reads val[i] as a head's input)
     }
-}
-
-__global__ void ovf_split_keys_kernel(const unsigned long long *__restrict__ key, int n, int *__restrict__ vox)
-{
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) vox[i] = (int)(unsigned)key[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0 && mx > 0.0f) atomicMax(&s_max, __float_as_uint(mx));
+    __syncthreads();
+    const unsigned int cm = s_max;
+    if (threadIdx.x == 0) colmax_bits[c] = cm;
+    const float thr = rel_thr * __uint_as_float(cm);
+    // keep and compact, in cell order
+    for (unsigned int base = 0; base < n; base += kOvfBlock) {
+        const unsigned int i = base + threadIdx.x;
+        const bool head = i < n && (i == 0 || key[i - 1] != key[i]);
+        const bool keep = head && csr_keep(val[i], thr);
+        const unsigned int bal = __ballot_sync(0xffffffffu, keep);
+        if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = __popc(bal);
+        __syncthreads();
+        unsigned int woff = 0, tot = 0;
+        for (int w = 0; w < kOvfBlock / 32; ++w) { const unsigned int t = s_warp[w]; if (w < (int)(threadIdx.x >> 5)) woff += t; tot += t; }
+        const unsigned int carry = s_carry;
+        if (keep) { const unsigned int pos = off + carry + woff + __popc(bal & lanemask_lt()); out_idx[pos] = (int)key[i]; out_val[pos] = val[i]; }
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry = carry + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) kept_cnt[c] = s_carry;
 }
 
 // final assembly: row r = merge of its staged box entries (a) and its kept overflow entries (b), both ascending in voxel

@@ -221,10 +221,13 @@ def test_influence_groups_and_replay_give_the_same_matrix(bind):
     overflow, p_ovf = run()                             # tight boxes: the overflow list fills the rows
     eng.set_knob(bind.KNOB_OVF_CAP, 0)                  # no list: the replay path
     replay, p_replay = run()
-    assert p_base == 2 and p_small == 1 + eng.n_spots and p_ovf == 2 and p_replay == 3, (p_base, p_small, p_ovf, p_replay)
+    eng.set_knob(bind.KNOB_OVF_CAP, 1 << 25); eng.set_knob(bind.KNOB_OVF_SORT_CAP, 8)      # a list, but buckets of more than 8 entries
+    bucket, p_bucket = run()                            # per column are not sorted: those columns are replayed with a larger box
+    eng.set_knob(bind.KNOB_OVF_SORT_CAP, 16384)
+    assert p_base == 2 and p_small == 1 + eng.n_spots and p_ovf == 2 and p_replay == 3 and p_bucket >= 3, (p_base, p_small, p_ovf, p_replay, p_bucket)
     # the same histories in another launch order: identical structure up to entries at the threshold, values to fp32 sums
     none = np.zeros(eng.nvox, dtype=bool); zero = np.zeros(eng.nvox)
-    for other in (small, overflow, replay):
+    for other in (small, overflow, replay, bucket):
         check_csr_structure(*other, eng.n_spots, eng.nvox)
         for g in range(eng.n_spots):
             dense = np.zeros(eng.nvox, dtype=np.float32)
