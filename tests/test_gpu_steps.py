@@ -115,13 +115,19 @@ def build_states(bind, O, w, pb, recs, hids, N):
 
 @pytest.mark.parametrize("case", list(STEP_CASES))
 def test_every_step_from_the_oracles_state(bind, case):
-    O = orc()
-    w = STEP_CASES[case]()
-    seed = 1
     N = 20000 if case not in ("config3",) else 10_000_000
     n_tr = 1024 if case != "config3" else 512
-    eng = bind.Engine(w)
-    pb = oracle_problem(w)
+    check_every_step(bind, STEP_CASES[case](), case, N, n_tr)
+
+
+def check_every_step(bind, w, case, N, n_tr, params_kw=None):
+    """Every step of n_tr traced oracle histories replayed from the oracle's pre-step state; params_kw = non-default
+    parameters given to both sides."""
+    O = orc()
+    seed = 1
+    kw = params_kw or {}
+    eng = bind.Engine(w, bind.default_params(**kw))
+    pb = oracle_problem(w, params=O.default_params(**kw))
     hids = (np.arange(n_tr, dtype=np.uint64) * np.uint64(N // n_tr))
     recs = O.trace(pb, hids, N, seed, max_steps=1200)
     states, exp = build_states(bind, O, w, pb, recs, hids, N)
