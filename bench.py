@@ -552,7 +552,7 @@ def measure_influence(hps, steps, warmup):
                       "unit": "GB/s", "frac": alg / wr_s / 1e9 / hbm_gbs if wr_s > 0 else None,
                       "bytes_as_implemented": impl, "achieved_as_implemented": impl / wr_s / 1e9 if wr_s > 0 else None,
                       "note": "algorithmic = 8 B x nnz written + 3 reads x 4 B of every box element (max, count, emit); the class also times the "
-                              "library sort of the overflow list", "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"},
+                              "overflow-list kernels", "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"},
            "optimiser_iteration": opt,
            "paper_context": "41.6 s for 13 influence matrices (P:L205-207): other data, other hardware"}
     eng.close()
