@@ -43,7 +43,7 @@ struct PoolEntry { void *p; size_t bytes; int device; };
 std::mutex g_pool_mu;
 std::vector<PoolEntry> g_pool;
 size_t g_pool_bytes = 0;
-constexpr size_t kPoolLimit = (size_t)6 << 30;
+constexpr size_t kPoolLimit = (size_t)16 << 30;
 
 int current_device() { int d = 0; cudaGetDevice(&d); return d; }
 
@@ -51,9 +51,11 @@ void *pool_take(size_t want, size_t &got)
 {
     const int dev = current_device();
     std::lock_guard<std::mutex> lk(g_pool_mu);
+    // best fit; a buffer of up to 16x the size asked for is still better than a cudaMalloc (tens of ms for the record
+    // queues of a plan whose beam line differs from the previous plans')
     int best = -1;
     for (int i = 0; i < (int)g_pool.size(); ++i)
-        if (g_pool[i].device == dev && g_pool[i].bytes >= want && g_pool[i].bytes <= 2 * want + 4096 && (best < 0 || g_pool[i].bytes < g_pool[best].bytes)) best = i;
+        if (g_pool[i].device == dev && g_pool[i].bytes >= want && g_pool[i].bytes <= 16 * want + 4096 && (best < 0 || g_pool[i].bytes < g_pool[best].bytes)) best = i;
     if (best < 0) return nullptr;
     void *p = g_pool[best].p; got = g_pool[best].bytes;
     g_pool_bytes -= got;
