@@ -266,6 +266,21 @@ int vpmc_robust_iteration(vpmc_t *h, const vpmc_csr *mats, int32_t n_sc, int64_t
                           const float *weight_dev, float *doses_ws_dev, float *resid_ws_dev, float *grad_dev, double *objective_dev,
                           void *cuda_stream);
 
+/* The one entry point that allocates nothing -- for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  vpmc_spmv_grad_static computes exactly what vpmc_spmv_grad computes, with the same
+ * two kernels in the same order (bit-identical result), but its scratch -- two partial sums per chunk of 8192 entries -- is a
+ * file-scope device array of the library instead of a buffer from the cache: no cudaMalloc, cudaFree, event creation or other
+ * allocating call happens inside it, under any input.  The array holds VPMC_STATIC_MAX_NNZ entries' worth of chunks = 256 KB,
+ * and every GPU that loads the library keeps those 256 KB until the process exits.  Its device address is looked up once per
+ * device in vpmc_create (cudaGetSymbolAddress, with the handle's device current); if that failed, this call returns
+ * VPMC_ERR_CUDA with the reason.  m->nnz > VPMC_STATIC_MAX_NNZ is rejected with VPMC_ERR_INVALID_ARG (use vpmc_spmv_grad).
+ * ALL calls on a device share the one array, from any handle and any stream: calls that overlap on the GPU race on it and give
+ * wrong sums -- enqueue them on one stream, or order them with events.  The array keeps the last call's contents; nothing in
+ * it has to start at zero (every partial sum that is read is written earlier in the same call), so nothing is cleared.
+ * m, r_dev, grad_dev as for vpmc_spmv_grad, all [device], caller-owned.  Not covered by vpmc_get_timing. */
+#define VPMC_STATIC_MAX_NNZ (1LL << 28)
+int vpmc_spmv_grad_static(vpmc_t *h, const vpmc_csr *m, const float *r_dev, float *grad_dev, int accumulate, void *cuda_stream);
+
 /* S:8f-3: 3-D gamma index of two dose grids on this engine's CT grid ("3D Gamma passing rate", Table 2; ref. 80),
  * computed on the device.  S:8c-C6: global normalisation -- dose criterion dd_rel x max(ref); voxels with ref >= threshold_rel
  * x max(ref) are evaluated; a voxel passes if |eval - ref| <= criterion at zero distance, else if min over the lattice points

@@ -23,10 +23,11 @@ EXPORTS = ["vpmc_version", "vpmc_default_params", "vpmc_create", "vpmc_destroy",
            "vpmc_get_uncertainty", "vpmc_trace", "vpmc_get_launch_count", "vpmc_last_error", "vpmc_set_timing",
            "vpmc_get_timing", "vpmc_set_workspace_limit", "vpmc_step_from_state", "vpmc_set_knob", "vpmc_digests", "vpmc_dose_to_uncertainty",
            "vpmc_get_run_info", "vpmc_bench_red", "vpmc_get_aperture_tables", "vpmc_set_shard", "vpmc_get_influence_stats", "vpmc_spmv_dose", "vpmc_spmv_grad",
-           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_set_aperture_polygon", "vpmc_gamma", "vpmc_set_scoring_grid",
+           "vpmc_worst_case", "vpmc_robust_iteration", "vpmc_spmv_grad_static", "vpmc_set_aperture_polygon", "vpmc_gamma", "vpmc_set_scoring_grid",
            "vpmc_get_scoring_dims"]
 
 STEP_SOURCE, STEP_DRIFT_TO_RS, STEP_RS, STEP_DRIFT_TO_AP, STEP_AP, STEP_CT_ENTRY, STEP_CT = range(7)
+STATIC_MAX_NNZ = 1 << 28          # VPMC_STATIC_MAX_NNZ
 KNOB_CHUNK, KNOB_BOX_GROW, KNOB_BOX_PAD, KNOB_OVF_CAP, KNOB_LUT_GLOBAL, KNOB_VERBOSE, KNOB_OVF_SORT_CAP = range(7)
 
 
@@ -148,6 +149,7 @@ def lib():
         L.vpmc_get_influence_stats.argtypes = [C.c_void_p, C.POINTER(InfluenceStats)]
         L.vpmc_spmv_dose.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vpmc_spmv_grad.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.vpmc_spmv_grad_static.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.vpmc_worst_case.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vpmc_robust_iteration.argtypes = [C.c_void_p, C.POINTER(_Csr), C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -407,6 +409,17 @@ class Engine:
         assert r.is_cuda and r.dtype == torch.float32 and r.is_contiguous() and out.numel() == c.n_rows
         st = torch.cuda.current_stream() if stream is None else stream
         self._check(lib().vpmc_spmv_grad(self._h, C.byref(c), r.data_ptr(), out.data_ptr(), 1 if accumulate else 0, st.cuda_stream))
+        return out
+
+    def spmv_grad_static(self, m, r, out, accumulate: bool = False, stream=None):
+        """vpmc_spmv_grad_static: spmv_grad with the library's static scratch -- no device allocation inside the call, so `out`
+        (n_rows floats) is the caller's; at most STATIC_MAX_NNZ entries; calls that overlap on the GPU race on the scratch."""
+        import torch
+        c = self._csr(m)
+        assert r.is_cuda and r.dtype == torch.float32 and r.is_contiguous()
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.numel() == c.n_rows
+        st = torch.cuda.current_stream() if stream is None else stream
+        self._check(lib().vpmc_spmv_grad_static(self._h, C.byref(c), r.data_ptr(), out.data_ptr(), 1 if accumulate else 0, st.cuda_stream))
         return out
 
     def worst_case(self, doses, target, weight, stream=None):

@@ -33,6 +33,39 @@ static thread_local std::string g_create_err;
 static constexpr size_t kMaxSmemLut = 16 * 1024;      // larger material tables are read through L1 instead: a 64 KB table in
                                                       // shared memory costs the voxel kernel its fourth CTA per SM (measured +1-2.5 %)
 
+// ---- vpmc_spmv_grad_static: the one entry point that allocates nothing (include/vpmc.h).  Its scratch -- the first / last
+// partial sums per chunk of spmv_grad_kernel -- lives in this file-scope device array: 2 floats per chunk of kSpmvChunk entries,
+// VPMC_STATIC_MAX_NNZ entries at most = 256 KB, held by every GPU that loads the library until the process exits.  In host
+// code the NAME of the array is a host-side stand-in, not a device address: static_scratch_for_device() asks the runtime for
+// the address once per device (with that device current) and the launches are given that pointer.
+static_assert(VPMC_STATIC_MAX_NNZ % kSpmvChunk == 0, "the static scratch is sized in whole chunks");
+constexpr int kStaticChunks = (int)(VPMC_STATIC_MAX_NNZ / kSpmvChunk);
+static __device__ __align__(256) float g_spmv_static_part[2 * kStaticChunks];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+float *g_static_ptr[kMaxDevices] = {};
+bool g_static_tried[kMaxDevices] = {};
+std::string g_static_err[kMaxDevices];
+
+// device address of g_spmv_static_part on the CURRENT device `dev` (looked up once per device); NULL + *err on failure
+float *static_scratch_for_device(int dev, std::string *err)
+{
+    if (dev < 0 || dev >= kMaxDevices) { if (err) *err = "device index beyond the static-scratch table"; return nullptr; }
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_tried[dev]) {
+        g_static_tried[dev] = true;
+        void *ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_spmv_static_part);
+        if (e != cudaSuccess) { cudaGetLastError(); g_static_err[dev] = std::string("cudaGetSymbolAddress(g_spmv_static_part): ") + cudaGetErrorString(e); }
+        else g_static_ptr[dev] = static_cast<float *>(ptr);
+    }
+    if (!g_static_ptr[dev] && err) *err = g_static_err[dev];
+    return g_static_ptr[dev];
+}
+}  // namespace
+
 // grow-only device buffer
 static int ensure(vpmc_t *h, DevBuf &b, size_t bytes);
 
@@ -247,6 +280,7 @@ extern "C" int vpmc_create(vpmc_t **out, const vpmc_ct *ct, const vpmc_calib *ca
     h->sn[0] = ct->n[0]; h->sn[1] = ct->n[1]; h->sn[2] = ct->n[2];
     cudaGetDevice(&h->device);
     cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    h->static_scratch = static_scratch_for_device(h->device, &h->static_scratch_err);     // set-up of vpmc_spmv_grad_static; create does not fail on it
     DevGrid &G = h->G;
     G.nx = ct->n[0]; G.ny = ct->n[1]; G.nz = ct->n[2];
     G.hx = ct->h[0]; G.hy = ct->h[1]; G.hz = ct->h[2];
@@ -637,3 +671,31 @@ extern "C" int vpmc_get_launch_count(vpmc_t *h, uint64_t *out)
 }
 
 #include "vpmc_run.inl"
+
+// ---- the entry point that allocates nothing (include/vpmc.h): vpmc_spmv_grad with its scratch in g_spmv_static_part.
+// No cudaMalloc / cudaFree / buffer cache / event creation on this path; the two kernels are the ones vpmc_spmv_grad launches.
+extern "C" int vpmc_spmv_grad_static(vpmc_t *h, const vpmc_csr *m, const float *r_dev, float *grad_dev, int accumulate, void *cuda_stream)
+{
+    if (!h) return VPMC_ERR_INVALID_ARG;
+    int rc = check_csr(h, m); if (rc) return rc;
+    if ((m->n_rows > 0 && !grad_dev) || (m->nnz > 0 && !r_dev)) FAIL(h, VPMC_ERR_INVALID_ARG, "bad spmv_grad_static arguments");
+    if (m->nnz > (int64_t)VPMC_STATIC_MAX_NNZ)
+        FAIL(h, VPMC_ERR_INVALID_ARG, "vpmc_spmv_grad_static: %lld entries exceed VPMC_STATIC_MAX_NNZ = %lld (the static scratch holds %d chunks of %d entries); use vpmc_spmv_grad",
+             (long long)m->nnz, (long long)VPMC_STATIC_MAX_NNZ, kStaticChunks, kSpmvChunk);
+    if (!h->static_scratch) FAIL(h, VPMC_ERR_CUDA, "vpmc_spmv_grad_static: no static scratch on device %d: %s", h->device, h->static_scratch_err.c_str());
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->last_stream = st; h->launched = true;
+    const int nc = spmv_chunks(m->nnz);
+    // every partial the fix-up reads is written by the gather of the same call: nothing in the scratch has to start at zero
+    float *fp = h->static_scratch, *lp = fp + kStaticChunks;
+    if (nc > 0) {
+        spmv_grad_kernel<<<nc, kSpmvBlock, 0, st>>>((const long long *)m->row_ptr, m->col, m->val, m->n_rows, m->nnz, r_dev, grad_dev, accumulate, fp, lp);
+        h->launches += 1;
+    }
+    if (m->n_rows > 0) {
+        spmv_grad_fixup_kernel<<<(m->n_rows + 255) / 256, 256, 0, st>>>((const long long *)m->row_ptr, m->n_rows, fp, lp, grad_dev, accumulate);
+        h->launches += 1;
+    }
+    CU(h, cudaGetLastError());
+    return VPMC_OK;
+}

@@ -105,6 +105,8 @@ struct vpmc {
     vpmc_influence_stats inf_stats = {};
     DevBuf gamma_buf;                 // counters + list of the voxels that fail the zero-distance test (vpmc_gamma)
     DevBuf spmv_part;                 // first / last partial sums per chunk of vpmc_spmv_grad
+    float *static_scratch = nullptr;  // device address of the file-scope scratch of vpmc_spmv_grad_static on h->device (vpmc_api.cu)
+    std::string static_scratch_err;
     size_t workspace_limit = 0;       // bytes of influence scratch per group (0 = automatic)
 
     // knobs (vpmc_set_knob)
