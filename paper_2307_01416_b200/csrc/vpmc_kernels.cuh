@@ -921,6 +921,20 @@ __device__ __forceinline__ void box_next(const int4 dm, int &bx, int &by, int &b
 {
     if (++bx == dm.x) { bx = 0; if (++by == dm.y) { by = 0; ++bz; } }
 }
+// voxel indices of the thread's kPerThread consecutive elements from e on, for boxes at least kPerThread wide: the first
+// nrow lie in e's row (vA + i), the others in the next row (vB + i); no per-element carry chain
+struct BoxRun { int vA, vB, nrow; };
+__device__ __forceinline__ BoxRun box_run(const CsrCols &cc, unsigned int e, const int4 lo, const int4 dm)
+{
+    int bx, by, bz;
+    box_decode(e, dm, bx, by, bz);
+    BoxRun r;
+    r.vA = (lo.x + bx) + cc.nx * ((lo.y + by) + cc.ny * (lo.z + bz));
+    r.nrow = dm.x - bx;
+    if (++by == dm.y) { by = 0; ++bz; }
+    r.vB = lo.x + cc.nx * ((lo.y + by) + cc.ny * (lo.z + bz)) - r.nrow;      // beyond the box only for elements beyond cnt (never kept)
+    return r;
+}
 // the thread's kPerThread = 8 consecutive elements: two 16-byte loads when it owns all eight and they are aligned (always
 // the case inside a box: offsets and tiles are multiples of 8 elements), element-wise otherwise; missing elements read 0
 __device__ __forceinline__ void load8(const float *p, int cnt, float x[kPerThread])
@@ -954,15 +968,23 @@ csr_max_kernel(const CsrCols cc, float *__restrict__ data, const short *__restri
 #pragma unroll
         for (int i = 0; i < kPerThread; ++i) any = any || (x[i] != 0.0f);
         if (CONVERT && any) {
-            int bx, by, bz;
-            box_decode(e, dm, bx, by, bz);
+            if (dm.x >= kPerThread) {
+                const BoxRun br = box_run(cc, e, lo, dm);
 #pragma unroll
-            for (int i = 0; i < kPerThread; ++i) {
-                if (x[i] != 0.0f) {
-                    const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
-                    x[i] = __fdiv_rn(coef * x[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, v));
+                for (int i = 0; i < kPerThread; ++i)
+                    if (x[i] != 0.0f)
+                        x[i] = __fdiv_rn(coef * x[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, (long long)((i < br.nrow ? br.vA : br.vB) + i)));
+            } else {
+                int bx, by, bz;
+                box_decode(e, dm, bx, by, bz);
+#pragma unroll
+                for (int i = 0; i < kPerThread; ++i) {
+                    if (x[i] != 0.0f) {
+                        const long long v = (lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz));
+                        x[i] = __fdiv_rn(coef * x[i], score_density(cell_rho, hu, lut, hu_min, n_lut, rho_min, v));
+                    }
+                    box_next(dm, bx, by, bz);
                 }
-                box_next(dm, bx, by, bz);
             }
             if (cnt == kPerThread && (reinterpret_cast<size_t>(p) & 15) == 0) {
                 *reinterpret_cast<float4 *>(p) = make_float4(x[0], x[1], x[2], x[3]);
@@ -1067,16 +1089,27 @@ csr_emit_kernel(const CsrCols cc, const float *__restrict__ data, const unsigned
         unsigned int woff = 0;
         for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += wsum[w];
         long long pos = __ldg(col_base + c) + (long long)__ldg(tile_off + tile) + woff + inc - k;
-        int bx = 0, by = 0, bz = 0;
-        if (k) box_decode(e, dm, bx, by, bz);
+        if (k && dm.x >= kPerThread) {
+            const BoxRun br = box_run(cc, e, lo, dm);
 #pragma unroll
-        for (int i = 0; i < kPerThread; ++i) {
-            if (csr_keep(x[i], thr)) {
-                out_idx[pos] = (int)((lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz)));
-                out_val[pos] = x[i];
-                ++pos;
+            for (int i = 0; i < kPerThread; ++i)
+                if (csr_keep(x[i], thr)) {
+                    out_idx[pos] = (i < br.nrow ? br.vA : br.vB) + i;
+                    out_val[pos] = x[i];
+                    ++pos;
+                }
+        } else if (k) {
+            int bx, by, bz;
+            box_decode(e, dm, bx, by, bz);
+#pragma unroll
+            for (int i = 0; i < kPerThread; ++i) {
+                if (csr_keep(x[i], thr)) {
+                    out_idx[pos] = (int)((lo.x + bx) + (long long)cc.nx * ((lo.y + by) + (long long)cc.ny * (lo.z + bz)));
+                    out_val[pos] = x[i];
+                    ++pos;
+                }
+                box_next(dm, bx, by, bz);
             }
-            box_next(dm, bx, by, bz);
         }
         __syncthreads();
     }
