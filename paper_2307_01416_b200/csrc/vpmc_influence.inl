@@ -38,13 +38,31 @@ static int grow_keep(vpmc_t *h, DevBuf &b, size_t bytes, size_t keep, cudaStream
     return VPMC_OK;
 }
 
+// grid of a writer pass that strides over the tiles: all CTAs resident at once (n_sm x the kernel's own occupancy, looked up
+// once) -- with a fixed 8 per SM the 40-register conversion pass ran 1.33 waves, its last third on a third of the machine
+static int tile_grid(vpmc_t *h, const void *kernel, int n_tiles)
+{
+    static std::mutex mu;
+    static std::vector<std::pair<const void *, int>> cache;      // per kernel; every device here is the same part
+    int occ = 0;
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        for (auto &e : cache) if (e.first == kernel) occ = e.second;
+        if (occ == 0) {
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, 0) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 4; }
+            cache.push_back({ kernel, occ });
+        }
+    }
+    return std::max(1, std::min(n_tiles, h->n_sm * occ));
+}
+
 // writer pass 1 over a set of columns: (E_dep -> dose value,) column maxima
 static int csr_max_pass(vpmc_t *h, const CsrCols &cc, float *data, bool convert, float coef, cudaStream_t st)
 {
     int rc = ensure(h, h->inf_colmax, (size_t)cc.n_cols * sizeof(unsigned int)); if (rc) return rc;
     CU(h, cudaMemsetAsync(h->inf_colmax.p, 0, (size_t)cc.n_cols * sizeof(unsigned int), st));
     if (cc.n_tiles > 0) {
-        const int grid = std::max(1, std::min(cc.n_tiles, h->n_sm * 8));
+        const int grid = convert ? tile_grid(h, (const void *)csr_max_kernel<true>, cc.n_tiles) : tile_grid(h, (const void *)csr_max_kernel<false>, cc.n_tiles);
         TimedScope ts(h, st, 3);
         if (convert)
             csr_max_kernel<true><<<grid, kBlock, 0, st>>>(cc, data, h->d_hu, h->d_lut, h->G.hu_min, h->G.n_lut, h->params.rho_min, coef, h->inf_colmax.as<unsigned int>(), h->d_cell_rho);
@@ -63,7 +81,7 @@ static int csr_count_pass(vpmc_t *h, const CsrCols &cc, const float *data, float
     rc = ensure(h, h->inf_colnnz, (size_t)cc.n_cols * sizeof(long long)); if (rc) return rc;
     TimedScope ts(h, st, 3);
     if (cc.n_tiles > 0) {
-        csr_count_kernel<<<std::max(1, std::min(cc.n_tiles, h->n_sm * 8)), kBlock, 0, st>>>(cc, data, h->inf_colmax.as<unsigned int>(), rel_thr, h->inf_tilecnt.as<unsigned int>());
+        csr_count_kernel<<<tile_grid(h, (const void *)csr_count_kernel, cc.n_tiles), kBlock, 0, st>>>(cc, data, h->inf_colmax.as<unsigned int>(), rel_thr, h->inf_tilecnt.as<unsigned int>());
         h->launches += 1;
     }
     csr_tile_scan_kernel<<<cc.n_cols, kBlock, 0, st>>>(cc, h->inf_tilecnt.as<unsigned int>(), h->inf_colnnz.as<long long>());
@@ -97,7 +115,7 @@ extern "C" int vpmc_csr_from_dense(vpmc_t *h, const float *col_dev, int64_t n, f
     if (col_out_dev && nnz > 0) {
         std::vector<long long> base(1, 0ll);
         rc = upload(h, h->inf_colbase, base, st); if (rc) return rc;
-        csr_emit_kernel<<<std::max(1, std::min(cc.n_tiles, h->n_sm * 8)), kBlock, 0, st>>>(cc, col_dev, h->inf_colmax.as<unsigned int>(), rel_threshold,
+        csr_emit_kernel<<<tile_grid(h, (const void *)csr_emit_kernel, cc.n_tiles), kBlock, 0, st>>>(cc, col_dev, h->inf_colmax.as<unsigned int>(), rel_threshold,
                                                                                          h->inf_tilecnt.as<unsigned int>(), h->inf_colbase.as<long long>(), col_out_dev, val_out_dev);
         CU(h, cudaGetLastError());
         h->launches += 1;
@@ -333,7 +351,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                         (rc = grow_keep(h, h->inf_stage_val, (size_t)(staged + add) * sizeof(float), (size_t)staged * sizeof(float), st)) ||
                         (rc = upload(h, h->inf_colbase, base, st))) return rc;
                     TimedScope ts(h, st, 3);
-                    csr_emit_kernel<<<std::max(1, std::min(cc.n_tiles, h->n_sm * 8)), kBlock, 0, st>>>(cc, cb.scratch, h->inf_colmax.as<unsigned int>(), rel_threshold,
+                    csr_emit_kernel<<<tile_grid(h, (const void *)csr_emit_kernel, cc.n_tiles), kBlock, 0, st>>>(cc, cb.scratch, h->inf_colmax.as<unsigned int>(), rel_threshold,
                                                                                                      h->inf_tilecnt.as<unsigned int>(), h->inf_colbase.as<long long>(),
                                                                                                      h->inf_stage_idx.as<int>(), h->inf_stage_val.as<float>());
                     CU(h, cudaGetLastError());

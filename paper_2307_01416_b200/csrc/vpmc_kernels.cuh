@@ -1227,25 +1227,61 @@ ovf_columns_kernel(const unsigned int *__restrict__ b_cell, const float *__restr
 // final assembly: row r = merge of its staged box entries (a) and its kept overflow entries (b), both ascending in voxel
 // index and disjoint, into the scenario's CSR arrays.  Position of an element = its rank in its own list + the number of
 // elements of the other list below it (binary search).
+constexpr int kGatherStage = 8192;
 __global__ void csr_gather_rows_kernel(int n_rows, const long long *__restrict__ src_off, const long long *__restrict__ ovf_off,
                                        const int *__restrict__ ovf_n, const long long *__restrict__ row_ptr,
                                        const int *__restrict__ s_idx, const float *__restrict__ s_val,
                                        const int *__restrict__ o_idx, const float *__restrict__ o_val,
                                        int *__restrict__ idx, float *__restrict__ val)
 {
+    __shared__ int s_o[kGatherStage];        // the row's overflow indices: the box elements' searches stay inside the SM
     for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
         const long long dst = __ldg(row_ptr + r), n = __ldg(row_ptr + r + 1) - dst, sa = __ldg(src_off + r);
         const int nb = __ldg(ovf_n + r);
         const long long na = n - nb, sb = __ldg(ovf_off + r);
+        // four elements per thread in flight: with one, the copy ran at 1.8 TB/s (bytes in flight per SM / latency)
         if (nb == 0) {
-            for (long long i = threadIdx.x; i < na; i += blockDim.x) { idx[dst + i] = s_idx[sa + i]; val[dst + i] = s_val[sa + i]; }
+            long long i = threadIdx.x;
+            for (; i + 3 * blockDim.x < na; i += 4 * blockDim.x) {
+                int v[4]; float x[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { v[u] = __ldg(s_idx + sa + i + u * blockDim.x); x[u] = __ldg(s_val + sa + i + u * blockDim.x); }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { idx[dst + i + u * blockDim.x] = v[u]; val[dst + i + u * blockDim.x] = x[u]; }
+            }
+            for (; i < na; i += blockDim.x) { idx[dst + i] = s_idx[sa + i]; val[dst + i] = s_val[sa + i]; }
             continue;
         }
-        for (long long i = threadIdx.x; i < na; i += blockDim.x) {
-            const int v = s_idx[sa + i];
-            int lo = 0, hi = nb;
-            while (lo < hi) { const int mid = (lo + hi) >> 1; if (o_idx[sb + mid] < v) lo = mid + 1; else hi = mid; }
-            idx[dst + i + lo] = v; val[dst + i + lo] = s_val[sa + i];
+        if (nb <= kGatherStage) {
+            __syncthreads();                  // the previous row's searches are done
+            for (int j = threadIdx.x; j < nb; j += blockDim.x) s_o[j] = o_idx[sb + j];
+            __syncthreads();
+            long long i = threadIdx.x;
+            for (; i + 3 * blockDim.x < na; i += 4 * blockDim.x) {
+                int v[4]; float x[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { v[u] = __ldg(s_idx + sa + i + u * blockDim.x); x[u] = __ldg(s_val + sa + i + u * blockDim.x); }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    int lo = 0, hi = nb;
+                    while (lo < hi) { const int mid = (lo + hi) >> 1; if (s_o[mid] < v[u]) lo = mid + 1; else hi = mid; }
+                    idx[dst + i + u * blockDim.x + lo] = v[u]; val[dst + i + u * blockDim.x + lo] = x[u];
+                }
+            }
+            for (; i < na; i += blockDim.x) {
+                const int v = s_idx[sa + i];
+                const float x = s_val[sa + i];
+                int lo = 0, hi = nb;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (s_o[mid] < v) lo = mid + 1; else hi = mid; }
+                idx[dst + i + lo] = v; val[dst + i + lo] = x;
+            }
+        } else {
+            for (long long i = threadIdx.x; i < na; i += blockDim.x) {
+                const int v = s_idx[sa + i];
+                int lo = 0, hi = nb;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (o_idx[sb + mid] < v) lo = mid + 1; else hi = mid; }
+                idx[dst + i + lo] = v; val[dst + i + lo] = s_val[sa + i];
+            }
         }
         for (int j = threadIdx.x; j < nb; j += blockDim.x) {
             const int v = o_idx[sb + j];
