@@ -229,12 +229,19 @@ def ncu_summary(ncu_csv, bench_log, config):
     import re
     line = [l for l in open(bench_log) if l.startswith("{")][-1]
     b = json.loads(line)
-    calls = b["profile_units"]["steps_run"]          # the profiled run must be --no-e2e --no-subrecords: nothing else launches these kernels
-    units = {"beam_kernel": b["profile_units"]["slab_steps_per_step"] * calls, "voxel_kernel": b["profile_units"]["ct_steps_per_step"] * calls}
+    if config == "config4":
+        # influence build: only the MODE 1 voxel kernel (private boxes) counts its steps in the tallies; the pilot (MODE 2) does not
+        calls = b["profile_units"]["builds_run"]
+        units = {"voxel_kernel_box": b["profile_units"]["ct_steps_per_build"] * calls}
+    else:
+        calls = b["profile_units"]["steps_run"]          # the profiled run must be --no-e2e --no-subrecords: nothing else launches these kernels
+        units = {"beam_kernel": b["profile_units"]["slab_steps_per_step"] * calls, "voxel_kernel": b["profile_units"]["ct_steps_per_step"] * calls}
     acc = collections.defaultdict(lambda: collections.defaultdict(float))
     for r in csv.DictReader(l for l in open(ncu_csv) if l.startswith('"')):
         name = re.sub(r"^void ", "", r["Kernel Name"])
         name = re.sub(r"^vpk::", "", name)
+        if config == "config4" and re.match(r"voxel_kernel<(\(int\))?1,", name):
+            name = "voxel_kernel_box"
         name = re.sub(r"[<(].*", "", name)
         try:
             v = float(r["Metric Value"].replace(",", ""))
@@ -448,7 +455,6 @@ def run_b200(args):
             sub["config5_polygon"]["relative_to_bitmap"] = rp["value"] / rec["value"] if args.workload == "config5" else None
         sub["config3"] = measure_to_uncertainty(CONFIG3_SEEDS)
         sub["config4"] = measure_influence(10_000, 1, 1)
-        sub["config4"]["roofline_voxel_box"] = None
         out["configs"] = sub
         out["dose_at_0p5pct"] = {"workload": sub["config3"]["workload"], "seconds": sub["config3"]["seconds_mean"], "seconds_std": sub["config3"]["seconds_std"], "seconds_median": sub["config3"]["seconds_median"],
                                  "uncertainty_max": sub["config3"]["uncertainty_max"], "target": 0.005}
@@ -534,7 +540,27 @@ def measure_influence(hps, steps, warmup):
     tm = eng.timing()
     st = eng.influence_stats()
     opt = measure_optimiser(eng, sc, hps, w, hbm_gbs, peak_kind)
-    tl = eng.tallies()
+    tl = eng.tallies()                                                # of the last build: every history of every scenario once
+    ct_steps = int(tl.as_dict()["n_steps_ct"])
+    box = None
+    vox_ms, vox_n = tm["voxel"][0] / steps, tm["voxel"][1] / steps
+    if vox_ms > 0:
+        _, sm_max_mhz, _ = load_peaks()
+        peak = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e9
+        counts = load_inst_counts("config4")
+        row = counts.get("voxel_kernel_box") if counts else None
+        ipu = float(row["thread_inst_per_unit"]) if row else None
+        box = {"kernel": "voxel_kernel<1, ...> (BoxScorer)", "bound": "alu", "peak": peak, "unit": "Glane-inst/s", "ct_steps_per_build": ct_steps,
+               "voxel_class_ms": vox_ms, "launches": vox_n, "inst_per_unit": ipu, "inst_per_unit_survey": SURVEY_INST_PER_STEP,
+               "achieved": ipu * ct_steps / (vox_ms * 1e-3) / 1e9 if ipu else None,
+               "frac": ipu * ct_steps / (vox_ms * 1e-3) / 1e9 / peak if ipu else None,
+               "frac_survey_count": SURVEY_INST_PER_STEP * ct_steps / (vox_ms * 1e-3) / 1e9 / peak,
+               "lanes_per_inst": float(row["lanes_per_inst"]) if row else None,
+               "red": {"sectors_per_unit": float(row["red_sectors_per_unit"])} if row else None,
+               "l2": {"bytes_per_unit": float(row["l2_bytes_per_unit"]), "hit_pct": float(row["l2_hit_pct"])} if row else None,
+               "note": "the voxel timing class also holds the pilot launches (MODE 2, bounding boxes), whose steps are not counted: the fraction is a lower bound",
+               "inst_source": "profiles/r2_inst_per_step.csv row (config4, voxel_kernel_box): ncu counters of the MODE 1 launches of a build at 2000 "
+                              "histories per spot / CT steps counted by the kernels" if row else "no committed ncu counts for this config"}
     n_hist = len(sc) * eng.n_spots * hps
     wr_s = tm["writer"][0] * 1e-3 / steps
     alg = 8.0 * st["nnz"] + 12.0 * st["box_elements"]                 # nnz (col + val) written once + three 4-byte reads of every box element
@@ -553,7 +579,8 @@ def measure_influence(hps, steps, warmup):
                       "bytes_as_implemented": impl, "achieved_as_implemented": impl / wr_s / 1e9 if wr_s > 0 else None,
                       "note": "algorithmic = 8 B x nnz written + 3 reads x 4 B of every box element (max, count, emit); the class also times the "
                               "overflow-list kernels", "peak_source": peak_kind + " MEASURED_PEAKS.json hbm_gbs"},
-           "optimiser_iteration": opt,
+           "optimiser_iteration": opt, "roofline_voxel_box": box,
+           "profile_units": {"builds_run": warmup + steps + 1, "ct_steps_per_build": ct_steps},
            "paper_context": "41.6 s for 13 influence matrices (P:L205-207): other data, other hardware"}
     eng.close()
     return out
