@@ -215,6 +215,43 @@ __device__ __forceinline__ unsigned int warp_push_slot(unsigned int *counter, bo
     return base + (unsigned)__popc(m & lanemask_lt());
 }
 
+// Slot of this thread's record with ONE atomic per block: with one per warp, a chunk of 2^23 records sends 2.6e5 atomics to
+// the same address, and the L2 serialises those (source_kernel: its incident-energy and record-count atomics were its whole
+// run time).  Worth it only where the block's warps arrive together -- behind divergent work the barrier costs more than
+// the atomics (measured in ap_entry_kernel).  Must be called by all threads of the block, once per kernel.
+__device__ __forceinline__ unsigned int block_push_slot(unsigned int *counter, bool want)
+{
+    __shared__ unsigned int s_cnt[kWarps];
+    __shared__ unsigned int s_base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned int m = __ballot_sync(0xffffffffu, want);
+    if (lane == 0) s_cnt[warp] = (unsigned)__popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int run = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) { const unsigned int c = s_cnt[w]; s_cnt[w] = run; run += c; }
+        s_base = run ? atomicAdd(counter, run) : 0u;
+    }
+    __syncthreads();
+    return s_base + s_cnt[warp] + (unsigned)__popc(m & lanemask_lt());
+}
+
+// block sum of a double in a fixed order, valid in thread 0.  Must be called by all threads of the block, once per kernel.
+__device__ __forceinline__ double block_sum_thread0(double v)
+{
+    __shared__ double s_v[kWarps];
+    v = warp_sum(v);
+    if ((threadIdx.x & 31) == 0) s_v[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) t += s_v[w];
+    }
+    return t;
+}
+
 __device__ __forceinline__ void queue_store(const Queue &q, unsigned int slot, const Hist &h)
 {
     if (slot >= q.capacity) return;
@@ -288,6 +325,8 @@ source_kernel(const Ctx c, const WorkMap wm, const unsigned long long item0, con
     int dest = 0;                      // 1 range shifter, 2 aperture queue, 3 CT queue, 4 escaped
     Hist h;
     h.E = 0.0f; h.step = 0u; h.region = 0;
+    int reg = -1;
+    NullTracer tr;
     if (k < wm.n_items) {
         int g; unsigned long long hid;
         map_item(wm, item0 + k, g, hid, h.col);
@@ -295,25 +334,28 @@ source_kernel(const Ctx c, const WorkMap wm, const unsigned long long item0, con
         const int beam = __ldg(spot_beam + g);
         sample_source(c.P, c.beams[beam], beam, __ldg(spots + g), __ldg(spot_R0 + g), h, c.K);
         inc = (double)h.E;
-        NullTracer tr;
-        const int reg = h.region & 0xff;
+        reg = h.region & 0xff;
         if (reg == REG_TO_RS) dest = (rs_enter(c, h, tr) == BEAM_CONT) ? 1 : 4;
-        else if (reg == REG_TO_AP) { const int st = ap_enter(c, h, tr); dest = (st == BEAM_EXIT) ? 3 : (st == BEAM_CONT ? 2 : 4); }
-        else dest = 3;
     }
-    const unsigned s_rs = warp_push_slot(sb.count, dest == 1, lane);
-    const unsigned s_ap = warp_push_slot(q_ap.count, dest == 2, lane);
-    const unsigned s_ct = warp_push_slot(q_ct.count, dest == 3, lane);
+    // Up to here every warp of the block has done the same work: the range-shifter records and the incident energy are
+    // pushed with one atomic per BLOCK (block_push_slot, block_sum_thread0).  The opening phase below is divergent -- a barrier
+    // behind it would make every warp wait for the block's slowest -- so the two queues it feeds keep one atomic per warp.
+    const unsigned s_rs = block_push_slot(sb.count, dest == 1);
+    inc = block_sum_thread0(inc);
+    if (threadIdx.x == 0 && inc != 0.0) atomicAdd(&tal->incident, inc);
     if (dest == 1) {
         const unsigned long long rb = (unsigned long long)__double_as_longlong(h.R);
         sb.s0[s_rs] = make_uint4(h.g0, h.g1, h.g2, h.g3);
         sb.s1[s_rs] = make_uint4(__float_as_uint(h.E), __float_as_uint(h.tau_star), (unsigned)h.col | ((unsigned)(h.region >> 8) << 24), h.step);
         sb.s2[s_rs] = make_uint4((unsigned)rb, (unsigned)(rb >> 32), h.hid_lo, h.hid_hi);
-    } else if (dest == 2) queue_store(q_ap, s_ap, h);
+    }
+    if (reg == REG_TO_AP) { const int st = ap_enter(c, h, tr); dest = (st == BEAM_EXIT) ? 3 : (st == BEAM_CONT ? 2 : 4); }
+    else if (reg >= 0 && reg != REG_TO_RS) dest = 3;
+    const unsigned s_ap = warp_push_slot(q_ap.count, dest == 2, lane);
+    const unsigned s_ct = warp_push_slot(q_ct.count, dest == 3, lane);
+    if (dest == 2) queue_store(q_ap, s_ap, h);
     else if (dest == 3) queue_store(q_ct, s_ct, h);
     book_escapes_converged(tal, dest == 4, h.E, h.step);
-    inc = warp_sum(inc);
-    if (lane == 0 && inc != 0.0) atomicAdd(&tal->incident, inc);
 }
 
 // Aperture entry of the histories that left the range shifter, one thread per record: vacuum drift to the aperture
@@ -442,12 +484,22 @@ entry_kernel(const Ctx c, const Queue q, DevTallies *tal)
         q.q2[i] = make_float4(h.lx, h.ly, h.lz, b.w);
         q.q3[i] = make_uint4(e.x, e.y, h.step, e.w);
     }
+    // the drift-step count is booked once per block (every warp has some: one same-address atomic per warp otherwise);
+    // escapes are rare and stay per warp
+    __shared__ unsigned int s_dev[kWarps];
     esc = warp_sum(esc);
     n_esc = __reduce_add_sync(0xffffffffu, n_esc); n_dev = __reduce_add_sync(0xffffffffu, n_dev);
     if ((threadIdx.x & 31) == 0) {
+        s_dev[threadIdx.x >> 5] = n_dev;
         if (esc != 0.0) atomicAdd(&tal->escaped, esc);
         if (n_esc) atomicAdd(&tal->n_escaped, (unsigned long long)n_esc);
-        if (n_dev) atomicAdd(&tal->n_steps_dev, (unsigned long long)n_dev);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) t += s_dev[w];
+        if (t) atomicAdd(&tal->n_steps_dev, t);
     }
 }
 
