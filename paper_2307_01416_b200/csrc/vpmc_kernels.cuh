@@ -524,6 +524,7 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
     Hist h;
     h.region = REG_CT; h.col = 0; h.step = 0u;
     float hdep = 0.0f;
+    int hu_pre = 0;                    // HU of the voxel the lane's history stands in (fetched ahead of the step that needs it)
     const unsigned n_q = min(*q.count, q.capacity);
     const unsigned nxy = (unsigned)(c.G.nx * c.G.ny);
     int pend = CONT;                       // cause of a finished history whose bookkeeping is still due
@@ -562,6 +563,7 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
                             h.R = __longlong_as_double((long long)(((unsigned long long)f.y << 32) | f.x));
                             h.hid_lo = f.z; h.hid_hi = f.w;
                             hdep = 0.0f;
+                            hu_pre = (int)__ldg(c.hu + h.g3);
                             sc.begin(h);
                             alive = true;
                         }
@@ -575,9 +577,10 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         }
         if (alive) {
             int cause;
-            if (SMEM_LUT) cause = ct_step<FL>(c, LutShared{ lut_s }, h, hdep, lc, sc, tr);
-            else cause = ct_step<FL>(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr);
+            if (SMEM_LUT) cause = ct_step<FL>(c, LutShared{ lut_s }, h, hdep, lc, sc, tr, &hu_pre);
+            else cause = ct_step<FL>(c, LutGlobal{ lut_g }, h, hdep, lc, sc, tr, &hu_pre);
             if (cause != CONT) { alive = false; pend = cause; }
+            else hu_pre = (int)__ldg(c.hu + h.g3);            // the next step's voxel: in flight during the refill pass and the face distances
         }
     }
     flush_warp_tallies(wt_all + warp, lc, tal, lane);

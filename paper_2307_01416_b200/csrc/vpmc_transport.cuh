@@ -629,15 +629,17 @@ __device__ __forceinline__ int ct_entry(const Ctx &c, Hist &h, LaneCounters &lc,
 
 // One voxel step of history h (S4, S5, S6/S7).  Returns CONT or the cause that ended the history; the once-per-history
 // tallies are booked by book_ct_end() in the kernel's refill pass.  hdep = energy deposited in the CT so far.
+// hu_pre (optional): the HU of the voxel the history stands in, fetched by the caller at the end of the previous step (the
+// voxel kernel does: HU -> table is a chain of two dependent loads at the head of the step, 6 % of its stall samples).
 template <int FL, class Lut, class Scorer, class Tracer>
 __device__ __forceinline__ int ct_step(const Ctx &c, const Lut &lut, Hist &h, float &hdep, LaneCounters &lc,
-                                       Scorer &sc, Tracer &tr)
+                                       Scorer &sc, Tracer &tr, const int *hu_pre = nullptr)
 {
     const DevParams &P = c.P;
     const DevGrid &G = c.G;
     int ax; bool up;
     const float d = face_distance(G, h, ax, up);
-    int t = (int)__ldg(c.hu + h.g3) - G.hu_min;
+    int t = (hu_pre ? *hu_pre : (int)__ldg(c.hu + h.g3)) - G.hu_min;
     t = min(max(t, 0), G.n_lut - 1);
     const float4 mv = lut[t];                 // rsp, rho, xsp / X0_w, 1 / rsp
     const Medium m = { mv.x * c.rsp_scale, mv.w * c.inv_rsp_scale, mv.y, mv.z, P.za_w * mv.y };
