@@ -48,7 +48,7 @@ def test_static_scratch_gradient_equals_the_existing_path_twice_in_a_row():
     for m, r, o in zip(dev, rs, outs):                                            # two calls in a row, nothing in between
         eng.spmv_grad_static(m, r, o)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free0                                  # no device memory was taken
+    assert torch.cuda.mem_get_info()[0] >= free0                                  # no device memory was taken
     for m, r, o, g in zip(mats, rs, outs, ref):
         g_abs = rob.spmv_grad((m[0], m[1], np.abs(m[2])), np.abs(r.cpu().numpy()))
         assert np.all(np.abs(o.cpu().numpy().astype(np.float64) - g.cpu().numpy().astype(np.float64)) <= 1e-6 * g_abs + 1e-30)
