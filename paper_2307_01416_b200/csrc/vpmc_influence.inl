@@ -261,8 +261,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                 CU(h, cudaMemcpyAsync(obb.data(), h->inf_bbox.p, obb.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
                 CU(h, cudaMemcpyAsync(&n_ovf, h->ovf_ctr.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
                 CU(h, cudaStreamSynchronize(st));
-                n_ovf = std::min(n_ovf, ovf_cap);
-                h->inf_stats.ovf_deposits += n_ovf;
+                n_ovf = std::min(n_ovf, ovf_cap);            // slots handed out, sentinels of the warps' unused stretches included
                 // overflow entries per column; a column with more than a CTA sorts is treated like one that lost deposits
                 std::vector<unsigned int> ovf_cnt(nc, 0u), ovf_off(nc, 0u);
                 if (n_ovf > 0) {
@@ -277,6 +276,7 @@ extern "C" int vpmc_influence(vpmc_t *h, const vpmc_scenario *scs, int32_t n_sc,
                     bool any_big = false;
                     unsigned int run = 0;
                     for (int c = 0; c < nc; ++c) { ovf_off[c] = run; run += ovf_cnt[c]; if (ovf_cnt[c] > h->ovf_sort_cap) { big[c] = 1; any_big = true; } }
+                    h->inf_stats.ovf_deposits += run;
                     if (any_big) {
                         rc = upload(h, h->inf_skip, big, st); if (rc) return rc;
                         ovf_bbox_kernel<<<g1, 256, 0, st>>>(h->ovf_key.as<unsigned long long>(), n_ovf, h->inf_skip.as<int>(), h->sn[0], h->sn[1], h->inf_bbox.as<int>());

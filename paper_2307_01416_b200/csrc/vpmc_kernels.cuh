@@ -95,6 +95,9 @@ struct DoseScorer {            // MODE 0: E_dep[batch][v] += dE, fp32 RED into L
         atomicAdd(edep + (size_t)h.col * nvox + v, dep);
     }
     __device__ __forceinline__ void end(const Hist &) {}
+    __device__ __forceinline__ void attach(unsigned int *) {}
+    __device__ __forceinline__ void room(int) {}
+    __device__ __forceinline__ void finish(int) {}
 };
 
 __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int x1, int y1, int z1)
@@ -103,8 +106,19 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
     atomicMax(bb + 3, x1); atomicMax(bb + 4, y1); atomicMax(bb + 5, z1);
 }
 
+// MODE 1 appends a deposit outside its column's box to the overflow list.  One returning atomicAdd on the list's counter
+// per such deposit (0.12 % of the steps) made the lane -- and with it the warp -- wait for a round trip to ONE contended L2
+// address: a quarter of the kernel's stall samples.  Instead a warp reserves a STRETCH of kOvfStretch slots with one global
+// atomic and hands them out through a cursor in shared memory; room() (all lanes, every pass of the step loop) reserves the
+// next stretch before fewer than kOvfRoom slots are left and fills what it abandons with sentinel keys (column 0xffffffff:
+// skipped by the list's consumers), finish() does the same at the end of the kernel.  A deposit that finds no slot (nothing
+// reserved yet, or more outside deposits in one step than were left) takes the global atomic as before.
+constexpr unsigned int kOvfStretch = 64, kOvfRoom = 8;
+constexpr unsigned long long kOvfSentinel = ~0ull;
+
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
     ColumnBoxes cb; ScoreGeom sg;
+    unsigned int *ws;          // shared memory, this warp's stretch of the overflow list: [0] next slot, [1] end
     // the history's column box, read once when the lane takes the history (three dependent loads per deposit otherwise:
     // ncu long_scoreboard 2.2 against 0.5 in dose mode): low corner, extent, element offset of the box
     int lx, ly, lz, dx, dy, dz;
@@ -124,13 +138,33 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
             atomicAdd(cb.scratch + off + (bx + (unsigned long long)dx * (by + (unsigned long long)dy * bz)), dep);
         else {
             const int c = h.col;
-            const unsigned slot = atomicAdd(cb.ovf_count, 1u);
+            unsigned slot = atomicAdd(ws, 1u);
+            if (slot >= ws[1]) slot = atomicAdd(cb.ovf_count, 1u);
             const unsigned int v = sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3;
             if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | v; cb.ovf_val[slot] = dep; }
             else bbox_merge(cb.bbox + 6 * c, sx, sy, sz, sx, sy, sz);
         }
     }
     __device__ __forceinline__ void end(const Hist &) {}
+    __device__ __forceinline__ void attach(unsigned int *warp_state) { ws = warp_state; }
+    __device__ __forceinline__ void close_stretch(unsigned int nxt, unsigned int end, int lane)
+    {
+        for (unsigned int i = min(nxt, end) + lane; i < end; i += 32)
+            if (i < cb.ovf_cap) { cb.ovf_key[i] = kOvfSentinel; cb.ovf_val[i] = 0.0f; }
+    }
+    __device__ __forceinline__ void room(int lane)             // all 32 lanes
+    {
+        const unsigned int nxt = ws[0], end = ws[1];
+        if (nxt + kOvfRoom <= end || (nxt | end) == 0u) return; // enough slots left, or no outside deposit so far
+        close_stretch(nxt, end, lane);
+        unsigned int base = 0;
+        if (lane == 0) base = atomicAdd(cb.ovf_count, kOvfStretch);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        __syncwarp();
+        if (lane == 0) { ws[0] = base; ws[1] = base + kOvfStretch; }
+        __syncwarp();
+    }
+    __device__ __forceinline__ void finish(int lane) { __syncwarp(); close_stretch(ws[0], ws[1], lane); }
 };
 
 struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits of each column
@@ -145,6 +179,9 @@ struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits o
         x1 = max(x1, sx); y1 = max(y1, sy); z1 = max(z1, sz);
     }
     __device__ __forceinline__ void end(const Hist &h) { if (x1 >= 0) bbox_merge(bbox + 6 * h.col, x0, y0, z0, x1, y1, z1); }
+    __device__ __forceinline__ void attach(unsigned int *) {}
+    __device__ __forceinline__ void room(int) {}
+    __device__ __forceinline__ void finish(int) {}
 };
 
 template <int MODE> struct ScorerOf;
@@ -156,7 +193,7 @@ struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; ScoreGe
 
 template <int MODE> __device__ __forceinline__ typename ScorerOf<MODE>::type make_scorer(const ScoreArgs &a);
 template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox, a.sg }; }
-template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { BoxScorer s; s.cb = a.cb; s.sg = a.sg; s.lx = s.ly = s.lz = 0; s.dx = s.dy = s.dz = 0; s.off = 0ull; return s; }
+template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { BoxScorer s; s.cb = a.cb; s.sg = a.sg; s.ws = nullptr; s.lx = s.ly = s.lz = 0; s.dx = s.dy = s.dz = 0; s.off = 0ull; return s; }
 template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; s.sg = a.sg; return s; }
 
 // ------------------------------------------------------------------------------------------- S1-S7
@@ -519,6 +556,10 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         for (int i = threadIdx.x; i < c.G.n_lut; i += blockDim.x) lut_s[i] = lut_g[i];
     __syncthreads();
     typename ScorerOf<MODE>::type sc = make_scorer<MODE>(sa);
+    __shared__ unsigned int s_ovf[kWarps][2];              // MODE 1: the warps' stretches of the overflow list (BoxScorer)
+    if (lane < 2) s_ovf[warp][lane] = 0u;
+    __syncwarp();
+    sc.attach(s_ovf[warp]);
     NullTracer tr;
     LaneCounters lc;
     Hist h;
@@ -534,6 +575,7 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
         const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != CONT);
         const int n_free = __popc(free_mask);
+        sc.room(lane);
         if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
             if (!alive && pend != CONT) sc.end(h);
             book_ct_end(c.P, h, !alive && pend != CONT, pend, hdep, wt_all + warp, lane);
@@ -583,6 +625,7 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
             else hu_pre = (int)__ldg(c.hu + h.g3);            // the next step's voxel: in flight during the refill pass and the face distances
         }
     }
+    sc.finish(lane);
     flush_warp_tallies(wt_all + warp, lc, tal, lane);
 }
 
@@ -1187,7 +1230,10 @@ constexpr int kOvfBlock = 1024;
 
 __global__ void ovf_hist_kernel(const unsigned long long *__restrict__ key, unsigned int n, unsigned int *__restrict__ col_cnt)
 {
-    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) atomicAdd(col_cnt + (unsigned)(key[i] >> 32), 1u);
+    for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const unsigned c = (unsigned)(key[i] >> 32);
+        if (c != 0xffffffffu) atomicAdd(col_cnt + c, 1u);       // not a sentinel (BoxScorer::close_stretch)
+    }
 }
 
 // bounding box (scoring-grid coordinates) of the overflow entries of the columns flagged in `lost`
@@ -1195,7 +1241,7 @@ __global__ void ovf_bbox_kernel(const unsigned long long *__restrict__ key, unsi
 {
     for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const unsigned c = (unsigned)(key[i] >> 32), v = (unsigned)key[i];
-        if (!__ldg(lost + c)) continue;
+        if (c == 0xffffffffu || !__ldg(lost + c)) continue;
         const int z = (int)(v / (unsigned)(snx * sny)), rem = (int)(v - (unsigned)z * (unsigned)(snx * sny)), y = rem / snx, x = rem - y * snx;
         bbox_merge(bbox + 6 * c, x, y, z, x, y, z);
     }
@@ -1208,6 +1254,7 @@ __global__ void ovf_scatter_kernel(const unsigned long long *__restrict__ key, c
     for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const unsigned long long k = key[i];
         const unsigned c = (unsigned)(k >> 32);
+        if (c == 0xffffffffu) continue;
         const unsigned pos = __ldg(col_off + c) + atomicAdd(cursor + c, 1u);
         b_cell[pos] = (unsigned)k; b_val[pos] = val[i];
     }
