@@ -109,11 +109,11 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
 // MODE 1 appends a deposit outside its column's box to the overflow list.  One returning atomicAdd on the list's counter
 // per such deposit (0.12 % of the steps) made the lane -- and with it the warp -- wait for a round trip to ONE contended L2
 // address: a quarter of the kernel's stall samples.  Instead a warp reserves a STRETCH of kOvfStretch slots with one global
-// atomic and hands them out through a cursor in shared memory; room() (all lanes, every pass of the step loop) reserves the
-// next stretch before fewer than kOvfRoom slots are left and fills what it abandons with sentinel keys (column 0xffffffff:
+// atomic and hands them out through a cursor in shared memory; room() (all lanes, in the refill pass of the step loop) reserves
+// the next stretch when fewer than kOvfRoom slots are left and fills what it abandons with sentinel keys (column 0xffffffff:
 // skipped by the list's consumers), finish() does the same at the end of the kernel.  A deposit that finds no slot (nothing
 // reserved yet, or more outside deposits in one step than were left) takes the global atomic as before.
-constexpr unsigned int kOvfStretch = 64, kOvfRoom = 8;
+constexpr unsigned int kOvfStretch = 64, kOvfRoom = 16;
 constexpr unsigned long long kOvfSentinel = ~0ull;
 
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
@@ -575,8 +575,8 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         const unsigned free_mask = __ballot_sync(0xffffffffu, !alive);
         const unsigned pend_mask = __ballot_sync(0xffffffffu, !alive && pend != CONT);
         const int n_free = __popc(free_mask);
-        sc.room(lane);
         if ((n_free >= kRefillMin || n_free == 32) && (!exhausted || pend_mask)) {
+            sc.room(lane);
             if (!alive && pend != CONT) sc.end(h);
             book_ct_end(c.P, h, !alive && pend != CONT, pend, hdep, wt_all + warp, lane);
             pend = alive ? pend : CONT;
