@@ -95,7 +95,7 @@ struct DoseScorer {            // MODE 0: E_dep[batch][v] += dE, fp32 RED into L
         atomicAdd(edep + (size_t)h.col * nvox + v, dep);
     }
     __device__ __forceinline__ void end(const Hist &) {}
-    __device__ __forceinline__ void attach(unsigned int *) {}
+    __device__ __forceinline__ void attach(int) {}
     __device__ __forceinline__ void room(int) {}
     __device__ __forceinline__ void finish(int) {}
 };
@@ -115,10 +115,18 @@ __device__ __forceinline__ void bbox_merge(int *bb, int x0, int y0, int z0, int 
 // reserved yet, or more outside deposits in one step than were left) takes the global atomic as before.
 constexpr unsigned int kOvfStretch = 64, kOvfRoom = 16;
 constexpr unsigned long long kOvfSentinel = ~0ull;
+constexpr int kOvfWarps = 8;              // = kBlock / 32 of the voxel kernel (static_assert there)
+
+// this warp's stretch of the overflow list, in shared memory: [0] next slot, [1] end.  Found through the thread index where it
+// is needed (rare paths) instead of being carried: the MODE 1 kernel has no register to spare.
+__device__ __forceinline__ unsigned int *ovf_warp_state()
+{
+    __shared__ unsigned int s_ovf[kOvfWarps][2];
+    return s_ovf[threadIdx.x >> 5];
+}
 
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
     ColumnBoxes cb; ScoreGeom sg;
-    unsigned int *ws;          // shared memory, this warp's stretch of the overflow list: [0] next slot, [1] end
     // the history's column box, read once when the lane takes the history (three dependent loads per deposit otherwise:
     // ncu long_scoreboard 2.2 against 0.5 in dose mode): low corner, extent, element offset of the box
     int lx, ly, lz, dx, dy, dz;
@@ -138,6 +146,7 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
             atomicAdd(cb.scratch + off + (bx + (unsigned long long)dx * (by + (unsigned long long)dy * bz)), dep);
         else {
             const int c = h.col;
+            unsigned int *ws = ovf_warp_state();
             unsigned slot = atomicAdd(ws, 1u);
             if (slot >= ws[1]) slot = atomicAdd(cb.ovf_count, 1u);
             const unsigned int v = sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3;
@@ -146,7 +155,7 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
         }
     }
     __device__ __forceinline__ void end(const Hist &) {}
-    __device__ __forceinline__ void attach(unsigned int *warp_state) { ws = warp_state; }
+    __device__ __forceinline__ void attach(int lane) { unsigned int *ws = ovf_warp_state(); if (lane < 2) ws[lane] = 0u; __syncwarp(); }
     __device__ __forceinline__ void close_stretch(unsigned int nxt, unsigned int end, int lane)
     {
         for (unsigned int i = min(nxt, end) + lane; i < end; i += 32)
@@ -154,6 +163,7 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
     }
     __device__ __forceinline__ void room(int lane)             // all 32 lanes
     {
+        unsigned int *ws = ovf_warp_state();
         const unsigned int nxt = ws[0], end = ws[1];
         if (nxt + kOvfRoom <= end || (nxt | end) == 0u) return; // enough slots left, or no outside deposit so far
         close_stretch(nxt, end, lane);
@@ -164,7 +174,7 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
         if (lane == 0) { ws[0] = base; ws[1] = base + kOvfStretch; }
         __syncwarp();
     }
-    __device__ __forceinline__ void finish(int lane) { __syncwarp(); close_stretch(ws[0], ws[1], lane); }
+    __device__ __forceinline__ void finish(int lane) { __syncwarp(); const unsigned int *ws = ovf_warp_state(); close_stretch(ws[0], ws[1], lane); }
 };
 
 struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits of each column
@@ -179,7 +189,7 @@ struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits o
         x1 = max(x1, sx); y1 = max(y1, sy); z1 = max(z1, sz);
     }
     __device__ __forceinline__ void end(const Hist &h) { if (x1 >= 0) bbox_merge(bbox + 6 * h.col, x0, y0, z0, x1, y1, z1); }
-    __device__ __forceinline__ void attach(unsigned int *) {}
+    __device__ __forceinline__ void attach(int) {}
     __device__ __forceinline__ void room(int) {}
     __device__ __forceinline__ void finish(int) {}
 };
@@ -193,7 +203,7 @@ struct ScoreArgs { float *edep; unsigned long long nvox; ColumnBoxes cb; ScoreGe
 
 template <int MODE> __device__ __forceinline__ typename ScorerOf<MODE>::type make_scorer(const ScoreArgs &a);
 template <> __device__ __forceinline__ DoseScorer make_scorer<0>(const ScoreArgs &a) { return DoseScorer{ a.edep, a.nvox, a.sg }; }
-template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { BoxScorer s; s.cb = a.cb; s.sg = a.sg; s.ws = nullptr; s.lx = s.ly = s.lz = 0; s.dx = s.dy = s.dz = 0; s.off = 0ull; return s; }
+template <> __device__ __forceinline__ BoxScorer make_scorer<1>(const ScoreArgs &a) { BoxScorer s; s.cb = a.cb; s.sg = a.sg; s.lx = s.ly = s.lz = 0; s.dx = s.dy = s.dz = 0; s.off = 0ull; return s; }
 template <> __device__ __forceinline__ BoundsScorer make_scorer<2>(const ScoreArgs &a) { BoundsScorer s; s.bbox = a.cb.bbox; s.sg = a.sg; return s; }
 
 // ------------------------------------------------------------------------------------------- S1-S7
@@ -556,10 +566,8 @@ voxel_kernel(const Ctx c, const Queue q, const float4 *__restrict__ lut_g, const
         for (int i = threadIdx.x; i < c.G.n_lut; i += blockDim.x) lut_s[i] = lut_g[i];
     __syncthreads();
     typename ScorerOf<MODE>::type sc = make_scorer<MODE>(sa);
-    __shared__ unsigned int s_ovf[kWarps][2];              // MODE 1: the warps' stretches of the overflow list (BoxScorer)
-    if (lane < 2) s_ovf[warp][lane] = 0u;
-    __syncwarp();
-    sc.attach(s_ovf[warp]);
+    static_assert(kOvfWarps == kWarps, "one stretch of the overflow list per warp of the block");
+    sc.attach(lane);                                       // MODE 1: the warp's (empty) stretch of the overflow list
     NullTracer tr;
     LaneCounters lc;
     Hist h;
