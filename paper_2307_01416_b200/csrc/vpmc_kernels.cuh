@@ -125,6 +125,33 @@ __device__ __forceinline__ unsigned int *ovf_warp_state()
     return s_ovf[threadIdx.x >> 5];
 }
 
+// The two rare paths are kept out of line: inlined, their registers cost the step loop its constants (the kernel re-loaded
+// them from the constant bank every pass: +30 instructions per step, measured).
+// (arguments by value: a reference to the scorer's ColumnBoxes would put the struct on the local stack)
+__device__ __noinline__ void ovf_append(unsigned long long *ovf_key, float *ovf_val, unsigned int *ovf_count, unsigned int ovf_cap, int *bbox,
+                                        int c, unsigned int v, float dep, int sx, int sy, int sz)
+{
+    unsigned int *ws = ovf_warp_state();
+    unsigned int slot = atomicAdd(ws, 1u);
+    if (slot >= ws[1]) slot = atomicAdd(ovf_count, 1u);
+    if (slot < ovf_cap) { ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | v; ovf_val[slot] = dep; }
+    else bbox_merge(bbox + 6 * c, sx, sy, sz, sx, sy, sz);
+}
+
+__device__ __noinline__ void ovf_reserve(unsigned long long *ovf_key, float *ovf_val, unsigned int *ovf_count, unsigned int ovf_cap, int lane)   // all 32 lanes
+{
+    unsigned int *ws = ovf_warp_state();
+    const unsigned int nxt = ws[0], end = ws[1];
+    for (unsigned int i = min(nxt, end) + lane; i < end; i += 32)
+        if (i < ovf_cap) { ovf_key[i] = kOvfSentinel; ovf_val[i] = 0.0f; }
+    unsigned int base = 0;
+    if (lane == 0) base = atomicAdd(ovf_count, kOvfStretch);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    __syncwarp();
+    if (lane == 0) { ws[0] = base; ws[1] = base + kOvfStretch; }
+    __syncwarp();
+}
+
 struct BoxScorer {             // MODE 1: per-column private box; a deposit outside it goes to the overflow list
     ColumnBoxes cb; ScoreGeom sg;
     // the history's column box, read once when the lane takes the history (three dependent loads per deposit otherwise:
@@ -144,37 +171,24 @@ struct BoxScorer {             // MODE 1: per-column private box; a deposit outs
         const int bx = sx - lx, by = sy - ly, bz = sz - lz;
         if ((unsigned)bx < (unsigned)dx && (unsigned)by < (unsigned)dy && (unsigned)bz < (unsigned)dz)
             atomicAdd(cb.scratch + off + (bx + (unsigned long long)dx * (by + (unsigned long long)dy * bz)), dep);
-        else {
-            const int c = h.col;
-            unsigned int *ws = ovf_warp_state();
-            unsigned slot = atomicAdd(ws, 1u);
-            if (slot >= ws[1]) slot = atomicAdd(cb.ovf_count, 1u);
-            const unsigned int v = sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3;
-            if (slot < cb.ovf_cap) { cb.ovf_key[slot] = ((unsigned long long)(unsigned)c << 32) | v; cb.ovf_val[slot] = dep; }
-            else bbox_merge(cb.bbox + 6 * c, sx, sy, sz, sx, sy, sz);
-        }
+        else ovf_append(cb.ovf_key, cb.ovf_val, cb.ovf_count, cb.ovf_cap, cb.bbox, h.col, sg.on ? (unsigned)(sx + sg.snx * (sy + sg.sny * sz)) : h.g3, dep, sx, sy, sz);
     }
     __device__ __forceinline__ void end(const Hist &) {}
     __device__ __forceinline__ void attach(int lane) { unsigned int *ws = ovf_warp_state(); if (lane < 2) ws[lane] = 0u; __syncwarp(); }
-    __device__ __forceinline__ void close_stretch(unsigned int nxt, unsigned int end, int lane)
-    {
-        for (unsigned int i = min(nxt, end) + lane; i < end; i += 32)
-            if (i < cb.ovf_cap) { cb.ovf_key[i] = kOvfSentinel; cb.ovf_val[i] = 0.0f; }
-    }
     __device__ __forceinline__ void room(int lane)             // all 32 lanes
     {
-        unsigned int *ws = ovf_warp_state();
+        const unsigned int *ws = ovf_warp_state();
         const unsigned int nxt = ws[0], end = ws[1];
         if (nxt + kOvfRoom <= end || (nxt | end) == 0u) return; // enough slots left, or no outside deposit so far
-        close_stretch(nxt, end, lane);
-        unsigned int base = 0;
-        if (lane == 0) base = atomicAdd(cb.ovf_count, kOvfStretch);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        __syncwarp();
-        if (lane == 0) { ws[0] = base; ws[1] = base + kOvfStretch; }
-        __syncwarp();
+        ovf_reserve(cb.ovf_key, cb.ovf_val, cb.ovf_count, cb.ovf_cap, lane);
     }
-    __device__ __forceinline__ void finish(int lane) { __syncwarp(); const unsigned int *ws = ovf_warp_state(); close_stretch(ws[0], ws[1], lane); }
+    __device__ __forceinline__ void finish(int lane)           // closes the stretch the warp still holds
+    {
+        __syncwarp();
+        const unsigned int *ws = ovf_warp_state();
+        for (unsigned int i = min(ws[0], ws[1]) + lane; i < ws[1]; i += 32)
+            if (i < cb.ovf_cap) { cb.ovf_key[i] = kOvfSentinel; cb.ovf_val[i] = 0.0f; }
+    }
 };
 
 struct BoundsScorer {          // MODE 2 (pilot): bounding box of the deposits of each column
